@@ -1,0 +1,192 @@
+/*
+ * psl.h -- C-ABI of the B200 phase-space source library (libpsl_b200.so).
+ *
+ * The data-parallel hot path of Townson et al., "GPU-based Monte Carlo radiotherapy dose
+ * calculation using phase-space sources" (arXiv 1302.1861; PAPER.md = /root/reference/PAPER.md):
+ * packed linac phase-space records are loaded in chunks (sec. 2.3.3), decoded,
+ * tested against the secondary-collimator (jaw) model (sec. 2.2), weighted by the
+ * fluence map, culled by the phase-space-let (PSL) region of interest
+ * and bucketed by particle type, energy bin and position bin
+ * into contiguous structure-of-arrays batches, "one energy division before proceeding to the
+ * next".  Every step runs in CUDA kernels for sm_100a; there is no CPU path.
+ *
+ * Conventions
+ *   - Plain C, no torch types.  Every pointer says HOST or DEVICE.
+ *   - Beam's-eye-view frame: beam axis +z through (0,0); lengths in cm, energies in MeV.
+ *   - All work is enqueued on psl_config.stream (plus one internal copy stream ordered to it with
+ *     events).  Calls return once the work is enqueued unless stated otherwise.
+ *   - Errors are return codes; nothing aborts, nothing throws, and a call that fails leaves the
+ *     context as it was before the call.  psl_last_error() gives a one-line description.
+ *   - A context is not thread-safe.  Total records per context < 2^32.
+ *
+ * Arithmetic contract: every expression that decides a bin, a key, the jaw
+ * predicate or a map pixel is evaluated in fp32, one IEEE-754 round-to-nearest operation at a
+ * time, with no FMA contraction; outputs E, x, y, u, v are bit copies of the inputs.
+ */
+#ifndef PSL_H
+#define PSL_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct psl_ctx psl_ctx; /* opaque; one per phase-space */
+
+typedef enum {
+    PSL_OK = 0,
+    PSL_ERR_ARG = 1,      /* bad argument or configuration */
+    PSL_ERR_STATE = 2,    /* call out of order (e.g. psl_get_batch before psl_build_batches) */
+    PSL_ERR_CAPACITY = 3, /* workspace too small, or more records / chunks than configured */
+    PSL_ERR_GEOMETRY = 4, /* planes out of order */
+    PSL_ERR_CUDA = 5      /* a CUDA runtime call failed; see psl_last_error() */
+} psl_status;
+
+enum { PSL_MODE_ONTHEFLY = 0, /* paper methods 1 and 2: sort on the fly by (type, energy) */
+       PSL_MODE_INDEX = 1 };  /* paper method 3: pre-sorted PSL index, per-beam ROI selection */
+enum { PSL_EBIN_LINEAR = 0,   /* n_ebins uniform bins on [e_min, e_max] */
+       PSL_EBIN_EDGES = 1 };  /* caller-supplied ascending edge table with n_ebins+1 entries */
+enum { PSL_MEM_PAGEABLE = 0, PSL_MEM_PINNED = 1, PSL_MEM_DEVICE = 2 };
+enum { PSL_OUT_PROJ = 1u,           /* also write xp, yp: the position at the fluence-map plane */
+       PSL_DROP_ZERO_WEIGHT = 2u }; /* drop survivors whose final weight is exactly 0 (default: keep) */
+
+/* One phase-space particle: 28 bytes, packed, little-endian.  type: 0 photon, 1 electron, 2 positron.
+ * (u, v) are direction cosines; the third one is w = sqrt(1 - u^2 - v^2) > 0 (always downstream). */
+typedef struct {
+    int32_t type;
+    float E, x, y, u, v, wt;
+} psl_record;
+
+/* z of each plane along the beam axis.  Must satisfy z_src < z_plane <= z_jaw_x, z_jaw_y, z_map <= z_iso. */
+typedef struct {
+    float z_src, z_plane, z_jaw_x, z_jaw_y, z_map, z_iso;
+} psl_geometry;
+
+typedef struct {
+    uint32_t struct_size; /* sizeof(psl_config), checked */
+    int32_t mode;         /* PSL_MODE_* */
+    int32_t n_types;      /* 3, or 2 = electrons and positrons share a division */
+    int32_t ebin_mode;    /* PSL_EBIN_* */
+    int32_t n_ebins;
+    float e_min, e_max;
+    const float* e_edges; /* HOST, n_ebins+1 ascending floats, copied by psl_create; NULL in linear mode */
+    int32_t n_xbins, n_ybins; /* 1 x 1 = no position bins (methods 1 and 2) */
+    float x_min, y_min, dx, dy; /* grid origin and bin size at z_plane; x_min/dx and y_min/dy must be integers */
+    psl_geometry geom;
+    uint64_t max_records;      /* capacity: total records loaded between resets */
+    uint64_t max_host_records; /* of those, how many may arrive from HOST memory (device landing zone) */
+    uint64_t max_beam_records; /* INDEX mode: most records one beam's ROI may select; 0 = max_records */
+    uint32_t max_chunks;       /* most psl_load_chunk calls between resets; 0 = 4096 */
+    uint32_t flags;            /* PSL_OUT_PROJ | PSL_DROP_ZERO_WEIGHT */
+    int32_t device;            /* CUDA device ordinal */
+    void* stream;              /* cudaStream_t owned by the caller (NULL = default stream) */
+    void* workspace;           /* DEVICE memory owned by the caller, 256-byte aligned */
+    uint64_t workspace_bytes;  /* >= psl_workspace_bytes(cfg) */
+} psl_config;
+
+/* One treatment field.  NULL beam = method 1: no jaws, no map, weight untouched. */
+typedef struct {
+    int32_t has_jaws;
+    float jaw_x1, jaw_x2, jaw_y1, jaw_y2; /* aperture [x1,x2) x [y1,y2) as projected at z_iso */
+    const float* fluence;                 /* DEVICE, map_ny x map_nx row-major fp32, or NULL = no map */
+    int32_t map_nx, map_ny;
+    float map_x0, map_y0, map_dx, map_dy; /* pixel grid at z_map; map_x0/map_dx, map_y0/map_dy integers */
+    int32_t has_roi;                      /* INDEX mode only */
+    float roi_x1, roi_x2, roi_y1, roi_y2; /* rectangle at z_plane */
+    float mu_weight;                      /* MU_i / MU_total */
+    float gantry_deg, coll_deg, couch_deg; /* carried as metadata only */
+} psl_beam;
+
+/* Every record loaded is counted in exactly one of the six n_* classes below (tested in this order). */
+typedef struct {
+    uint64_t n_in;
+    uint64_t n_invalid;      /* type not in {0,1,2}, a non-finite field, E <= 0, or u^2+v^2 >= 1 */
+    uint64_t n_outside_grid; /* valid, but outside the position grid */
+    uint64_t n_roi_skipped;  /* in a position bin the ROI does not select (their records are never read) */
+    uint64_t n_jaw_rejected; /* hit a jaw */
+    uint64_t n_zero_weight;  /* dropped because of PSL_DROP_ZERO_WEIGHT */
+    uint64_t n_survivors;
+    double sum_wt_in;      /* sum of wt over valid records */
+    double sum_wt_indexed; /* sum of wt over valid records inside the grid */
+    double sum_wt_out;     /* sum of final weights over survivors */
+} psl_stats;
+
+/* A contiguous run of output slots.  All pointers are DEVICE, BORROWED from the workspace and valid
+ * until the next psl_build_batches / psl_reset / psl_destroy on the context.  Each array pointer
+ * addresses slot `first` (i.e. element 0 of the batch).  Slots are ordered by key
+ * key = ((t * n_ebins + ie) * n_ybins + iy) * n_xbins + ix, input order inside a key. */
+typedef struct {
+    uint32_t first;  /* absolute slot of the first element */
+    uint32_t count;
+    const float *E, *x, *y, *u, *v; /* bit copies of the record fields */
+    const float* w;                 /* sqrt(1-u^2-v^2); NULL for the bare index */
+    const float* wt;                /* final weight (wt * F) * mu_weight; the record's wt for the bare index */
+    const float *xp, *yp;           /* position at z_map; NULL unless PSL_OUT_PROJ */
+    const uint32_t* src_index;      /* load-order index of the record */
+    const uint32_t* bin_offsets;    /* n_bins+1 ABSOLUTE slot offsets of this batch's position bins */
+    uint32_t n_bins;                /* n_xbins * n_ybins */
+} psl_batch;
+
+/* Bytes of device workspace a configuration needs (cfg->workspace* ignored).  0 on a bad configuration. */
+uint64_t psl_workspace_bytes(const psl_config* cfg);
+
+/* Validate, copy the configuration, carve the workspace.  May allocate small pinned HOST buffers and one
+ * CUDA stream + a few events.  *out is untouched on error (the reason is then readable with
+ * psl_last_error(NULL)). */
+psl_status psl_create(const psl_config* cfg, psl_ctx** out);
+
+/* Append n records ("particle data are copied in chunks").  `records` is HOST pageable, HOST
+ * pinned or DEVICE memory per mem_kind.  n must be a multiple of 4 except for the last chunk before a
+ * build.  HOST chunks are copied on the internal copy stream into the workspace (pageable ones through two
+ * pinned staging buffers); the source must stay untouched until psl_wait_loads() or any later
+ * synchronising call returns.  DEVICE chunks are BORROWED, not copied: they must stay valid and unchanged
+ * until the next psl_reset/psl_destroy (ONTHEFLY) or until the index is finalised (INDEX).  In INDEX mode
+ * the chunk's keys are counted as soon as it lands, overlapping the next chunk's transfer. */
+psl_status psl_load_chunk(psl_ctx* ctx, const void* records, uint64_t n, int32_t mem_kind);
+
+/* Block the HOST until every chunk loaded so far has left its source buffer. */
+psl_status psl_wait_loads(psl_ctx* ctx);
+
+/* ONTHEFLY: decode every loaded record, apply the beam's jaws / fluence map / MU weight, histogram,
+ * scan and stably scatter the survivors by (type, energy[, position]) key.  May be called again with a
+ * different beam.  INDEX: the first call finalises the index (sort of all valid in-grid records by the
+ * full key; synchronises once); with beam != NULL it then builds that beam's batches from the index,
+ * reading only the position bins the ROI selects.  beam == NULL exposes the index itself.
+ * stats may be NULL; if not, the call synchronises the stream and fills it. */
+psl_status psl_build_batches(psl_ctx* ctx, const psl_beam* beam, psl_stats* stats);
+
+/* Synchronise and report the statistics of the latest build. */
+psl_status psl_get_stats(psl_ctx* ctx, psl_stats* stats);
+
+/* The (type division t, energy bin ie) batch of the latest build; t = ie = -1 gives the whole output as
+ * one run.  Waits for the (tiny) batch-offset copy of that build, not for the whole stream. */
+psl_status psl_get_batch(psl_ctx* ctx, int32_t t, int32_t ie, psl_batch* out);
+
+/* DEVICE pointers to counts[K] and offsets[K+1] of the latest build. */
+psl_status psl_get_tables(psl_ctx* ctx, const uint32_t** counts, const uint32_t** offsets, uint32_t* n_keys);
+
+/* HOST only.  ROI rectangle {x1, x2, y1, y2} at z_plane for a beam's jaws (Fig. 1 caption
+ * PAPER.md:196): per axis, the line from the field centre at z_iso through the jaw edge at the jaw plane,
+ * extended to z_plane, widened by `margin`.  PSL_ERR_GEOMETRY unless z_jaw < z_iso on both axes. */
+psl_status psl_roi_from_jaws(const psl_geometry* g, const psl_beam* beam, float margin, float roi_out[4]);
+
+/* HOST only.  The inclusive rectangle {rx0, rx1, ry0, ry1} of position bins with positive-area overlap with
+ * the beam's ROI ("any portion of its area"); rx0 > rx1 or ry0 > ry1 when nothing is selected. */
+psl_status psl_roi_bins(const psl_ctx* ctx, const psl_beam* beam, int32_t bins_out[4]);
+
+/* Forget all chunks and results (keeps the configuration and workspace). */
+psl_status psl_reset(psl_ctx* ctx);
+
+void psl_destroy(psl_ctx* ctx);
+
+/* Last error of this context (ctx == NULL: of the last failed psl_create / context-free call on this thread). */
+const char* psl_last_error(const psl_ctx* ctx);
+
+/* Number of kernels this context has launched since creation (for bench.py's gpu_launches). */
+uint64_t psl_kernel_launches(const psl_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PSL_H */

@@ -1,0 +1,903 @@
+// psl_api.cu -- host side of libpsl_b200.so: the C-ABI of include/psl.h.
+//
+// Argument checking, workspace carving, stream/event plumbing and kernel launches only; every step of the
+// hot path runs in the kernels of psl_partition.cuh / psl_beam.cuh.  There is no CPU fallback: without a
+// CUDA device every call that needs one returns PSL_ERR_CUDA.
+#include "../../include/psl.h"
+
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+#include <vector>
+
+#include "psl_beam.cuh"
+#include "psl_device.cuh"
+#include "psl_partition.cuh"
+
+using namespace psl;
+
+namespace {
+
+thread_local char g_err[256] = "";
+
+constexpr uint64_t kAlign = 256;
+constexpr uint64_t kStageBytes = 32ull << 20;  // pinned staging buffers for pageable sources (two of them)
+
+struct Layout {
+    uint64_t total = 0;
+    uint64_t raw = 0, tiles = 0, tstats = 0, scan_sums = 0, scalars = 0, edges = 0, stats = 0, batch_off = 0;
+    // ONTHEFLY
+    uint64_t table = 0, out[10] = {0}, offsets = 0, counts = 0;
+    // INDEX
+    uint64_t table_a = 0, table_b = 0, aos = 0, hi16 = 0, idx[7] = {0}, keyfull = 0, idx_offsets = 0, idx_counts = 0,
+             idx_batch_off = 0;
+    uint64_t seg = 0, beam_out[10] = {0}, beam_keys = 0, beam_offsets = 0, beam_counts = 0, lookback = 0, bstats = 0,
+             beam_stats = 0;
+};
+
+struct Derived {
+    uint32_t K = 0, n_batches = 0, n_pos = 0;
+    uint32_t lo_bits = 0, B_lo = 0, B_hi = 0;
+    uint32_t tiles_cap = 0, tiles_b_cap = 0, max_chunks = 0;
+    uint64_t max_beam = 0;
+    uint32_t max_seg = 0;
+    uint32_t scan_blocks_cap = 0;
+};
+
+void set_err(char* dst, const char* fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(dst, 256, fmt, ap);
+    va_end(ap);
+}
+
+bool is_integer_ratio(float a, float d, int32_t* out)
+{
+    double r = (double)a / (double)d;
+    double n = nearbyint(r);
+    if (fabs(r - n) > 1e-6 * fmax(1.0, fabs(r))) return false;
+    if (fabs(n) > 1e9) return false;
+    *out = (int32_t)n;
+    return true;
+}
+
+psl_status check_geometry(const psl_geometry& g, char* err)
+{
+    bool ok = isfinite(g.z_src) && isfinite(g.z_plane) && isfinite(g.z_jaw_x) && isfinite(g.z_jaw_y) && isfinite(g.z_map) &&
+              isfinite(g.z_iso) && g.z_src < g.z_plane && g.z_plane <= g.z_jaw_x && g.z_plane <= g.z_jaw_y &&
+              g.z_plane <= g.z_map && g.z_jaw_x <= g.z_iso && g.z_jaw_y <= g.z_iso && g.z_map <= g.z_iso;
+    if (!ok) {
+        set_err(err, "geometry: need z_src < z_plane <= z_jaw_x, z_jaw_y, z_map <= z_iso");
+        return PSL_ERR_GEOMETRY;
+    }
+    return PSL_OK;
+}
+
+psl_status derive(const psl_config* c, Derived* d, char* err)
+{
+    if (!c) { set_err(err, "config is NULL"); return PSL_ERR_ARG; }
+    if (c->struct_size != sizeof(psl_config)) { set_err(err, "config.struct_size %u != %zu", c->struct_size, sizeof(psl_config)); return PSL_ERR_ARG; }
+    if (c->mode != PSL_MODE_ONTHEFLY && c->mode != PSL_MODE_INDEX) { set_err(err, "config.mode"); return PSL_ERR_ARG; }
+    if (c->n_types != 2 && c->n_types != 3) { set_err(err, "config.n_types must be 2 or 3"); return PSL_ERR_ARG; }
+    if (c->n_ebins < 1 || c->n_ebins > 1024) { set_err(err, "config.n_ebins must be 1..1024"); return PSL_ERR_ARG; }
+    if (c->ebin_mode == PSL_EBIN_LINEAR) {
+        if (!(isfinite(c->e_min) && isfinite(c->e_max) && c->e_max > c->e_min)) { set_err(err, "config: need e_max > e_min"); return PSL_ERR_ARG; }
+    } else if (c->ebin_mode == PSL_EBIN_EDGES) {
+        if (!c->e_edges) { set_err(err, "config.e_edges is NULL in edge mode"); return PSL_ERR_ARG; }
+        for (int i = 0; i < c->n_ebins; ++i)
+            if (!(c->e_edges[i] < c->e_edges[i + 1])) { set_err(err, "config.e_edges must be strictly ascending"); return PSL_ERR_ARG; }
+    } else { set_err(err, "config.ebin_mode"); return PSL_ERR_ARG; }
+    if (c->n_xbins < 1 || c->n_ybins < 1 || c->n_xbins > 4096 || c->n_ybins > 4096) { set_err(err, "config.n_xbins/n_ybins must be 1..4096"); return PSL_ERR_ARG; }
+    uint64_t n_pos = (uint64_t)c->n_xbins * (uint64_t)c->n_ybins;
+    if (n_pos > 1 || c->mode == PSL_MODE_INDEX) {
+        int32_t t;
+        if (!(c->dx > 0 && c->dy > 0 && isfinite(c->dx) && isfinite(c->dy))) { set_err(err, "config: dx, dy must be positive"); return PSL_ERR_ARG; }
+        if (!is_integer_ratio(c->x_min, c->dx, &t) || !is_integer_ratio(c->y_min, c->dy, &t)) { set_err(err, "config: x_min/dx and y_min/dy must be integers"); return PSL_ERR_ARG; }
+    }
+    psl_status gs = check_geometry(c->geom, err);
+    if (gs != PSL_OK) return gs;
+    uint64_t K = (uint64_t)c->n_types * c->n_ebins * n_pos;
+    if (c->max_records == 0 || c->max_records >= (1ull << 32)) { set_err(err, "config.max_records must be 1..2^32-1"); return PSL_ERR_ARG; }
+    if (c->max_host_records > c->max_records) { set_err(err, "config.max_host_records > max_records"); return PSL_ERR_ARG; }
+    d->K = (uint32_t)K;
+    d->n_pos = (uint32_t)n_pos;
+    d->n_batches = (uint32_t)(c->n_types * c->n_ebins);
+    d->max_chunks = c->max_chunks ? c->max_chunks : 4096u;
+    uint64_t tiles_cap = (c->max_records + kTile - 1) / kTile + d->max_chunks;
+    d->tiles_b_cap = (uint32_t)((c->max_records + kTile - 1) / kTile);
+    if (c->mode == PSL_MODE_ONTHEFLY) {
+        if (K > kMaxBuckets) { set_err(err, "ONTHEFLY mode handles at most %d keys (got %llu); use PSL_MODE_INDEX", kMaxBuckets, (unsigned long long)K); return PSL_ERR_ARG; }
+        if (K * tiles_cap >= (1ull << 32)) { set_err(err, "keys x tiles overflows 32 bits"); return PSL_ERR_CAPACITY; }
+    } else {
+        if (K > (uint64_t)kMaxBuckets * kMaxBuckets) { set_err(err, "INDEX mode handles at most %d keys", kMaxBuckets * kMaxBuckets); return PSL_ERR_ARG; }
+        uint32_t bits = 0;
+        while ((1ull << bits) < K) ++bits;  // K <= 2^bits
+        uint32_t lo = (bits + 1) / 2;
+        while ((((K - 1) >> lo) + 1) > (uint64_t)kMaxBuckets) ++lo;
+        d->lo_bits = lo;
+        d->B_lo = (uint32_t)((K < (1ull << lo)) ? K : (1ull << lo));
+        if (d->B_lo < 1) d->B_lo = 1;
+        d->B_hi = (uint32_t)(((K - 1) >> lo) + 1);
+        if ((uint64_t)d->B_lo * tiles_cap >= (1ull << 32) || (uint64_t)d->B_hi * d->tiles_b_cap >= (1ull << 32)) { set_err(err, "buckets x tiles overflows 32 bits"); return PSL_ERR_CAPACITY; }
+        d->max_beam = c->max_beam_records ? c->max_beam_records : c->max_records;
+        if (d->max_beam > c->max_records) d->max_beam = c->max_records;
+        d->max_seg = d->n_batches * (uint32_t)c->n_ybins;
+    }
+    d->tiles_cap = (uint32_t)tiles_cap;
+    uint64_t Lmax = c->mode == PSL_MODE_ONTHEFLY ? K * tiles_cap
+                                                  : ((uint64_t)d->B_lo * tiles_cap > (uint64_t)d->B_hi * d->tiles_b_cap
+                                                         ? (uint64_t)d->B_lo * tiles_cap
+                                                         : (uint64_t)d->B_hi * d->tiles_b_cap);
+    d->scan_blocks_cap = (uint32_t)((Lmax + kScanBlock - 1) / kScanBlock);
+    return PSL_OK;
+}
+
+uint64_t take(uint64_t* cur, uint64_t bytes)
+{
+    uint64_t at = *cur;
+    *cur = (at + bytes + kAlign - 1) / kAlign * kAlign;
+    return at;
+}
+
+void plan(const psl_config* c, const Derived& d, Layout* L)
+{
+    uint64_t cur = 0;
+    const uint64_t N = c->max_records;
+    const bool proj = (c->flags & PSL_OUT_PROJ) != 0;
+    L->raw = take(&cur, c->max_host_records * kRecBytes);
+    L->tiles = take(&cur, (uint64_t)d.tiles_cap * sizeof(TileDesc));
+    L->tstats = take(&cur, (uint64_t)d.tiles_cap * sizeof(TileStats));
+    L->scan_sums = take(&cur, (uint64_t)(d.scan_blocks_cap + 1) * 4);
+    L->scalars = take(&cur, 64);
+    L->edges = take(&cur, (uint64_t)(c->n_ebins + 1) * 4);
+    L->stats = take(&cur, sizeof(DevStats));
+    L->batch_off = take(&cur, (uint64_t)(d.n_batches + 1) * 4);
+    if (c->mode == PSL_MODE_ONTHEFLY) {
+        L->table = take(&cur, (uint64_t)d.K * d.tiles_cap * 4);
+        for (int i = 0; i < 10; ++i) L->out[i] = ((i == 7 || i == 8) && !proj) ? 0 : take(&cur, N * 4);
+        L->offsets = take(&cur, (uint64_t)(d.K + 1) * 4);
+        L->counts = take(&cur, (uint64_t)d.K * 4);
+    } else {
+        L->table_a = take(&cur, (uint64_t)d.B_lo * d.tiles_cap * 4);
+        L->table_b = take(&cur, (uint64_t)d.B_hi * d.tiles_b_cap * 4);
+        L->aos = take(&cur, N * 32);
+        L->hi16 = take(&cur, N * 2);
+        for (int i = 0; i < 7; ++i) L->idx[i] = take(&cur, N * 4);
+        L->keyfull = take(&cur, N * 4);
+        L->idx_offsets = take(&cur, (uint64_t)(d.K + 1) * 4);
+        L->idx_counts = take(&cur, (uint64_t)d.K * 4);
+        L->idx_batch_off = take(&cur, (uint64_t)(d.n_batches + 1) * 4);
+        L->seg = take(&cur, (uint64_t)(3 * d.max_seg + 1) * 4);
+        for (int i = 0; i < 10; ++i) L->beam_out[i] = ((i == 7 || i == 8) && !proj) ? 0 : take(&cur, d.max_beam * 4);
+        L->beam_keys = take(&cur, d.max_beam * 4);
+        L->beam_offsets = take(&cur, (uint64_t)(d.K + 1) * 4);
+        L->beam_counts = take(&cur, (uint64_t)d.K * 4);
+        uint64_t bt = (d.max_beam + kTile - 1) / kTile + 1;
+        L->lookback = take(&cur, bt * 8);
+        L->bstats = take(&cur, bt * sizeof(BeamTileStats));
+        L->beam_stats = take(&cur, sizeof(DevBeamStats));
+    }
+    L->total = cur;
+}
+
+enum ResultKind { RES_NONE = 0, RES_OTF = 1, RES_INDEX = 2, RES_BEAM = 3 };
+
+}  // namespace
+
+struct psl_ctx {
+    psl_config cfg;
+    Derived d;
+    Layout L;
+    DevGrid grid;
+    std::vector<float> edges;
+    uint8_t* ws = nullptr;
+    cudaStream_t stream = nullptr, copy_stream = nullptr;
+    cudaEvent_t ev_chunk = nullptr, ev_main = nullptr, ev_batch = nullptr, ev_seg = nullptr, ev_stage[2] = {nullptr, nullptr};
+    void* h_stage[2] = {nullptr, nullptr};
+    int stage_next = 0;
+    // pinned host mirrors
+    uint32_t* h_batch_off = nullptr;   // n_batches+1
+    uint32_t* h_idx_offsets = nullptr; // K+1 (INDEX)
+    uint32_t* h_seg = nullptr;         // 3*max_seg+1
+    DevStats* h_stats = nullptr;
+    DevBeamStats* h_beam_stats = nullptr;
+    uint32_t* h_scalars = nullptr;
+    bool seg_pending = false;
+    // state
+    uint64_t n_records = 0, n_host_records = 0;
+    uint32_t n_tiles = 0, n_chunks = 0;
+    bool ragged = false;  // a chunk with n % 4 != 0 was loaded: no more chunks may follow
+    bool indexed = false;
+    int result = RES_NONE;
+    DevStats idx_stats = {};
+    uint64_t n_idx = 0, last_M = 0;
+    uint64_t launches = 0;
+    char err[256] = "";
+};
+
+namespace {
+
+#define CU(call)                                                                                           \
+    do {                                                                                                   \
+        cudaError_t e_ = (call);                                                                           \
+        if (e_ != cudaSuccess) {                                                                           \
+            set_err(ctx->err, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
+            return PSL_ERR_CUDA;                                                                           \
+        }                                                                                                  \
+    } while (0)
+
+#define LAUNCHED()                                    \
+    do {                                              \
+        ctx->launches += 1;                           \
+        CU(cudaGetLastError());                       \
+    } while (0)
+
+template <typename T>
+T* at(psl_ctx* ctx, uint64_t off) { return reinterpret_cast<T*>(ctx->ws + off); }
+
+uint32_t* scalar(psl_ctx* ctx, int i) { return at<uint32_t>(ctx, ctx->L.scalars) + i; }
+enum { SC_TOTAL = 0, SC_NIDX = 1, SC_TILE_COUNTER = 2, SC_BEAM_NSURV = 3 };
+
+DevGrid make_grid(const psl_config& c, const Derived& d, const float* dev_edges)
+{
+    DevGrid g;
+    g.n_types = c.n_types;
+    g.ebin_mode = c.ebin_mode;
+    g.n_ebins = c.n_ebins;
+    g.e_min = c.e_min;
+    g.dE = c.ebin_mode == PSL_EBIN_LINEAR ? (float)(((double)c.e_max - (double)c.e_min) / (double)c.n_ebins) : 1.0f;
+    g.e_edges = dev_edges;
+    g.has_pos = d.n_pos > 1;
+    g.n_xbins = c.n_xbins;
+    g.n_ybins = c.n_ybins;
+    g.ix0 = g.iy0 = 0;
+    g.inv_dx = g.inv_dy = 1.0f;
+    if (g.has_pos) {
+        is_integer_ratio(c.x_min, c.dx, &g.ix0);
+        is_integer_ratio(c.y_min, c.dy, &g.iy0);
+        g.inv_dx = (float)(1.0 / (double)c.dx);
+        g.inv_dy = (float)(1.0 / (double)c.dy);
+    }
+    g.n_pos = d.n_pos;
+    return g;
+}
+
+float edge_at_jaw_plane(float edge_iso, float z_jaw, const psl_geometry& g)
+{
+    return (float)((double)edge_iso * ((double)z_jaw - (double)g.z_src) / ((double)g.z_iso - (double)g.z_src));
+}
+
+psl_status make_beam(const psl_ctx* ctx, const psl_beam* b, DevBeam* out, char* err)
+{
+    const psl_config& c = ctx->cfg;
+    DevBeam v;
+    memset(&v, 0, sizeof v);
+    v.dzM = c.geom.z_map - c.geom.z_plane;
+    v.mu = 1.0f;
+    v.out_proj = (c.flags & PSL_OUT_PROJ) ? 1u : 0u;
+    if (b) {
+        v.has_beam = 1;
+        if (!isfinite(b->mu_weight)) { set_err(err, "beam.mu_weight is not finite"); return PSL_ERR_ARG; }
+        v.mu = b->mu_weight;
+        v.drop_zero = (c.flags & PSL_DROP_ZERO_WEIGHT) ? 1u : 0u;
+        if (b->has_jaws) {
+            if (!(b->jaw_x1 <= b->jaw_x2 && b->jaw_y1 <= b->jaw_y2)) { set_err(err, "beam: jaw edges out of order"); return PSL_ERR_ARG; }
+            v.has_jaws = 1;
+            v.X1 = edge_at_jaw_plane(b->jaw_x1, c.geom.z_jaw_x, c.geom);
+            v.X2 = edge_at_jaw_plane(b->jaw_x2, c.geom.z_jaw_x, c.geom);
+            v.Y1 = edge_at_jaw_plane(b->jaw_y1, c.geom.z_jaw_y, c.geom);
+            v.Y2 = edge_at_jaw_plane(b->jaw_y2, c.geom.z_jaw_y, c.geom);
+            v.dzJx = c.geom.z_jaw_x - c.geom.z_plane;
+            v.dzJy = c.geom.z_jaw_y - c.geom.z_plane;
+        }
+        if (b->fluence) {
+            if (b->map_nx < 1 || b->map_ny < 1 || !(b->map_dx > 0) || !(b->map_dy > 0)) { set_err(err, "beam: bad fluence map shape"); return PSL_ERR_ARG; }
+            if (!is_integer_ratio(b->map_x0, b->map_dx, &v.px0) || !is_integer_ratio(b->map_y0, b->map_dy, &v.py0)) { set_err(err, "beam: map_x0/map_dx and map_y0/map_dy must be integers"); return PSL_ERR_ARG; }
+            v.has_map = 1;
+            v.fluence = b->fluence;
+            v.map_nx = b->map_nx;
+            v.map_ny = b->map_ny;
+            v.inv_mdx = (float)(1.0 / (double)b->map_dx);
+            v.inv_mdy = (float)(1.0 / (double)b->map_dy);
+        }
+        if (b->has_roi) {
+            if (c.mode != PSL_MODE_INDEX) { set_err(err, "beam.has_roi needs PSL_MODE_INDEX"); return PSL_ERR_ARG; }
+            if (!(isfinite(b->roi_x1) && isfinite(b->roi_x2) && isfinite(b->roi_y1) && isfinite(b->roi_y2))) { set_err(err, "beam: ROI is not finite"); return PSL_ERR_ARG; }
+        }
+    }
+    *out = v;
+    return PSL_OK;
+}
+
+// bins c of [origin + c d, origin + (c+1) d) with positive-length overlap with (lo, hi)
+void select_axis(double origin, double d, int n, double lo, double hi, int* first, int* last)
+{
+    int f = (int)fmax(0.0, floor((lo - origin) / d) - 1.0);
+    if (!(lo - origin > 0)) f = 0;
+    while (f < n && !(origin + (double)(f + 1) * d > lo)) ++f;
+    double lg = floor((hi - origin) / d) + 1.0;
+    int l = lg >= (double)n ? n - 1 : (lg < 0 ? -1 : (int)lg);
+    while (l >= 0 && !(origin + (double)l * d < hi)) --l;
+    *first = f;
+    *last = l;
+}
+
+void roi_bins(const psl_config& c, const psl_beam* b, int32_t out[4])
+{
+    if (!b || !b->has_roi) {
+        out[0] = 0; out[1] = c.n_xbins - 1; out[2] = 0; out[3] = c.n_ybins - 1;
+        return;
+    }
+    select_axis(c.x_min, c.dx, c.n_xbins, b->roi_x1, b->roi_x2, &out[0], &out[1]);
+    select_axis(c.y_min, c.dy, c.n_ybins, b->roi_y1, b->roi_y2, &out[2], &out[3]);
+}
+
+template <typename Kern>
+cudaError_t allow_smem(Kern k, uint32_t bytes)
+{
+    return cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
+
+// exclusive scan of table (virtual order bucket-major, tile-minor); grand total -> *total_dev
+psl_status run_scan(psl_ctx* ctx, uint32_t* table, uint32_t B, uint32_t n_tiles, uint32_t stride, uint32_t* total_dev)
+{
+    uint64_t L64 = (uint64_t)B * n_tiles;
+    uint32_t L = (uint32_t)L64;
+    uint32_t nb = (uint32_t)((L64 + kScanBlock - 1) / kScanBlock);
+    uint32_t* sums = at<uint32_t>(ctx, ctx->L.scan_sums);
+    k_scan_reduce<<<nb, kScanThreads, 0, ctx->stream>>>(table, n_tiles, stride, L, sums);
+    LAUNCHED();
+    k_scan_sums<<<1, 1024, 0, ctx->stream>>>(sums, nb, total_dev);
+    LAUNCHED();
+    k_scan_apply<<<nb, kScanThreads, 0, ctx->stream>>>(table, n_tiles, stride, L, sums);
+    LAUNCHED();
+    return PSL_OK;
+}
+
+SoAOut soa_out(psl_ctx* ctx, const uint64_t off[10])
+{
+    SoAOut o;
+    o.E = at<float>(ctx, off[0]); o.x = at<float>(ctx, off[1]); o.y = at<float>(ctx, off[2]);
+    o.u = at<float>(ctx, off[3]); o.v = at<float>(ctx, off[4]); o.w = at<float>(ctx, off[5]);
+    o.wt = at<float>(ctx, off[6]);
+    o.xp = at<float>(ctx, off[7]); o.yp = at<float>(ctx, off[8]);
+    o.src = at<uint32_t>(ctx, off[9]);
+    return o;
+}
+
+psl_status build_onthefly(psl_ctx* ctx, const DevBeam& bm)
+{
+    const Derived& d = ctx->d;
+    const Layout& L = ctx->L;
+    uint32_t* table = at<uint32_t>(ctx, L.table);
+    uint32_t* offsets = at<uint32_t>(ctx, L.offsets);
+    uint32_t* counts = at<uint32_t>(ctx, L.counts);
+    uint32_t* batch_off = at<uint32_t>(ctx, L.batch_off);
+    DevStats* stats = at<DevStats>(ctx, L.stats);
+    const uint32_t nt = ctx->n_tiles;
+    if (nt == 0) {
+        CU(cudaMemsetAsync(offsets, 0, (uint64_t)(d.K + 1) * 4, ctx->stream));
+        CU(cudaMemsetAsync(counts, 0, (uint64_t)d.K * 4, ctx->stream));
+        CU(cudaMemsetAsync(batch_off, 0, (uint64_t)(d.n_batches + 1) * 4, ctx->stream));
+        CU(cudaMemsetAsync(stats, 0, sizeof(DevStats), ctx->stream));
+    } else {
+        const TileDesc* tiles = at<TileDesc>(ctx, L.tiles);
+        TileStats* ts = at<TileStats>(ctx, L.tstats);
+        uint32_t sm_count = tile_smem_bytes(kTile * kRecBytes, d.K, ctx->cfg.n_ebins + 1, false, false);
+        uint32_t sm_scatter = tile_smem_bytes(kTile * kRecBytes, d.K, ctx->cfg.n_ebins + 1, true, true);
+        k_count_raw<false><<<nt, kThreads, sm_count, ctx->stream>>>(tiles, 0, ctx->grid, bm, d.K, 0, table, d.tiles_cap, ts);
+        LAUNCHED();
+        psl_status s = run_scan(ctx, table, d.K, nt, d.tiles_cap, scalar(ctx, SC_TOTAL));
+        if (s != PSL_OK) return s;
+        k_offsets_from_table<<<(d.K + 1 + 255) / 256, 256, 0, ctx->stream>>>(table, d.tiles_cap, d.K, scalar(ctx, SC_TOTAL),
+                                                                           offsets, counts, d.n_pos, d.n_batches, batch_off);
+        LAUNCHED();
+        k_scatter_otf<<<nt, kThreads, sm_scatter, ctx->stream>>>(tiles, ctx->grid, bm, d.K, table, d.tiles_cap,
+                                                                soa_out(ctx, L.out), ts);
+        LAUNCHED();
+        k_reduce_stats<<<1, 1024, 0, ctx->stream>>>(ts, nt, stats);
+        LAUNCHED();
+    }
+    CU(cudaMemcpyAsync(ctx->h_batch_off, batch_off, (uint64_t)(d.n_batches + 1) * 4, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaMemcpyAsync(ctx->h_stats, stats, sizeof(DevStats), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaEventRecord(ctx->ev_batch, ctx->stream));
+    ctx->result = RES_OTF;
+    return PSL_OK;
+}
+
+IdxOut idx_out(psl_ctx* ctx)
+{
+    const Layout& L = ctx->L;
+    IdxOut o;
+    o.E = at<float>(ctx, L.idx[0]); o.x = at<float>(ctx, L.idx[1]); o.y = at<float>(ctx, L.idx[2]);
+    o.u = at<float>(ctx, L.idx[3]); o.v = at<float>(ctx, L.idx[4]); o.wt = at<float>(ctx, L.idx[5]);
+    o.src = at<uint32_t>(ctx, L.idx[6]);
+    o.key = at<uint32_t>(ctx, L.keyfull);
+    return o;
+}
+
+// INDEX: the one-off sort of every valid in-grid record by the full key ("only needs to be
+// performed once per phase-space").  Pass-A counts were taken chunk by chunk in psl_load_chunk.
+psl_status finalize_index(psl_ctx* ctx)
+{
+    const Derived& d = ctx->d;
+    const Layout& L = ctx->L;
+    uint32_t* idx_offsets = at<uint32_t>(ctx, L.idx_offsets);
+    uint32_t* idx_counts = at<uint32_t>(ctx, L.idx_counts);
+    uint32_t* idx_batch = at<uint32_t>(ctx, L.idx_batch_off);
+    DevStats* stats = at<DevStats>(ctx, L.stats);
+    const uint32_t nt = ctx->n_tiles;
+    if (nt == 0) {
+        CU(cudaMemsetAsync(idx_offsets, 0, (uint64_t)(d.K + 1) * 4, ctx->stream));
+        CU(cudaMemsetAsync(idx_counts, 0, (uint64_t)d.K * 4, ctx->stream));
+        CU(cudaMemsetAsync(idx_batch, 0, (uint64_t)(d.n_batches + 1) * 4, ctx->stream));
+        CU(cudaMemsetAsync(stats, 0, sizeof(DevStats), ctx->stream));
+        CU(cudaMemsetAsync(scalar(ctx, SC_NIDX), 0, 4, ctx->stream));
+    } else {
+        DevBeam none;
+        memset(&none, 0, sizeof none);
+        const TileDesc* tiles = at<TileDesc>(ctx, L.tiles);
+        uint32_t* table_a = at<uint32_t>(ctx, L.table_a);
+        uint32_t* table_b = at<uint32_t>(ctx, L.table_b);
+        uint4* aos = at<uint4>(ctx, L.aos);
+        uint16_t* hi16 = at<uint16_t>(ctx, L.hi16);
+        psl_status s = run_scan(ctx, table_a, d.B_lo, nt, d.tiles_cap, scalar(ctx, SC_NIDX));
+        if (s != PSL_OK) return s;
+        uint32_t sm_a = tile_smem_bytes(kTile * kRecBytes, d.B_lo, ctx->cfg.n_ebins + 1, true, false);
+        k_scatter_idx_a<<<nt, kThreads, sm_a, ctx->stream>>>(tiles, ctx->grid, none, d.B_lo, d.lo_bits, table_a, d.tiles_cap, aos, hi16);
+        LAUNCHED();
+        uint32_t ntb = (uint32_t)((ctx->n_records + kTile - 1) / kTile);
+        k_count_hi16<<<ntb, kThreads, d.B_hi * 4, ctx->stream>>>(hi16, scalar(ctx, SC_NIDX), d.B_hi, table_b, d.tiles_b_cap);
+        LAUNCHED();
+        s = run_scan(ctx, table_b, d.B_hi, ntb, d.tiles_b_cap, scalar(ctx, SC_TOTAL));
+        if (s != PSL_OK) return s;
+        uint32_t sm_b = tile_smem_bytes(kTile * 32, d.B_hi, 0, true, true);
+        k_scatter_idx_b<<<ntb, kThreads, sm_b, ctx->stream>>>(aos, hi16, scalar(ctx, SC_NIDX), d.B_hi, table_b, d.tiles_b_cap, idx_out(ctx));
+        LAUNCHED();
+        k_offsets_by_search<<<(d.K + 1 + 255) / 256, 256, 0, ctx->stream>>>(at<uint32_t>(ctx, L.keyfull), scalar(ctx, SC_NIDX), d.K, idx_offsets);
+        LAUNCHED();
+        k_counts_from_offsets<<<(d.K + 1 + 255) / 256, 256, 0, ctx->stream>>>(idx_offsets, d.K, idx_counts, d.n_pos, d.n_batches, idx_batch);
+        LAUNCHED();
+        k_reduce_stats<<<1, 1024, 0, ctx->stream>>>(at<TileStats>(ctx, L.tstats), nt, stats);
+        LAUNCHED();
+    }
+    CU(cudaMemcpyAsync(ctx->h_idx_offsets, idx_offsets, (uint64_t)(d.K + 1) * 4, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaMemcpyAsync(ctx->h_stats, stats, sizeof(DevStats), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    ctx->idx_stats = *ctx->h_stats;
+    ctx->n_idx = ctx->h_idx_offsets[d.K];
+    ctx->indexed = true;
+    return PSL_OK;
+}
+
+psl_status expose_index(psl_ctx* ctx)
+{
+    const Derived& d = ctx->d;
+    for (uint32_t b = 0; b <= d.n_batches; ++b) ctx->h_batch_off[b] = ctx->h_idx_offsets[(uint64_t)b * d.n_pos];
+    CU(cudaEventRecord(ctx->ev_batch, ctx->stream));
+    ctx->result = RES_INDEX;
+    return PSL_OK;
+}
+
+psl_status build_beam_from_index(psl_ctx* ctx, const psl_beam* beam, const DevBeam& bm)
+{
+    const Derived& d = ctx->d;
+    const Layout& L = ctx->L;
+    const psl_config& c = ctx->cfg;
+    int32_t sel[4];
+    roi_bins(c, beam, sel);
+    const bool empty = sel[0] > sel[1] || sel[2] > sel[3];
+    const uint32_t n_rows = empty ? 0u : (uint32_t)(sel[3] - sel[2] + 1);
+    const uint32_t n_seg = d.n_batches * n_rows;
+
+    // row segments from the host copy of offsets[]: no device work, no record touched
+    if (ctx->seg_pending) {
+        CU(cudaEventSynchronize(ctx->ev_seg));
+        ctx->seg_pending = false;
+    }
+    uint32_t* vstart = ctx->h_seg;
+    uint32_t* src = ctx->h_seg + (d.max_seg + 1);
+    uint32_t* keybase = src + d.max_seg;
+    uint64_t M = 0;
+    uint32_t sidx = 0;
+    for (uint32_t b = 0; b < d.n_batches && !empty; ++b) {
+        for (int32_t iy = sel[2]; iy <= sel[3]; ++iy) {
+            uint32_t row = (b * (uint32_t)c.n_ybins + (uint32_t)iy) * (uint32_t)c.n_xbins;
+            uint32_t lo = ctx->h_idx_offsets[row + (uint32_t)sel[0]];
+            uint32_t hi = ctx->h_idx_offsets[row + (uint32_t)sel[1] + 1];
+            vstart[sidx] = (uint32_t)M;
+            src[sidx] = lo;
+            keybase[sidx] = row;
+            M += hi - lo;
+            ++sidx;
+        }
+    }
+    vstart[n_seg] = (uint32_t)M;
+    if (M > d.max_beam) {
+        set_err(ctx->err, "beam ROI selects %llu records, more than max_beam_records %llu", (unsigned long long)M, (unsigned long long)d.max_beam);
+        return PSL_ERR_CAPACITY;
+    }
+    uint32_t* d_seg = at<uint32_t>(ctx, L.seg);
+    uint32_t* beam_offsets = at<uint32_t>(ctx, L.beam_offsets);
+    uint32_t* beam_counts = at<uint32_t>(ctx, L.beam_counts);
+    uint32_t* batch_off = at<uint32_t>(ctx, L.batch_off);
+    uint32_t* beam_keys = at<uint32_t>(ctx, L.beam_keys);
+    DevBeamStats* bstat = at<DevBeamStats>(ctx, L.beam_stats);
+    const uint32_t nt = (uint32_t)((M + kTile - 1) / kTile);
+    CU(cudaMemsetAsync(scalar(ctx, SC_TILE_COUNTER), 0, 8, ctx->stream));  // tile counter + survivor count
+    if (nt == 0) {
+        CU(cudaMemsetAsync(bstat, 0, sizeof(DevBeamStats), ctx->stream));
+    } else {
+        CU(cudaMemcpyAsync(d_seg, ctx->h_seg, (uint64_t)(3 * d.max_seg + 1) * 4, cudaMemcpyHostToDevice, ctx->stream));
+        CU(cudaEventRecord(ctx->ev_seg, ctx->stream));
+        ctx->seg_pending = true;
+        CU(cudaMemsetAsync(at<uint8_t>(ctx, L.lookback), 0, (uint64_t)nt * 8, ctx->stream));
+        SegTable st;
+        st.vstart = d_seg;
+        st.src = d_seg + (d.max_seg + 1);
+        st.keybase = st.src + d.max_seg;
+        st.n_seg = n_seg;
+        st.M = (uint32_t)M;
+        IdxIn in;
+        in.E = at<float>(ctx, L.idx[0]); in.x = at<float>(ctx, L.idx[1]); in.y = at<float>(ctx, L.idx[2]);
+        in.u = at<float>(ctx, L.idx[3]); in.v = at<float>(ctx, L.idx[4]); in.wt = at<float>(ctx, L.idx[5]);
+        in.src = at<uint32_t>(ctx, L.idx[6]);
+        k_beam_compact<<<nt, kThreads, 11 * kTile * 4, ctx->stream>>>(st, in, ctx->grid, bm, soa_out(ctx, L.beam_out), beam_keys,
+                                                                     at<unsigned long long>(ctx, L.lookback),
+                                                                     scalar(ctx, SC_TILE_COUNTER), at<BeamTileStats>(ctx, L.bstats),
+                                                                     scalar(ctx, SC_BEAM_NSURV));
+        LAUNCHED();
+        k_reduce_beam_stats<<<1, 1024, 0, ctx->stream>>>(at<BeamTileStats>(ctx, L.bstats), nt, bstat);
+        LAUNCHED();
+    }
+    k_offsets_by_search<<<(d.K + 1 + 255) / 256, 256, 0, ctx->stream>>>(beam_keys, scalar(ctx, SC_BEAM_NSURV), d.K, beam_offsets);
+    LAUNCHED();
+    k_counts_from_offsets<<<(d.K + 1 + 255) / 256, 256, 0, ctx->stream>>>(beam_offsets, d.K, beam_counts, d.n_pos, d.n_batches, batch_off);
+    LAUNCHED();
+    CU(cudaMemcpyAsync(ctx->h_batch_off, batch_off, (uint64_t)(d.n_batches + 1) * 4, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaMemcpyAsync(ctx->h_beam_stats, bstat, sizeof(DevBeamStats), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaEventRecord(ctx->ev_batch, ctx->stream));
+    ctx->last_M = M;
+    ctx->result = RES_BEAM;
+    return PSL_OK;
+}
+
+psl_status fill_stats(psl_ctx* ctx, psl_stats* st)
+{
+    if (ctx->result == RES_NONE) { set_err(ctx->err, "no build yet"); return PSL_ERR_STATE; }
+    CU(cudaStreamSynchronize(ctx->stream));
+    memset(st, 0, sizeof *st);
+    st->n_in = ctx->n_records;
+    if (ctx->result == RES_OTF) {
+        const DevStats& s = *ctx->h_stats;
+        st->n_invalid = s.n_invalid; st->n_outside_grid = s.n_outside; st->n_jaw_rejected = s.n_jaw;
+        st->n_zero_weight = s.n_zero; st->n_survivors = s.n_surv;
+        st->sum_wt_in = s.sum_in; st->sum_wt_indexed = s.sum_idx; st->sum_wt_out = s.sum_out;
+    } else {
+        const DevStats& s = ctx->idx_stats;
+        st->n_invalid = s.n_invalid; st->n_outside_grid = s.n_outside;
+        st->sum_wt_in = s.sum_in; st->sum_wt_indexed = s.sum_idx;
+        if (ctx->result == RES_INDEX) {
+            st->n_survivors = ctx->n_idx;
+            st->sum_wt_out = s.sum_idx;
+        } else {
+            const DevBeamStats& b = *ctx->h_beam_stats;
+            st->n_roi_skipped = ctx->n_idx - ctx->last_M;
+            st->n_zero_weight = b.n_zero;
+            st->n_survivors = b.n_surv;
+            st->n_jaw_rejected = ctx->last_M - b.n_zero - b.n_surv;
+            st->sum_wt_out = b.sum_out;
+        }
+    }
+    return PSL_OK;
+}
+
+}  // namespace
+
+// =================================================================================================
+// C-ABI
+// =================================================================================================
+extern "C" {
+
+uint64_t psl_workspace_bytes(const psl_config* cfg)
+{
+    Derived d;
+    if (derive(cfg, &d, g_err) != PSL_OK) return 0;
+    Layout L;
+    plan(cfg, d, &L);
+    return L.total;
+}
+
+const char* psl_last_error(const psl_ctx* ctx) { return ctx ? ctx->err : g_err; }
+
+uint64_t psl_kernel_launches(const psl_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+void psl_destroy(psl_ctx* ctx)
+{
+    if (!ctx) return;
+    cudaSetDevice(ctx->cfg.device);
+    if (ctx->stream) cudaStreamSynchronize(ctx->stream);
+    if (ctx->copy_stream) {
+        cudaStreamSynchronize(ctx->copy_stream);
+        cudaStreamDestroy(ctx->copy_stream);
+    }
+    cudaEvent_t evs[] = {ctx->ev_chunk, ctx->ev_main, ctx->ev_batch, ctx->ev_seg, ctx->ev_stage[0], ctx->ev_stage[1]};
+    for (cudaEvent_t e : evs)
+        if (e) cudaEventDestroy(e);
+    void* hp[] = {ctx->h_stage[0], ctx->h_stage[1], ctx->h_batch_off, ctx->h_idx_offsets, ctx->h_seg, ctx->h_stats,
+                  ctx->h_beam_stats, ctx->h_scalars};
+    for (void* p : hp)
+        if (p) cudaFreeHost(p);
+    delete ctx;
+}
+
+psl_status psl_create(const psl_config* cfg, psl_ctx** out)
+{
+    if (!out) { set_err(g_err, "out is NULL"); return PSL_ERR_ARG; }
+    Derived d;
+    psl_status s = derive(cfg, &d, g_err);
+    if (s != PSL_OK) return s;
+    Layout L;
+    plan(cfg, d, &L);
+    if (!cfg->workspace || (reinterpret_cast<uintptr_t>(cfg->workspace) & (kAlign - 1))) { set_err(g_err, "config.workspace must be a 256-byte aligned DEVICE pointer"); return PSL_ERR_ARG; }
+    if (cfg->workspace_bytes < L.total) { set_err(g_err, "workspace too small: %llu < %llu bytes", (unsigned long long)cfg->workspace_bytes, (unsigned long long)L.total); return PSL_ERR_CAPACITY; }
+
+    psl_ctx* ctx = new (std::nothrow) psl_ctx();
+    if (!ctx) { set_err(g_err, "out of host memory"); return PSL_ERR_ARG; }
+    ctx->cfg = *cfg;
+    ctx->d = d;
+    ctx->L = L;
+    ctx->ws = static_cast<uint8_t*>(cfg->workspace);
+    ctx->stream = static_cast<cudaStream_t>(cfg->stream);
+    if (cfg->ebin_mode == PSL_EBIN_EDGES) {
+        ctx->edges.assign(cfg->e_edges, cfg->e_edges + cfg->n_ebins + 1);
+        ctx->cfg.e_edges = ctx->edges.data();
+    } else {
+        ctx->cfg.e_edges = nullptr;
+    }
+    auto fail = [&](psl_status code) {
+        memcpy(g_err, ctx->err, sizeof g_err);
+        psl_destroy(ctx);
+        return code;
+    };
+#define CUC(call)                                                                                   \
+    do {                                                                                            \
+        cudaError_t e_ = (call);                                                                    \
+        if (e_ != cudaSuccess) {                                                                    \
+            set_err(ctx->err, "%s failed: %s", #call, cudaGetErrorString(e_));                      \
+            return fail(PSL_ERR_CUDA);                                                              \
+        }                                                                                           \
+    } while (0)
+    CUC(cudaSetDevice(cfg->device));
+    CUC(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
+    cudaEvent_t* evs[] = {&ctx->ev_chunk, &ctx->ev_main, &ctx->ev_batch, &ctx->ev_seg, &ctx->ev_stage[0], &ctx->ev_stage[1]};
+    for (cudaEvent_t* e : evs) CUC(cudaEventCreateWithFlags(e, cudaEventDisableTiming));
+    CUC(cudaHostAlloc(&ctx->h_batch_off, (uint64_t)(d.n_batches + 1) * 4, cudaHostAllocDefault));
+    CUC(cudaHostAlloc(&ctx->h_stats, sizeof(DevStats), cudaHostAllocDefault));
+    CUC(cudaHostAlloc(&ctx->h_beam_stats, sizeof(DevBeamStats), cudaHostAllocDefault));
+    CUC(cudaHostAlloc(&ctx->h_scalars, 64, cudaHostAllocDefault));
+    if (cfg->mode == PSL_MODE_INDEX) {
+        CUC(cudaHostAlloc(&ctx->h_idx_offsets, (uint64_t)(d.K + 1) * 4, cudaHostAllocDefault));
+        CUC(cudaHostAlloc(&ctx->h_seg, (uint64_t)(3 * d.max_seg + 1) * 4, cudaHostAllocDefault));
+    }
+    float* dev_edges = at<float>(ctx, L.edges);
+    if (cfg->ebin_mode == PSL_EBIN_EDGES)
+        CUC(cudaMemcpyAsync(dev_edges, ctx->edges.data(), (uint64_t)(cfg->n_ebins + 1) * 4, cudaMemcpyHostToDevice, ctx->stream));
+    ctx->grid = make_grid(ctx->cfg, d, dev_edges);
+
+    // dynamic shared memory opt-in for the tile kernels
+    const uint32_t ne = cfg->n_ebins + 1;
+    if (cfg->mode == PSL_MODE_ONTHEFLY) {
+        CUC(allow_smem(k_count_raw<false>, tile_smem_bytes(kTile * kRecBytes, d.K, ne, false, false)));
+        CUC(allow_smem(k_scatter_otf, tile_smem_bytes(kTile * kRecBytes, d.K, ne, true, true)));
+    } else {
+        CUC(allow_smem(k_count_raw<true>, tile_smem_bytes(kTile * kRecBytes, d.B_lo, ne, false, false)));
+        CUC(allow_smem(k_scatter_idx_a, tile_smem_bytes(kTile * kRecBytes, d.B_lo, ne, true, false)));
+        CUC(allow_smem(k_count_hi16, d.B_hi * 4));
+        CUC(allow_smem(k_scatter_idx_b, tile_smem_bytes(kTile * 32, d.B_hi, 0, true, true)));
+        CUC(allow_smem(k_beam_compact, 11 * kTile * 4));
+    }
+    CUC(cudaStreamSynchronize(ctx->stream));
+#undef CUC
+    *out = ctx;
+    return PSL_OK;
+}
+
+psl_status psl_reset(psl_ctx* ctx)
+{
+    if (!ctx) return PSL_ERR_ARG;
+    CU(cudaSetDevice(ctx->cfg.device));
+    // later host-chunk copies must not overtake kernels of an earlier build that still read the landing zone
+    CU(cudaEventRecord(ctx->ev_main, ctx->stream));
+    CU(cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_main, 0));
+    ctx->n_records = ctx->n_host_records = 0;
+    ctx->n_tiles = ctx->n_chunks = 0;
+    ctx->ragged = false;
+    ctx->indexed = false;
+    ctx->result = RES_NONE;
+    ctx->n_idx = ctx->last_M = 0;
+    return PSL_OK;
+}
+
+psl_status psl_wait_loads(psl_ctx* ctx)
+{
+    if (!ctx) return PSL_ERR_ARG;
+    CU(cudaStreamSynchronize(ctx->copy_stream));
+    return PSL_OK;
+}
+
+psl_status psl_load_chunk(psl_ctx* ctx, const void* records, uint64_t n, int32_t mem_kind)
+{
+    if (!ctx) return PSL_ERR_ARG;
+    if (mem_kind != PSL_MEM_PAGEABLE && mem_kind != PSL_MEM_PINNED && mem_kind != PSL_MEM_DEVICE) { set_err(ctx->err, "load_chunk: bad mem_kind"); return PSL_ERR_ARG; }
+    if (n == 0) return PSL_OK;
+    if (!records) { set_err(ctx->err, "load_chunk: records is NULL"); return PSL_ERR_ARG; }
+    if (ctx->indexed) { set_err(ctx->err, "load_chunk: the index is already finalised; psl_reset first"); return PSL_ERR_STATE; }
+    if (ctx->ragged) { set_err(ctx->err, "load_chunk: a chunk whose size is not a multiple of 4 must be the last one"); return PSL_ERR_ARG; }
+    if (ctx->n_records + n > ctx->cfg.max_records) { set_err(ctx->err, "load_chunk: more than max_records"); return PSL_ERR_CAPACITY; }
+    if (ctx->n_chunks + 1 > ctx->d.max_chunks) { set_err(ctx->err, "load_chunk: more than max_chunks"); return PSL_ERR_CAPACITY; }
+    const bool host = mem_kind != PSL_MEM_DEVICE;
+    if (host && ctx->n_host_records + n > ctx->cfg.max_host_records) { set_err(ctx->err, "load_chunk: more host records than max_host_records"); return PSL_ERR_CAPACITY; }
+    CU(cudaSetDevice(ctx->cfg.device));
+
+    const uint8_t* dev_ptr;
+    if (host) {
+        uint8_t* dst = at<uint8_t>(ctx, ctx->L.raw) + ctx->n_host_records * kRecBytes;
+        const uint64_t bytes = n * kRecBytes;
+        if (mem_kind == PSL_MEM_PINNED) {
+            CU(cudaMemcpyAsync(dst, records, bytes, cudaMemcpyHostToDevice, ctx->copy_stream));
+        } else {
+            // pageable source: double-buffered pinned staging, the CPU copy of piece i+1 overlaps the DMA of piece i
+            for (int k = 0; k < 2; ++k)
+                if (!ctx->h_stage[k]) CU(cudaHostAlloc(&ctx->h_stage[k], kStageBytes, cudaHostAllocDefault));
+            const uint8_t* srcp = static_cast<const uint8_t*>(records);
+            for (uint64_t off = 0; off < bytes; off += kStageBytes) {
+                uint64_t piece = bytes - off < kStageBytes ? bytes - off : kStageBytes;
+                int k = ctx->stage_next;
+                CU(cudaEventSynchronize(ctx->ev_stage[k]));
+                memcpy(ctx->h_stage[k], srcp + off, piece);
+                CU(cudaMemcpyAsync(dst + off, ctx->h_stage[k], piece, cudaMemcpyHostToDevice, ctx->copy_stream));
+                CU(cudaEventRecord(ctx->ev_stage[k], ctx->copy_stream));
+                ctx->stage_next = k ^ 1;
+            }
+        }
+        CU(cudaEventRecord(ctx->ev_chunk, ctx->copy_stream));
+        CU(cudaStreamWaitEvent(ctx->stream, ctx->ev_chunk, 0));
+        dev_ptr = dst;
+    } else {
+        if (reinterpret_cast<uintptr_t>(records) & 3u) { set_err(ctx->err, "load_chunk: DEVICE records must be 4-byte aligned"); return PSL_ERR_ARG; }
+        dev_ptr = static_cast<const uint8_t*>(records);
+    }
+
+    const uint32_t nt = (uint32_t)((n + kTile - 1) / kTile);
+    const uint32_t tile0 = ctx->n_tiles;
+    TileDesc* tiles = at<TileDesc>(ctx, ctx->L.tiles);
+    k_fill_tiles<<<(nt + 255) / 256, 256, 0, ctx->stream>>>(tiles, tile0, nt, dev_ptr, (uint32_t)ctx->n_records, (uint32_t)n);
+    LAUNCHED();
+    if (ctx->cfg.mode == PSL_MODE_INDEX) {
+        // a8 for pass A, chunk by chunk: overlaps the transfer of the next chunk
+        DevBeam none;
+        memset(&none, 0, sizeof none);
+        uint32_t sm = tile_smem_bytes(kTile * kRecBytes, ctx->d.B_lo, ctx->cfg.n_ebins + 1, false, false);
+        k_count_raw<true><<<nt, kThreads, sm, ctx->stream>>>(tiles, tile0, ctx->grid, none, ctx->d.B_lo, (1u << ctx->d.lo_bits) - 1u,
+                                                            at<uint32_t>(ctx, ctx->L.table_a), ctx->d.tiles_cap,
+                                                            at<TileStats>(ctx, ctx->L.tstats));
+        LAUNCHED();
+    }
+    ctx->n_records += n;
+    if (host) ctx->n_host_records += n;
+    ctx->n_tiles += nt;
+    ctx->n_chunks += 1;
+    if (n % 4) ctx->ragged = true;
+    ctx->result = RES_NONE;
+    return PSL_OK;
+}
+
+psl_status psl_build_batches(psl_ctx* ctx, const psl_beam* beam, psl_stats* stats)
+{
+    if (!ctx) return PSL_ERR_ARG;
+    CU(cudaSetDevice(ctx->cfg.device));
+    DevBeam bm;
+    psl_status s = make_beam(ctx, beam, &bm, ctx->err);
+    if (s != PSL_OK) return s;
+    if (ctx->cfg.mode == PSL_MODE_ONTHEFLY) {
+        s = build_onthefly(ctx, bm);
+    } else {
+        if (!ctx->indexed) {
+            s = finalize_index(ctx);
+            if (s != PSL_OK) return s;
+        }
+        s = beam ? build_beam_from_index(ctx, beam, bm) : expose_index(ctx);
+    }
+    if (s != PSL_OK) return s;
+    if (stats) return fill_stats(ctx, stats);
+    return PSL_OK;
+}
+
+psl_status psl_get_stats(psl_ctx* ctx, psl_stats* stats)
+{
+    if (!ctx || !stats) return PSL_ERR_ARG;
+    return fill_stats(ctx, stats);
+}
+
+psl_status psl_get_tables(psl_ctx* ctx, const uint32_t** counts, const uint32_t** offsets, uint32_t* n_keys)
+{
+    if (!ctx) return PSL_ERR_ARG;
+    if (ctx->result == RES_NONE) { set_err(ctx->err, "get_tables: no build yet"); return PSL_ERR_STATE; }
+    const Layout& L = ctx->L;
+    uint64_t c = ctx->result == RES_OTF ? L.counts : (ctx->result == RES_INDEX ? L.idx_counts : L.beam_counts);
+    uint64_t o = ctx->result == RES_OTF ? L.offsets : (ctx->result == RES_INDEX ? L.idx_offsets : L.beam_offsets);
+    if (counts) *counts = at<uint32_t>(ctx, c);
+    if (offsets) *offsets = at<uint32_t>(ctx, o);
+    if (n_keys) *n_keys = ctx->d.K;
+    return PSL_OK;
+}
+
+psl_status psl_get_batch(psl_ctx* ctx, int32_t t, int32_t ie, psl_batch* out)
+{
+    if (!ctx || !out) return PSL_ERR_ARG;
+    if (ctx->result == RES_NONE) { set_err(ctx->err, "get_batch: no build yet"); return PSL_ERR_STATE; }
+    const bool whole = (t == -1 && ie == -1);
+    if (!whole && (t < 0 || t >= ctx->cfg.n_types || ie < 0 || ie >= ctx->cfg.n_ebins)) { set_err(ctx->err, "get_batch: (t, ie) out of range"); return PSL_ERR_ARG; }
+    CU(cudaEventSynchronize(ctx->ev_batch));
+    const Derived& d = ctx->d;
+    const Layout& L = ctx->L;
+    uint32_t b = whole ? 0u : (uint32_t)(t * ctx->cfg.n_ebins + ie);
+    uint32_t first = ctx->h_batch_off[b];
+    uint32_t last = ctx->h_batch_off[whole ? d.n_batches : b + 1];
+    memset(out, 0, sizeof *out);
+    out->first = first;
+    out->count = last - first;
+    out->n_bins = whole ? d.K : d.n_pos;
+    const bool proj = (ctx->cfg.flags & PSL_OUT_PROJ) != 0;
+    if (ctx->result == RES_INDEX) {
+        out->E = at<float>(ctx, L.idx[0]) + first; out->x = at<float>(ctx, L.idx[1]) + first; out->y = at<float>(ctx, L.idx[2]) + first;
+        out->u = at<float>(ctx, L.idx[3]) + first; out->v = at<float>(ctx, L.idx[4]) + first; out->wt = at<float>(ctx, L.idx[5]) + first;
+        out->src_index = at<uint32_t>(ctx, L.idx[6]) + first;
+        out->bin_offsets = at<uint32_t>(ctx, L.idx_offsets) + (uint64_t)b * d.n_pos;
+    } else {
+        const uint64_t* o = ctx->result == RES_OTF ? L.out : L.beam_out;
+        out->E = at<float>(ctx, o[0]) + first; out->x = at<float>(ctx, o[1]) + first; out->y = at<float>(ctx, o[2]) + first;
+        out->u = at<float>(ctx, o[3]) + first; out->v = at<float>(ctx, o[4]) + first; out->w = at<float>(ctx, o[5]) + first;
+        out->wt = at<float>(ctx, o[6]) + first;
+        if (proj) {
+            out->xp = at<float>(ctx, o[7]) + first;
+            out->yp = at<float>(ctx, o[8]) + first;
+        }
+        out->src_index = at<uint32_t>(ctx, o[9]) + first;
+        out->bin_offsets = at<uint32_t>(ctx, ctx->result == RES_OTF ? L.offsets : L.beam_offsets) + (uint64_t)b * d.n_pos;
+    }
+    return PSL_OK;
+}
+
+psl_status psl_roi_bins(const psl_ctx* ctx, const psl_beam* beam, int32_t bins_out[4])
+{
+    if (!ctx || !bins_out) return PSL_ERR_ARG;
+    roi_bins(ctx->cfg, beam, bins_out);
+    return PSL_OK;
+}
+
+psl_status psl_roi_from_jaws(const psl_geometry* g, const psl_beam* beam, float margin, float roi_out[4])
+{
+    if (!g || !beam || !roi_out) { set_err(g_err, "roi_from_jaws: NULL argument"); return PSL_ERR_ARG; }
+    psl_status s = check_geometry(*g, g_err);
+    if (s != PSL_OK) return s;
+    if (!(g->z_jaw_x < g->z_iso && g->z_jaw_y < g->z_iso)) { set_err(g_err, "roi_from_jaws: jaw planes must be upstream of the isocentre"); return PSL_ERR_GEOMETRY; }
+    const double zj[2] = {g->z_jaw_x, g->z_jaw_y};
+    const double e1[2] = {beam->jaw_x1, beam->jaw_y1}, e2[2] = {beam->jaw_x2, beam->jaw_y2};
+    for (int a = 0; a < 2; ++a) {
+        // the line from the field centre at z_iso through the jaw edge, extended up to z_plane
+        double to_jaw = (zj[a] - (double)g->z_src) / ((double)g->z_iso - (double)g->z_src);
+        double mid = 0.5 * (e1[a] + e2[a]);
+        double reach = ((double)g->z_iso - (double)g->z_plane) / ((double)g->z_iso - zj[a]);
+        roi_out[2 * a + 0] = (float)(mid + (e1[a] * to_jaw - mid) * reach - (double)margin);
+        roi_out[2 * a + 1] = (float)(mid + (e2[a] * to_jaw - mid) * reach + (double)margin);
+    }
+    return PSL_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,250 @@
+// psl_beam.cuh -- per-beam batches from the pre-sorted PSL index (paper method 3).
+//
+// The index stores every valid in-grid record sorted by key = ((t*N_E + ie)*N_y + iy)*N_x + ix, so the
+// records of one (type, energy, row iy) and columns rx0..rx1 are ONE contiguous range.  The host turns the
+// beam's ROI into that list of row segments from its copy of offsets[] (no device work, no record is read):
+// position bins outside the ROI are skipped without touching their records.
+// The kernel below walks the concatenated segments ("virtual" order = key order), applies the jaw test
+// (PAPER.md:55), the fluence-map weight and MU weight, and compacts the survivors
+// stably: virtual order IS the required output order, so the batch layout is a plain stream compaction.
+// The global slot of a tile's first survivor comes from a decoupled look-back over tile aggregates -- an
+// ordered prefix sum, so the result is deterministic.
+#pragma once
+
+#include "psl_device.cuh"
+#include "psl_partition.cuh"
+
+namespace psl {
+
+struct SegTable {
+    const uint32_t* vstart;   // [n_seg+1] virtual index of each segment's first record; vstart[n_seg] = M
+    const uint32_t* src;      // [n_seg] slot of that record in the index
+    const uint32_t* keybase;  // [n_seg] key of column 0 of the segment's row
+    uint32_t n_seg;
+    uint32_t M;               // records selected by the ROI
+};
+
+struct IdxIn {
+    const float *E, *x, *y, *u, *v, *wt;
+    const uint32_t* src;
+};
+
+struct BeamTileStats {  // 16 bytes
+    uint32_t n_zero, n_surv;
+    double sum_out;
+};
+
+constexpr unsigned long long kFlagAggregate = 1ull << 62;
+constexpr unsigned long long kFlagInclusive = 2ull << 62;
+constexpr unsigned long long kFlagMask = 3ull << 62;
+
+__device__ __forceinline__ unsigned long long ld_state(const unsigned long long* p)
+{
+    return *reinterpret_cast<const volatile unsigned long long*>(p);
+}
+
+// last s in [lo, hi] with vstart[s] <= v  (vstart[lo] <= v guaranteed)
+__device__ __forceinline__ uint32_t seg_of(const uint32_t* __restrict__ vstart, uint32_t lo, uint32_t hi, uint32_t v)
+{
+    while (lo < hi) {
+        uint32_t mid = lo + ((hi - lo + 1) >> 1);
+        if (__ldg(vstart + mid) <= v) lo = mid; else hi = mid - 1;
+    }
+    return lo;
+}
+
+constexpr int kBeamArrays = 12;  // E x y u v w wt xp yp src key + spare
+
+__global__ void __launch_bounds__(kThreads) k_beam_compact(SegTable seg, IdxIn in, const __grid_constant__ DevGrid g,
+                                                          const __grid_constant__ DevBeam bm, SoAOut out,
+                                                          uint32_t* __restrict__ out_key,
+                                                          unsigned long long* __restrict__ tile_state,
+                                                          uint32_t* __restrict__ tile_counter,
+                                                          BeamTileStats* __restrict__ bstats,
+                                                          uint32_t* __restrict__ n_surv_out)
+{
+    extern __shared__ __align__(128) uint8_t smem[];
+    uint32_t* stage = reinterpret_cast<uint32_t*>(smem);  // [11][kTile]
+    __shared__ uint32_t s_wc[2][kWarps];
+    __shared__ uint32_t s_ctl[4];  // tile, seg_first, seg_last, exclusive prefix
+    __shared__ double s_d[kWarps];
+    __shared__ uint32_t s_z[kWarps];
+
+    const uint32_t w = warp_id();
+    if (threadIdx.x == 0) s_ctl[0] = atomicAdd(tile_counter, 1u);  // tiles are handed out in order
+    __syncthreads();
+    const uint32_t tile = s_ctl[0];
+    const uint32_t v0 = tile * kTile;
+    const uint32_t cnt = min((uint32_t)kTile, seg.M - v0);
+    if (threadIdx.x == 0) s_ctl[1] = seg_of(seg.vstart, 0, seg.n_seg - 1, v0);
+    if (threadIdx.x == 32) s_ctl[2] = seg_of(seg.vstart, 0, seg.n_seg - 1, v0 + cnt - 1);
+    __syncthreads();
+    const uint32_t s_first = s_ctl[1], s_last = s_ctl[2];
+
+    uint32_t run = 0, n_zero = 0;
+    double sum_out = 0.0;
+#pragma unroll 1
+    for (int r = 0; r < kRounds; ++r) {
+        uint32_t lv = r * kThreads + threadIdx.x;
+        bool keep = false;
+        float E = 0, x = 0, y = 0, u = 0, v = 0, wz = 0, wt = 0, xm = 0, ym = 0;
+        uint32_t srci = 0, key = 0;
+        if (lv < cnt) {
+            uint32_t vv = v0 + lv;
+            uint32_t sg = seg_of(seg.vstart, s_first, s_last, vv);
+            uint32_t p = __ldg(seg.src + sg) + (vv - __ldg(seg.vstart + sg));
+            E = in.E[p]; x = in.x[p]; y = in.y[p]; u = in.u[p]; v = in.v[p];
+            float wt0 = in.wt[p];
+            srci = in.src[p];
+            int ix = 0;
+            if (g.has_pos) axis_bin(x, g.inv_dx, g.ix0, g.n_xbins, ix);
+            key = __ldg(seg.keybase + sg) + (uint32_t)ix;
+            float q = q_of(u, v), tx, ty;
+            slopes(u, v, q, wz, tx, ty);
+            keep = !(bm.has_jaws) || jaw_pass(bm, x, y, tx, ty);
+            xm = __fadd_rn(x, __fmul_rn(tx, bm.dzM));
+            ym = __fadd_rn(y, __fmul_rn(ty, bm.dzM));
+            wt = final_weight(bm, wt0, xm, ym);
+            if (keep && bm.drop_zero && wt == 0.0f) {
+                keep = false;
+                n_zero += 1;
+            }
+        }
+        uint32_t ballot = __ballot_sync(0xFFFFFFFFu, keep);
+        if (lane_id() == 0) s_wc[r & 1][w] = __popc(ballot);
+        __syncthreads();
+        uint32_t pre = 0, tot = 0;
+#pragma unroll
+        for (int k = 0; k < kWarps; ++k) {
+            uint32_t c = s_wc[r & 1][k];
+            pre += (k < (int)w) ? c : 0u;
+            tot += c;
+        }
+        if (keep) {
+            uint32_t pos = run + pre + __popc(ballot & lanemask_lt());
+            stage[0 * kTile + pos] = __float_as_uint(E);
+            stage[1 * kTile + pos] = __float_as_uint(x);
+            stage[2 * kTile + pos] = __float_as_uint(y);
+            stage[3 * kTile + pos] = __float_as_uint(u);
+            stage[4 * kTile + pos] = __float_as_uint(v);
+            stage[5 * kTile + pos] = __float_as_uint(wz);
+            stage[6 * kTile + pos] = __float_as_uint(wt);
+            stage[7 * kTile + pos] = __float_as_uint(xm);
+            stage[8 * kTile + pos] = __float_as_uint(ym);
+            stage[9 * kTile + pos] = srci;
+            stage[10 * kTile + pos] = key;
+            sum_out += (double)wt;
+        }
+        run += tot;
+    }
+    const uint32_t total = run;
+
+    // decoupled look-back (warp 0): exclusive prefix of `total` over the tiles before this one
+    if (w == 0) {
+        uint32_t excl = 0;
+        if (tile == 0) {
+            if (lane_id() == 0) atomicExch(&tile_state[0], kFlagInclusive | (unsigned long long)total);
+        } else {
+            if (lane_id() == 0) atomicExch(&tile_state[tile], kFlagAggregate | (unsigned long long)total);
+            int look = (int)tile - 1;
+            while (true) {
+                int idx = look - (int)lane_id();
+                unsigned long long st;
+                do {
+                    st = idx >= 0 ? ld_state(&tile_state[idx]) : kFlagInclusive;
+                } while (__any_sync(0xFFFFFFFFu, (st & kFlagMask) == 0ull));
+                uint32_t incl = __ballot_sync(0xFFFFFFFFu, (st & kFlagMask) == kFlagInclusive);
+                uint32_t val = (uint32_t)(st & 0xFFFFFFFFull);
+                if (incl) {
+                    int first = __ffs(incl) - 1;
+                    val = ((int)lane_id() <= first) ? val : 0u;
+                    excl += __reduce_add_sync(0xFFFFFFFFu, val);
+                    break;
+                }
+                excl += __reduce_add_sync(0xFFFFFFFFu, val);
+                look -= 32;
+            }
+            if (lane_id() == 0) atomicExch(&tile_state[tile], kFlagInclusive | (unsigned long long)(excl + total));
+        }
+        if (lane_id() == 0) {
+            s_ctl[3] = excl;
+            if (v0 + cnt == seg.M) *n_surv_out = excl + total;  // last tile
+        }
+    }
+    sum_out = warp_sum_double(sum_out);
+    n_zero = __reduce_add_sync(0xFFFFFFFFu, n_zero);
+    if (lane_id() == 0) {
+        s_d[w] = sum_out;
+        s_z[w] = n_zero;
+    }
+    __syncthreads();
+    const uint32_t gbase = s_ctl[3];
+
+    // coalesced copy-out of the tile's survivors
+    for (uint32_t j = threadIdx.x; j < total; j += kThreads) {
+        size_t d = (size_t)gbase + j;
+        out.E[d] = __uint_as_float(stage[0 * kTile + j]);
+        out.x[d] = __uint_as_float(stage[1 * kTile + j]);
+        out.y[d] = __uint_as_float(stage[2 * kTile + j]);
+        out.u[d] = __uint_as_float(stage[3 * kTile + j]);
+        out.v[d] = __uint_as_float(stage[4 * kTile + j]);
+        out.w[d] = __uint_as_float(stage[5 * kTile + j]);
+        out.wt[d] = __uint_as_float(stage[6 * kTile + j]);
+        if (bm.out_proj) {
+            out.xp[d] = __uint_as_float(stage[7 * kTile + j]);
+            out.yp[d] = __uint_as_float(stage[8 * kTile + j]);
+        }
+        out.src[d] = stage[9 * kTile + j];
+        out_key[d] = stage[10 * kTile + j];
+    }
+    if (threadIdx.x == 0) {
+        BeamTileStats bs = {0, total, 0.0};
+        for (int k = 0; k < kWarps; ++k) {
+            bs.sum_out += s_d[k];
+            bs.n_zero += s_z[k];
+        }
+        bstats[tile] = bs;
+    }
+}
+
+struct DevBeamStats {
+    unsigned long long n_zero, n_surv;
+    double sum_out;
+};
+
+__global__ void __launch_bounds__(1024) k_reduce_beam_stats(const BeamTileStats* __restrict__ ts, uint32_t n_tiles,
+                                                            DevBeamStats* __restrict__ out)
+{
+    __shared__ unsigned long long s_n[32][2];
+    __shared__ double s_d[32];
+    unsigned long long nz = 0, ns = 0;
+    double d = 0.0;
+    for (uint32_t t = threadIdx.x; t < n_tiles; t += 1024) {
+        BeamTileStats x = ts[t];
+        nz += x.n_zero;
+        ns += x.n_surv;
+        d += x.sum_out;
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        nz += __shfl_xor_sync(0xFFFFFFFFu, nz, o);
+        ns += __shfl_xor_sync(0xFFFFFFFFu, ns, o);
+    }
+    d = warp_sum_double(d);
+    if (lane_id() == 0) {
+        s_n[warp_id()][0] = nz;
+        s_n[warp_id()][1] = ns;
+        s_d[warp_id()] = d;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        DevBeamStats r = {0, 0, 0.0};
+        for (int k = 0; k < 32; ++k) {
+            r.n_zero += s_n[k][0];
+            r.n_surv += s_n[k][1];
+            r.sum_out += s_d[k];
+        }
+        *out = r;
+    }
+}
+
+}  // namespace psl

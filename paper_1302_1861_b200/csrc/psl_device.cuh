@@ -1,0 +1,305 @@
+// psl_device.cuh -- device-side building blocks shared by the kernels of libpsl_b200 (sm_100a only).
+//
+// Holds: the kernel-parameter structs, the per-record arithmetic of the hot path (validity, energy bin,
+// position bin, key, jaw projection, fluence lookup -- include/psl.h "Arithmetic contract"), the 1-D TMA
+// bulk-load of a tile of packed records into shared memory, and small block-level utilities.
+// This file shares nothing with oracle/ (the CPU checker).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <float.h>
+#include <stdint.h>
+
+namespace psl {
+
+constexpr int kTile = 2048;              // records per tile (= table granularity of every partition pass)
+constexpr int kThreads = 256;            // threads per CTA in the tile kernels
+constexpr int kWarps = kThreads / 32;    // 8
+constexpr int kRounds = kTile / kThreads;  // 8 records per thread
+constexpr int kWarpSpan = kTile / kWarps;  // 256 consecutive records owned by one warp
+constexpr int kRecWords = 7;             // 28-byte packed record
+constexpr int kRecBytes = 28;
+constexpr int kMaxBuckets = 2048;        // most buckets one partition pass handles
+constexpr uint32_t kNone = 0xFFFFFFFFu;
+
+enum : int { C_SURVIVOR = 0, C_INVALID = 1, C_OUTSIDE = 2, C_ROI = 3, C_JAW = 4, C_ZERO = 5 };
+
+struct DevGrid {
+    int32_t n_types, ebin_mode, n_ebins;
+    float e_min, dE;
+    const float* e_edges;  // DEVICE, n_ebins+1 (edge mode)
+    int32_t has_pos, n_xbins, n_ybins, ix0, iy0;
+    float inv_dx, inv_dy;
+    uint32_t n_pos;
+};
+
+struct DevBeam {
+    int32_t has_beam, has_jaws;
+    float X1, X2, Y1, Y2;  // aperture at the jaw planes
+    float dzJx, dzJy;      // z_jaw - z_plane
+    int32_t has_map;
+    const float* fluence;  // DEVICE
+    int32_t map_nx, map_ny, px0, py0;
+    float inv_mdx, inv_mdy;
+    float dzM;             // z_map - z_plane
+    float mu;
+    uint32_t drop_zero;
+    uint32_t out_proj;
+};
+
+struct TileDesc {  // 16 bytes
+    const void* ptr;       // first record of the tile
+    uint32_t first_index;  // load-order index of that record
+    uint32_t count;        // 1..kTile
+};
+
+struct TileStats {  // 48 bytes, one per tile, reduced in a fixed order (deterministic doubles)
+    uint32_t n_invalid, n_outside, n_jaw, n_zero, n_surv, pad;
+    double sum_in, sum_idx, sum_out;
+};
+
+struct Rec {
+    int32_t type;
+    float E, x, y, u, v, wt;
+};
+
+// ------------------------------------------------------------------------------------------------
+// per-record arithmetic.  Every floating-point operation is an explicit round-to-nearest intrinsic so
+// that no FMA can be formed (the TU is also compiled with -fmad=false).
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ bool is_finite(float a) { return fabsf(a) <= FLT_MAX; }
+
+// q = 1 - (u*u + v*v)   (records carry direction; the third cosine follows from the other two)
+__device__ __forceinline__ float q_of(float u, float v)
+{
+    return __fsub_rn(1.0f, __fadd_rn(__fmul_rn(u, u), __fmul_rn(v, v)));
+}
+
+__device__ __forceinline__ bool rec_valid(const Rec& r, float q)
+{
+    return ((uint32_t)r.type <= 2u) && is_finite(r.E) && is_finite(r.x) && is_finite(r.y) && is_finite(r.u) &&
+           is_finite(r.v) && is_finite(r.wt) && (r.E > 0.0f) && (q > 0.0f);
+}
+
+// Energy bin: linear = floor((E - e_min)/dE) clamped; edge table = number of interior edges <= E.
+__device__ __forceinline__ int energy_bin(const DevGrid& g, float E, const float* s_edges)
+{
+    if (g.ebin_mode == 0) {
+        float t = __fdiv_rn(__fsub_rn(E, g.e_min), g.dE);
+        if (t < 0.0f) return 0;
+        if (t >= (float)g.n_ebins) return g.n_ebins - 1;
+        return (int)floorf(t);
+    }
+    int lo = 1, hi = g.n_ebins;  // first k in [1, n_ebins) with edges[k] > E
+    while (lo < hi) {
+        int mid = (lo + hi) >> 1;
+        if (s_edges[mid] <= E) lo = mid + 1; else hi = mid;
+    }
+    return lo - 1;
+}
+
+// Bin of a coordinate on a grid whose bin k covers [k*d, (k+1)*d) in absolute coordinates and whose first
+// bin is i0 ("[x_i, x_i+dx]"; also used for fluence-map pixels).
+__device__ __forceinline__ bool axis_bin(float x, float inv_d, int i0, int n, int& out)
+{
+    float f = floorf(__fmul_rn(x, inv_d));
+    bool ok = (f >= (float)i0) && (f < (float)(i0 + n));
+    out = ok ? ((int)f - i0) : 0;
+    return ok;
+}
+
+__device__ __forceinline__ int type_division(const DevGrid& g, int type) { return (g.n_types == 2 && type > 1) ? 1 : type; }
+
+// Slopes dx/dz, dy/dz of the ray: t = 1/w, tx = u*t, ty = v*t with w = sqrt(q).
+__device__ __forceinline__ void slopes(float u, float v, float q, float& w, float& tx, float& ty)
+{
+    w = __fsqrt_rn(q);
+    float t = __fdiv_rn(1.0f, w);
+    tx = __fmul_rn(u, t);
+    ty = __fmul_rn(v, t);
+}
+
+// Jaw accept/reject: half-open aperture at one thin plane per jaw pair.
+__device__ __forceinline__ bool jaw_pass(const DevBeam& b, float x, float y, float tx, float ty)
+{
+    float xj = __fadd_rn(x, __fmul_rn(tx, b.dzJx));
+    float yj = __fadd_rn(y, __fmul_rn(ty, b.dzJy));
+    return (b.X1 <= xj) && (xj < b.X2) && (b.Y1 <= yj) && (yj < b.Y2);
+}
+
+// Final weight: containing pixel of the map at z_map, 0 outside, (wt*F)*mu.
+__device__ __forceinline__ float final_weight(const DevBeam& b, float wt, float xm, float ym)
+{
+    if (!b.has_beam) return wt;
+    if (!b.has_map) return __fmul_rn(wt, b.mu);
+    int px, py;
+    float F = 0.0f;
+    if (axis_bin(xm, b.inv_mdx, b.px0, b.map_nx, px) && axis_bin(ym, b.inv_mdy, b.py0, b.map_ny, py))
+        F = __ldg(b.fluence + (size_t)py * (size_t)b.map_nx + (size_t)px);
+    return __fmul_rn(__fmul_rn(wt, F), b.mu);
+}
+
+// Steps 1-4 (+6, +8 when a beam is given) for one raw record.  Returns the class; key is valid for every
+// class except C_INVALID / C_OUTSIDE.
+__device__ __forceinline__ int classify_raw(const DevGrid& g, const DevBeam& b, const Rec& r, const float* s_edges,
+                                            uint32_t& key)
+{
+    key = kNone;
+    float q = q_of(r.u, r.v);
+    if (!rec_valid(r, q)) return C_INVALID;
+    int ix = 0, iy = 0;
+    if (g.has_pos) {
+        if (!axis_bin(r.x, g.inv_dx, g.ix0, g.n_xbins, ix)) return C_OUTSIDE;
+        if (!axis_bin(r.y, g.inv_dy, g.iy0, g.n_ybins, iy)) return C_OUTSIDE;
+    }
+    int ie = energy_bin(g, r.E, s_edges);
+    key = (uint32_t)(type_division(g, r.type) * g.n_ebins + ie) * g.n_pos + (uint32_t)(iy * g.n_xbins + ix);
+    if (!b.has_beam) return C_SURVIVOR;
+    if (b.has_jaws || b.drop_zero) {
+        float w, tx, ty;
+        slopes(r.u, r.v, q, w, tx, ty);
+        if (b.has_jaws && !jaw_pass(b, r.x, r.y, tx, ty)) return C_JAW;
+        if (b.drop_zero) {
+            float xm = __fadd_rn(r.x, __fmul_rn(tx, b.dzM));
+            float ym = __fadd_rn(r.y, __fmul_rn(ty, b.dzM));
+            if (final_weight(b, r.wt, xm, ym) == 0.0f) return C_ZERO;
+        }
+    }
+    return C_SURVIVOR;
+}
+
+// ------------------------------------------------------------------------------------------------
+// shared-memory tile of packed records: 1-D TMA bulk copy (cp.async.bulk, SASS UBLKCP) completing on an
+// mbarrier; scalar fallback when the source is not 16-byte aligned or the byte count is not a multiple
+// of 16 (only the ragged last tile of a chunk).
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t phase)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE_%=;\n\t"
+        "bra WAIT_%=;\n\t"
+        "DONE_%=:\n\t}" ::"r"(smem_u32(bar)), "r"(phase) : "memory");
+}
+__device__ __forceinline__ void tma_load_1d(void* smem_dst, const void* gsrc, uint32_t bytes, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(smem_dst)),
+                 "l"(gsrc), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+
+// Bring `bytes` (a multiple of 4) from global into s_dst.  Must be called by all threads of the CTA; `bar`
+// must have been initialised (count 1) and made visible with a __syncthreads.  Ends with the data visible
+// to every thread.
+__device__ __forceinline__ void load_tile_bytes(uint32_t* s_dst, const void* gsrc, uint32_t bytes, uint64_t* bar,
+                                                uint32_t phase)
+{
+    bool bulk = ((reinterpret_cast<uintptr_t>(gsrc) & 15u) == 0) && ((bytes & 15u) == 0) && bytes > 0;
+    if (bulk) {
+        if (threadIdx.x == 0) {
+            mbar_expect_tx(bar, bytes);
+            tma_load_1d(s_dst, gsrc, bytes, bar);
+        }
+        mbar_wait(bar, phase);
+    } else {
+        const uint32_t* g = reinterpret_cast<const uint32_t*>(gsrc);
+        for (uint32_t i = threadIdx.x; i < bytes / 4; i += blockDim.x) s_dst[i] = __ldg(g + i);
+        __syncthreads();
+    }
+}
+
+__device__ __forceinline__ Rec rec_from_smem(const uint32_t* s_raw, int idx)
+{
+    const uint32_t* p = s_raw + idx * kRecWords;  // stride 7 words across lanes: conflict-free
+    Rec r;
+    r.type = (int32_t)p[0];
+    r.E = __uint_as_float(p[1]);
+    r.x = __uint_as_float(p[2]);
+    r.y = __uint_as_float(p[3]);
+    r.u = __uint_as_float(p[4]);
+    r.v = __uint_as_float(p[5]);
+    r.wt = __uint_as_float(p[6]);
+    return r;
+}
+
+// ------------------------------------------------------------------------------------------------
+// block utilities (kThreads threads)
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t lane_id() { return threadIdx.x & 31u; }
+__device__ __forceinline__ uint32_t warp_id() { return threadIdx.x >> 5; }
+__device__ __forceinline__ uint32_t lanemask_lt() { return (1u << lane_id()) - 1u; }
+
+__device__ __forceinline__ uint32_t warp_incl_scan(uint32_t v)
+{
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        uint32_t n = __shfl_up_sync(0xFFFFFFFFu, v, o);
+        if ((int)lane_id() >= o) v += n;
+    }
+    return v;
+}
+
+// exclusive scan of one value per thread over the CTA; s_warp holds >= kWarps+1 words; returns the
+// exclusive prefix, *total receives the CTA sum.  Contains two __syncthreads.
+__device__ __forceinline__ uint32_t block_excl_scan(uint32_t v, uint32_t* s_warp, uint32_t* total)
+{
+    uint32_t inc = warp_incl_scan(v);
+    if (lane_id() == 31) s_warp[warp_id()] = inc;
+    __syncthreads();
+    if (warp_id() == 0) {
+        uint32_t w = lane_id() < (uint32_t)(blockDim.x >> 5) ? s_warp[lane_id()] : 0u;
+        uint32_t wi = warp_incl_scan(w);
+        if (lane_id() < (uint32_t)(blockDim.x >> 5)) s_warp[lane_id()] = wi - w;
+        if (lane_id() == 31) s_warp[32] = wi;
+    }
+    __syncthreads();
+    uint32_t r = s_warp[warp_id()] + inc - v;
+    *total = s_warp[32];
+    return r;
+}
+
+__device__ __forceinline__ double warp_sum_double(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, o);
+    return v;
+}
+
+// Stable rank of a record inside its warp's slice of the tile: records of one warp arrive in rounds of 32
+// consecutive records; `cnt` is the warp's private running count per bucket.  Lanes with bucket == kNone
+// take no part.  Must be called by all 32 lanes.
+__device__ __forceinline__ uint32_t warp_rank(uint32_t bucket, uint16_t* cnt)
+{
+    uint32_t rank = 0;
+    uint32_t active = __ballot_sync(0xFFFFFFFFu, bucket != kNone);
+    if (bucket != kNone) {
+        uint32_t peers = __match_any_sync(active, bucket);
+        int leader = __ffs(peers) - 1;
+        uint32_t before = __popc(peers & lanemask_lt());
+        uint32_t base = 0;
+        if ((int)lane_id() == leader) {
+            base = cnt[bucket];
+            cnt[bucket] = (uint16_t)(base + __popc(peers));
+        }
+        base = __shfl_sync(peers, base, leader);
+        rank = base + before;
+    }
+    __syncwarp();
+    return rank;
+}
+
+}  // namespace psl

@@ -1,0 +1,312 @@
+"""-m gpu: the CUDA path (through the C-ABI, via the thin binding) against the CPU oracle, element by element,
+on the same seeded inputs.  Bit-exact for counts, offsets, permutation (src_index), survivor set and every
+copied field; floats within 1e-6 relative (north_star) -- and, per the arithmetic contract, bit-equal."""
+import numpy as np
+import pytest
+
+import workloads as W
+from helpers import assert_matches_oracle, dirty, library_result, run_library
+from oracle import psl_oracle as O
+
+pytestmark = pytest.mark.gpu
+
+
+def P():
+    import paper_1302_1861_b200 as P_
+
+    return P_
+
+
+def check(w, r, beam, chunk=0, mem="device", flags=0, proj=False):
+    ctx = run_library(w, r, beam, chunk=chunk, mem=mem, flags=flags)
+    lib = library_result(ctx)
+    orc = O.Oracle(w.grid, w.geometry, flags=flags & 2).build(r, beam)
+    assert_matches_oracle(lib, orc, proj=proj)
+    ctx.destroy()
+    return lib
+
+
+# ---------------------------------------------------------------------------------------------
+# ONTHEFLY (methods 1 and 2): configs 1-3
+# ---------------------------------------------------------------------------------------------
+def test_config1_tiny_open_field_full_size():
+    w = W.config(1)
+    r = w.records()
+    lib = check(w, r, w.beams[0])
+    assert 100 < lib["n_survivors"] < 600  # 4x4 field at isocentre = +-1 cm on the 40x40 plane
+
+
+def test_config1_variants_no_jaws_and_zero_projection_distance():
+    w = W.config(1)
+    r = w.records()
+    check(w, r, None)
+    check(w, r, W.make_beam(jaws=(-100, 100, -100, 100), mu_weight=0.25))
+    flat = dict(z_src=-100.0, z_plane=0.0, z_jaw_x=0.0, z_jaw_y=0.0, z_map=0.0, z_iso=0.0)
+    w0 = W.Workload("cfg1_flat", w.n_records, w.gen, w.mode, w.grid, geometry=flat, beams=w.beams)
+    lib = check(w0, r, w.beams[0])
+    keep = (r["x"] >= -2) & (r["x"] < 2) & (r["y"] >= -2) & (r["y"] < 2)
+    assert lib["n_survivors"] == int(keep.sum())
+
+
+@pytest.mark.parametrize("mem", ["device", "pinned", "pageable"])
+def test_config2_chunked_equals_oracle(mem):
+    w = W.config(2, 300_000)
+    r = w.records()
+    check(w, r, None, chunk=w.chunk_records, mem=mem)
+
+
+def test_chunking_does_not_change_a_single_byte():
+    w = W.config(2, 12_000)
+    r = dirty(w.records(), 1)
+    ref = library_result(run_library(w, r, None, chunk=0))
+    for chunk in (4, 1000, 2048, 4096 + 4, 11_996):
+        got = library_result(run_library(w, r, None, chunk=chunk, max_records=len(r)))
+        for k in ("counts", "offsets", "src_index", "E", "x", "y", "u", "v", "w", "wt"):
+            assert np.array_equal(ref[k].view(np.uint32), got[k].view(np.uint32)), (chunk, k)
+        assert ref["stats"] == got["stats"], chunk
+
+
+def test_config3_jaws_and_fluence_map():
+    w = W.config(3, 400_000)
+    r = dirty(w.records(), 3)
+    lib = check(w, r, w.beams[0], flags=1, proj=True)
+    f = lib["n_survivors"] / len(r)
+    assert 0.10 < f < 0.16  # (15/40)^2 = 14 %
+
+
+def test_zero_weight_policy():
+    w = W.config(3, 200_000)
+    r = w.records()
+    m = W.fluence_uniform(5)
+    m[:, :80] = 0.0
+    beam = W.make_beam(jaws=(-15, 15, -15, 15), fluence=m, mu_weight=0.5)
+    kept = check(w, r, beam)
+    assert (kept["wt"] == 0).any()
+    dropped = check(w, r, beam, flags=2)
+    assert dropped["stats"]["n_zero_weight"] == int((kept["wt"] == 0).sum())
+
+
+def test_two_type_divisions_and_asymmetric_jaws():
+    w = W.config(3, 150_000)
+    g2 = dict(w.grid, n_types=2, n_ebins=10)
+    w2 = W.Workload("two_types", w.n_records, w.gen, w.mode, g2)
+    r = dirty(w2.records(), 8)
+    check(w2, r, W.make_beam(jaws=(2.0, 14.0, -12.0, -4.0), fluence=W.fluence_uniform(2), mu_weight=1.0 / 3.0))
+
+
+def test_many_keys_in_one_pass():
+    w = W.config(3, 120_000)
+    g = dict(w.grid, n_ebins=600)  # 1800 keys: close to the single-pass limit
+    w2 = W.Workload("many_keys", w.n_records, w.gen, w.mode, g)
+    check(w2, w2.records(), W.make_beam(jaws=(-20, 20, -20, 20)))
+
+
+@pytest.mark.parametrize("n", [0, 1, 3, 4, 5, 2047, 2048, 2049, 4100])
+def test_ragged_and_empty_inputs(n):
+    w = W.config(2, max(n, 1))
+    r = dirty(w.records(), n)[:n] if n >= 8 else w.records()[:n]
+    check(w, r, None)
+    w3 = W.config(3, max(n, 1))
+    check(w3, w3.records()[:n], w3.beams[0])
+
+
+def test_everything_rejected():
+    w = W.config(3, 10_000)
+    r = w.records()
+    lib = check(w, r, W.make_beam(jaws=(30, 31, 30, 31)))
+    assert lib["n_survivors"] == 0 and lib["stats"]["n_jaw_rejected"] == len(r)
+    bad = r.copy()
+    bad["type"] = 9
+    lib = check(w, bad, None)
+    assert lib["stats"]["n_invalid"] == len(r)
+
+
+def test_rebuild_with_another_beam_and_run_to_run_determinism():
+    w = W.config(3, 100_000)
+    r = w.records()
+    ctx = run_library(w, r, w.beams[0], chunk=30_000)
+    a = library_result(ctx)
+    ctx.build_batches(W.make_beam(jaws=(-3, 3, -3, 3)))
+    b = library_result(ctx)
+    assert_matches_oracle(b, O.Oracle(w.grid, w.geometry).build(r, W.make_beam(jaws=(-3, 3, -3, 3))))
+    ctx.build_batches(w.beams[0])
+    c = library_result(ctx)
+    for k in ("counts", "offsets", "src_index", "w", "wt"):
+        assert np.array_equal(a[k].view(np.uint32), c[k].view(np.uint32))
+    assert a["stats"] == c["stats"]  # including the double sums: fixed-order reductions
+    ctx.reset()
+    ctx.load_chunk(__import__("torch").from_numpy(r[:5000].view(np.uint8).reshape(-1).copy()).cuda())
+    ctx.build_batches(None)
+    assert_matches_oracle(library_result(ctx), O.Oracle(w.grid, w.geometry).build(r[:5000], None))
+    ctx.destroy()
+
+
+def test_per_batch_views():
+    w = W.config(2, 50_000)
+    r = w.records()
+    ctx = run_library(w, r, None)
+    orc = O.Oracle(w.grid, w.geometry).build(r, None)
+    total = 0
+    for t in range(3):
+        for ie in (0, 5, 17, 63):
+            b = ctx.get_batch(t, ie)
+            k = t * 64 + ie
+            assert b["first"] == orc["offsets"][k] and b["count"] == orc["counts"][k]
+            got = b["src_index"].cpu().numpy().view(np.uint32)
+            assert np.array_equal(got, orc["src_index"][orc["offsets"][k]:orc["offsets"][k + 1]])
+            assert np.array_equal(b["bin_offsets"].cpu().numpy().view(np.uint32), orc["offsets"][k:k + 2])
+            total += b["count"]
+    assert total > 0
+    ctx.destroy()
+
+
+# ---------------------------------------------------------------------------------------------
+# INDEX (method 3, the PSL method): configs 4 and 5
+# ---------------------------------------------------------------------------------------------
+def index_result(ctx):
+    lib = library_result(ctx)
+    return lib
+
+
+def test_config4_index_then_beam():
+    w = W.config(4, 500_000)
+    r = dirty(w.records(), 4)
+    ctx = run_library(w, r, None, chunk=120_000)
+    orc = O.Oracle(w.grid, w.geometry)
+    assert_matches_oracle(library_result(ctx), orc.build(r, None), index_only=True)
+    ctx.build_batches(w.beams[0])
+    lib = library_result(ctx)
+    assert_matches_oracle(lib, orc.build(r, w.beams[0]))
+    assert ctx.roi_bins(w.beams[0]) == (28, 51, 28, 51) == orc.roi_bins(w.beams[0])
+    assert lib["stats"]["n_roi_skipped"] > 0.85 * len(r)
+    # per-batch view with position-bin offsets
+    o = orc.build(r, w.beams[0])
+    b = ctx.get_batch(0, 5)
+    k0 = 5 * 6400
+    assert b["first"] == o["offsets"][k0] and b["count"] == o["offsets"][k0 + 6400] - o["offsets"][k0]
+    assert np.array_equal(b["bin_offsets"].cpu().numpy().view(np.uint32), o["offsets"][k0:k0 + 6401])
+    ctx.destroy()
+
+
+def test_index_roi_edge_cases():
+    w = W.config(4, 200_000)
+    r = w.records()
+    ctx = run_library(w, r, None)
+    orc = O.Oracle(w.grid, w.geometry)
+    beams = [
+        W.make_beam(jaws=(-5, 5, -5, 5), roi=(-20, 20, -20, 20)),            # whole plane
+        W.make_beam(jaws=(-5, 5, -5, 5)),                                    # no ROI at all
+        W.make_beam(jaws=(-5, 5, -5, 5), roi=(3.0, 3.0, -20, 20)),           # zero-width ROI: nothing
+        W.make_beam(jaws=(-5, 5, -5, 5), roi=(50, 60, 50, 60)),              # off the plane
+        W.make_beam(roi=(-0.5, 0.5, 0.0, 0.5)),                              # ROI only, edges on bin edges
+        W.make_beam(jaws=(-40, 40, -40, 40), roi=(-7.3, 2.2, 1.1, 19.9), fluence=W.fluence_uniform(9), mu_weight=0.125),
+        W.make_beam(jaws=(1, 9, -9, -1), roi=(-25, 25, -25, 25)),
+    ]
+    for beam in beams:
+        ctx.build_batches(beam)
+        if beam["roi"] is not None:
+            ls, os_ = ctx.roi_bins(beam), orc.roi_bins(beam)
+            empty = lambda s: s[0] > s[1] or s[2] > s[3]  # noqa: E731
+            assert ls == os_ or (empty(ls) and empty(os_))
+        assert_matches_oracle(library_result(ctx), orc.build(r, beam))
+    ctx.destroy()
+
+
+def test_index_with_drop_zero_weight_and_projection_outputs():
+    w = W.config(4, 150_000)
+    r = w.records()
+    m = W.fluence_uniform(6)
+    m[80:, :] = 0.0
+    beam = W.make_beam(jaws=(-8, 8, -8, 8), fluence=m, roi=(-6, 6, -6, 6))
+    ctx = run_library(w, r, beam, flags=3)
+    assert_matches_oracle(library_result(ctx), O.Oracle(w.grid, w.geometry, flags=2).build(r, beam), proj=True)
+    ctx.destroy()
+
+
+@pytest.mark.parametrize("mem", ["pinned", "pageable", "device"])
+def test_config5_streamed_imrt_beams(mem):
+    w = W.config(5, 700_000)
+    r = w.records()
+    ctx = run_library(w, r, None, chunk=w.chunk_records, mem=mem)
+    orc = O.Oracle(w.grid, w.geometry)
+    assert_matches_oracle(library_result(ctx), orc.build(r, None), index_only=True)
+    for beam in w.beams:
+        ctx.build_batches(beam)
+        assert_matches_oracle(library_result(ctx), orc.build(r, beam))
+    ctx.destroy()
+
+
+def test_paper_sized_psl_grid_two_types():
+    # 20x20 cm^2, 1-cm bins, 10 energy bins, 2 type divisions = 8000 PSLs
+    g = W._grid(n_types=2, n_ebins=10, n_xbins=20, n_ybins=20, x_min=-10.0, y_min=-10.0, dx=1.0, dy=1.0)
+    w = W.Workload("paper_psl", 300_000, W.GenParams(77), W.MODE_INDEX, g)
+    r = dirty(w.records(), 6)
+    beam = W.make_beam(jaws=(-5, 5, -5, 5), roi=(-3.2, 3.2, -3.2, 3.2), fluence=W.fluence_uniform(1))
+    ctx = run_library(w, r, None)
+    orc = O.Oracle(g, w.geometry)
+    assert_matches_oracle(library_result(ctx), orc.build(r, None), index_only=True)
+    ctx.build_batches(beam)
+    assert_matches_oracle(library_result(ctx), orc.build(r, beam))
+    ctx.destroy()
+
+
+@pytest.mark.parametrize("n", [0, 1, 5, 2049])
+def test_index_ragged_and_empty(n):
+    w = W.config(4, max(n, 1))
+    r = w.records()[:n]
+    ctx = run_library(w, r, None)
+    orc = O.Oracle(w.grid, w.geometry)
+    assert_matches_oracle(library_result(ctx), orc.build(r, None), index_only=True)
+    ctx.build_batches(w.beams[0])
+    assert_matches_oracle(library_result(ctx), orc.build(r, w.beams[0]))
+    ctx.destroy()
+
+
+# ---------------------------------------------------------------------------------------------
+# error behaviour
+# ---------------------------------------------------------------------------------------------
+def test_error_codes():
+    import torch
+
+    p = P()
+    w = W.config(4, 10_000)
+    r = w.records()
+    raw = torch.from_numpy(r.view(np.uint8).reshape(-1).copy()).cuda()
+    ctx = p.PslContext(w.grid, w.geometry, w.mode, max_records=10_000, max_beam_records=16)
+    with pytest.raises(p.PslError) as e:
+        ctx.get_batch(0, 0)
+    assert e.value.status_name == "PSL_ERR_STATE"
+    ctx.load_chunk(raw)
+    with pytest.raises(p.PslError) as e:
+        ctx.load_chunk(raw[:28 * 4])
+    assert e.value.status_name == "PSL_ERR_CAPACITY"
+    ctx.build_batches(None)
+    with pytest.raises(p.PslError) as e:
+        ctx.load_chunk(raw[:28 * 4])
+    assert e.value.status_name == "PSL_ERR_STATE"
+    with pytest.raises(p.PslError) as e:
+        ctx.build_batches(w.beams[0])  # ROI selects far more than max_beam_records = 16
+    assert e.value.status_name == "PSL_ERR_CAPACITY"
+    with pytest.raises(p.PslError) as e:
+        ctx.get_batch(3, 0)
+    assert e.value.status_name == "PSL_ERR_ARG"
+    ctx.destroy()
+    w2 = W.config(2, 1000)
+    ctx = p.PslContext(w2.grid, w2.geometry, w2.mode, max_records=1000)
+    ctx.load_chunk(raw[:28 * 6])  # 6 records: not a multiple of 4 -> must be the last chunk
+    with pytest.raises(p.PslError) as e:
+        ctx.load_chunk(raw[:28 * 4])
+    assert e.value.status_name == "PSL_ERR_ARG"
+    with pytest.raises(p.PslError) as e:
+        ctx.build_batches(W.make_beam(roi=(-1, 1, -1, 1)))  # ROI needs the index
+    assert e.value.status_name == "PSL_ERR_ARG"
+    ctx.destroy()
+
+
+# ---------------------------------------------------------------------------------------------
+# full size, in the launch configuration bench.py times (config 2: 1e7 records, ten 1e6-record device chunks)
+# ---------------------------------------------------------------------------------------------
+def test_config2_full_size_element_by_element():
+    w = W.config(2)
+    r = w.records()
+    check(w, r, None, chunk=w.chunk_records, mem="device")
