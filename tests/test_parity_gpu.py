@@ -113,7 +113,7 @@ def test_ragged_and_empty_inputs(n):
 def test_everything_rejected():
     w = W.config(3, 10_000)
     r = w.records()
-    lib = check(w, r, W.make_beam(jaws=(30, 31, 30, 31)))
+    lib = check(w, r, W.make_beam(jaws=(50, 51, 50, 51)))
     assert lib["n_survivors"] == 0 and lib["stats"]["n_jaw_rejected"] == len(r)
     bad = r.copy()
     bad["type"] = 9
