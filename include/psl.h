@@ -186,6 +186,24 @@ const char* psl_last_error(const psl_ctx* ctx);
 /* Number of kernels this context has launched since creation (for bench.py's gpu_launches). */
 uint64_t psl_kernel_launches(const psl_ctx* ctx);
 
+/* Optional device-side timing of the library's own kernels, by class, with CUDA events recorded on the
+ * context's stream around each launch (a few microseconds of overhead per build while enabled). */
+enum { PSL_K_COUNT = 0,   /* histogram passes (a8) */
+       PSL_K_SCAN = 1,    /* exclusive scans (a9) */
+       PSL_K_SCATTER = 2, /* ONTHEFLY decode + jaw + fluence + stable scatter (a1-a7, a10) */
+       PSL_K_INDEX_A = 3, /* INDEX pass A scatter (a11) */
+       PSL_K_INDEX_B = 4, /* INDEX pass B scatter (a11) */
+       PSL_K_BEAM = 5,    /* per-beam ROI + jaw + fluence + compaction from the index (a5-a7, a10) */
+       PSL_K_OTHER = 6,   /* offsets / statistics / tile descriptors */
+       PSL_K_CLASSES = 7 };
+typedef struct {
+    double ms[PSL_K_CLASSES];         /* summed device time */
+    uint64_t launches[PSL_K_CLASSES]; /* timed brackets (SCAN: one bracket = its three kernels) */
+} psl_profile;
+psl_status psl_profile_enable(psl_ctx* ctx, int32_t on);
+/* Synchronises the stream, returns the totals since the last read (or enable) and clears them. */
+psl_status psl_profile_read(psl_ctx* ctx, psl_profile* out);
+
 #ifdef __cplusplus
 }
 #endif

@@ -77,6 +77,13 @@ class Batch(C.Structure):
                [("n_bins", C.c_uint32)]
 
 
+K_CLASSES = ("count", "scan", "scatter", "index_a", "index_b", "beam", "other")
+
+
+class Profile(C.Structure):
+    _fields_ = [("ms", C.c_double * 7), ("launches", C.c_uint64 * 7)]
+
+
 _lib = None
 
 
@@ -131,6 +138,10 @@ def load_library(build: bool = True):
     lib.psl_last_error.argtypes = [C.c_void_p]
     lib.psl_kernel_launches.restype = C.c_uint64
     lib.psl_kernel_launches.argtypes = [C.c_void_p]
+    lib.psl_profile_enable.restype = C.c_int
+    lib.psl_profile_enable.argtypes = [C.c_void_p, C.c_int32]
+    lib.psl_profile_read.restype = C.c_int
+    lib.psl_profile_read.argtypes = [C.c_void_p, P(Profile)]
     _lib = lib
     return lib
 
@@ -324,6 +335,15 @@ class PslContext:
 
     def kernel_launches(self) -> int:
         return int(self.lib.psl_kernel_launches(self._h))
+
+    def profile_enable(self, on: bool = True):
+        self._check(self.lib.psl_profile_enable(self._h, 1 if on else 0))
+
+    def profile_read(self) -> Dict:
+        """{class: (total ms, timed launches)} since the last read; synchronises"""
+        p = Profile()
+        self._check(self.lib.psl_profile_read(self._h, C.byref(p)))
+        return {name: (p.ms[i], int(p.launches[i])) for i, name in enumerate(K_CLASSES)}
 
     def destroy(self):
         if getattr(self, "_h", None) is not None and self._h:

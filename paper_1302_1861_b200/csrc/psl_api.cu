@@ -216,6 +216,11 @@ struct psl_ctx {
     DevStats idx_stats = {};
     uint64_t n_idx = 0, last_M = 0;
     uint64_t launches = 0;
+    // optional kernel timing (psl_profile_*)
+    bool profiling = false;
+    struct Bracket { int cls; cudaEvent_t a, b; };
+    std::vector<Bracket> brackets;        // recorded since the last read
+    std::vector<cudaEvent_t> event_pool;  // timing events ready for reuse
     char err[256] = "";
 };
 
@@ -235,6 +240,43 @@ namespace {
         ctx->launches += 1;                           \
         CU(cudaGetLastError());                       \
     } while (0)
+
+cudaEvent_t prof_event(psl_ctx* ctx)
+{
+    cudaEvent_t e = nullptr;
+    if (!ctx->event_pool.empty()) {
+        e = ctx->event_pool.back();
+        ctx->event_pool.pop_back();
+    } else if (cudaEventCreate(&e) != cudaSuccess) {
+        e = nullptr;
+    }
+    return e;
+}
+
+// RAII bracket: records a timing event on the stream before and after the launches in its scope
+struct Prof {
+    psl_ctx* ctx;
+    int cls;
+    cudaEvent_t a = nullptr;
+    Prof(psl_ctx* c, int k) : ctx(c), cls(k)
+    {
+        if (ctx->profiling && ctx->brackets.size() < 65536) {
+            a = prof_event(ctx);
+            if (a) cudaEventRecord(a, ctx->stream);
+        }
+    }
+    ~Prof()
+    {
+        if (!a) return;
+        cudaEvent_t b = prof_event(ctx);
+        if (b) {
+            cudaEventRecord(b, ctx->stream);
+            ctx->brackets.push_back({cls, a, b});
+        } else {
+            ctx->event_pool.push_back(a);
+        }
+    }
+};
 
 template <typename T>
 T* at(psl_ctx* ctx, uint64_t off) { return reinterpret_cast<T*>(ctx->ws + off); }
@@ -349,6 +391,7 @@ psl_status run_scan(psl_ctx* ctx, uint32_t* table, uint32_t B, uint32_t n_tiles,
     uint32_t L = (uint32_t)L64;
     uint32_t nb = (uint32_t)((L64 + kScanBlock - 1) / kScanBlock);
     uint32_t* sums = at<uint32_t>(ctx, ctx->L.scan_sums);
+    Prof prof(ctx, PSL_K_SCAN);
     k_scan_reduce<<<nb, kScanThreads, 0, ctx->stream>>>(table, n_tiles, stride, L, sums);
     LAUNCHED();
     k_scan_sums<<<1, 1024, 0, ctx->stream>>>(sums, nb, total_dev);
@@ -389,16 +432,22 @@ psl_status build_onthefly(psl_ctx* ctx, const DevBeam& bm)
         TileStats* ts = at<TileStats>(ctx, L.tstats);
         uint32_t sm_count = tile_smem_bytes(kTile * kRecBytes, d.K, ctx->cfg.n_ebins + 1, false, false);
         uint32_t sm_scatter = tile_smem_bytes(kTile * kRecBytes, d.K, ctx->cfg.n_ebins + 1, true, true);
-        k_count_raw<false><<<nt, kThreads, sm_count, ctx->stream>>>(tiles, 0, ctx->grid, bm, d.K, 0, table, d.tiles_cap, ts);
-        LAUNCHED();
+        {
+            Prof prof(ctx, PSL_K_COUNT);
+            k_count_raw<false><<<nt, kThreads, sm_count, ctx->stream>>>(tiles, 0, ctx->grid, bm, d.K, 0, table, d.tiles_cap, ts);
+            LAUNCHED();
+        }
         psl_status s = run_scan(ctx, table, d.K, nt, d.tiles_cap, scalar(ctx, SC_TOTAL));
         if (s != PSL_OK) return s;
         k_offsets_from_table<<<(d.K + 1 + 255) / 256, 256, 0, ctx->stream>>>(table, d.tiles_cap, d.K, scalar(ctx, SC_TOTAL),
                                                                            offsets, counts, d.n_pos, d.n_batches, batch_off);
         LAUNCHED();
-        k_scatter_otf<<<nt, kThreads, sm_scatter, ctx->stream>>>(tiles, ctx->grid, bm, d.K, table, d.tiles_cap,
-                                                                soa_out(ctx, L.out), ts);
-        LAUNCHED();
+        {
+            Prof prof(ctx, PSL_K_SCATTER);
+            k_scatter_otf<<<nt, kThreads, sm_scatter, ctx->stream>>>(tiles, ctx->grid, bm, d.K, table, d.tiles_cap,
+                                                                    soa_out(ctx, L.out), ts);
+            LAUNCHED();
+        }
         k_reduce_stats<<<1, 1024, 0, ctx->stream>>>(ts, nt, stats);
         LAUNCHED();
     }
@@ -448,16 +497,25 @@ psl_status finalize_index(psl_ctx* ctx)
         psl_status s = run_scan(ctx, table_a, d.B_lo, nt, d.tiles_cap, scalar(ctx, SC_NIDX));
         if (s != PSL_OK) return s;
         uint32_t sm_a = tile_smem_bytes(kTile * kRecBytes, d.B_lo, ctx->cfg.n_ebins + 1, true, false);
-        k_scatter_idx_a<<<nt, kThreads, sm_a, ctx->stream>>>(tiles, ctx->grid, none, d.B_lo, d.lo_bits, table_a, d.tiles_cap, aos, hi16);
-        LAUNCHED();
+        {
+            Prof prof(ctx, PSL_K_INDEX_A);
+            k_scatter_idx_a<<<nt, kThreads, sm_a, ctx->stream>>>(tiles, ctx->grid, none, d.B_lo, d.lo_bits, table_a, d.tiles_cap, aos, hi16);
+            LAUNCHED();
+        }
         uint32_t ntb = (uint32_t)((ctx->n_records + kTile - 1) / kTile);
-        k_count_hi16<<<ntb, kThreads, d.B_hi * 4, ctx->stream>>>(hi16, scalar(ctx, SC_NIDX), d.B_hi, table_b, d.tiles_b_cap);
-        LAUNCHED();
+        {
+            Prof prof(ctx, PSL_K_COUNT);
+            k_count_hi16<<<ntb, kThreads, d.B_hi * 4, ctx->stream>>>(hi16, scalar(ctx, SC_NIDX), d.B_hi, table_b, d.tiles_b_cap);
+            LAUNCHED();
+        }
         s = run_scan(ctx, table_b, d.B_hi, ntb, d.tiles_b_cap, scalar(ctx, SC_TOTAL));
         if (s != PSL_OK) return s;
         uint32_t sm_b = tile_smem_bytes(kTile * 32, d.B_hi, 0, true, true);
-        k_scatter_idx_b<<<ntb, kThreads, sm_b, ctx->stream>>>(aos, hi16, scalar(ctx, SC_NIDX), d.B_hi, table_b, d.tiles_b_cap, idx_out(ctx));
-        LAUNCHED();
+        {
+            Prof prof(ctx, PSL_K_INDEX_B);
+            k_scatter_idx_b<<<ntb, kThreads, sm_b, ctx->stream>>>(aos, hi16, scalar(ctx, SC_NIDX), d.B_hi, table_b, d.tiles_b_cap, idx_out(ctx));
+            LAUNCHED();
+        }
         k_offsets_by_search<<<(d.K + 1 + 255) / 256, 256, 0, ctx->stream>>>(at<uint32_t>(ctx, L.keyfull), scalar(ctx, SC_NIDX), d.K, idx_offsets);
         LAUNCHED();
         k_counts_from_offsets<<<(d.K + 1 + 255) / 256, 256, 0, ctx->stream>>>(idx_offsets, d.K, idx_counts, d.n_pos, d.n_batches, idx_batch);
@@ -546,11 +604,14 @@ psl_status build_beam_from_index(psl_ctx* ctx, const psl_beam* beam, const DevBe
         in.E = at<float>(ctx, L.idx[0]); in.x = at<float>(ctx, L.idx[1]); in.y = at<float>(ctx, L.idx[2]);
         in.u = at<float>(ctx, L.idx[3]); in.v = at<float>(ctx, L.idx[4]); in.wt = at<float>(ctx, L.idx[5]);
         in.src = at<uint32_t>(ctx, L.idx[6]);
-        k_beam_compact<<<nt, kThreads, 11 * kTile * 4, ctx->stream>>>(st, in, ctx->grid, bm, soa_out(ctx, L.beam_out), beam_keys,
-                                                                     at<unsigned long long>(ctx, L.lookback),
-                                                                     scalar(ctx, SC_TILE_COUNTER), at<BeamTileStats>(ctx, L.bstats),
-                                                                     scalar(ctx, SC_BEAM_NSURV));
-        LAUNCHED();
+        {
+            Prof prof(ctx, PSL_K_BEAM);
+            k_beam_compact<<<nt, kThreads, 11 * kTile * 4, ctx->stream>>>(st, in, ctx->grid, bm, soa_out(ctx, L.beam_out), beam_keys,
+                                                                         at<unsigned long long>(ctx, L.lookback),
+                                                                         scalar(ctx, SC_TILE_COUNTER), at<BeamTileStats>(ctx, L.bstats),
+                                                                         scalar(ctx, SC_BEAM_NSURV));
+            LAUNCHED();
+        }
         k_reduce_beam_stats<<<1, 1024, 0, ctx->stream>>>(at<BeamTileStats>(ctx, L.bstats), nt, bstat);
         LAUNCHED();
     }
@@ -628,6 +689,11 @@ void psl_destroy(psl_ctx* ctx)
     cudaEvent_t evs[] = {ctx->ev_chunk, ctx->ev_main, ctx->ev_batch, ctx->ev_seg, ctx->ev_stage[0], ctx->ev_stage[1]};
     for (cudaEvent_t e : evs)
         if (e) cudaEventDestroy(e);
+    for (auto& br : ctx->brackets) {
+        cudaEventDestroy(br.a);
+        cudaEventDestroy(br.b);
+    }
+    for (cudaEvent_t e : ctx->event_pool) cudaEventDestroy(e);
     void* hp[] = {ctx->h_stage[0], ctx->h_stage[1], ctx->h_batch_off, ctx->h_idx_offsets, ctx->h_seg, ctx->h_stats,
                   ctx->h_beam_stats, ctx->h_scalars};
     for (void* p : hp)
@@ -783,6 +849,7 @@ psl_status psl_load_chunk(psl_ctx* ctx, const void* records, uint64_t n, int32_t
         DevBeam none;
         memset(&none, 0, sizeof none);
         uint32_t sm = tile_smem_bytes(kTile * kRecBytes, ctx->d.B_lo, ctx->cfg.n_ebins + 1, false, false);
+        Prof prof(ctx, PSL_K_COUNT);
         k_count_raw<true><<<nt, kThreads, sm, ctx->stream>>>(tiles, tile0, ctx->grid, none, ctx->d.B_lo, (1u << ctx->d.lo_bits) - 1u,
                                                             at<uint32_t>(ctx, ctx->L.table_a), ctx->d.tiles_cap,
                                                             at<TileStats>(ctx, ctx->L.tstats));
@@ -871,6 +938,32 @@ psl_status psl_get_batch(psl_ctx* ctx, int32_t t, int32_t ie, psl_batch* out)
         out->src_index = at<uint32_t>(ctx, o[9]) + first;
         out->bin_offsets = at<uint32_t>(ctx, ctx->result == RES_OTF ? L.offsets : L.beam_offsets) + (uint64_t)b * d.n_pos;
     }
+    return PSL_OK;
+}
+
+psl_status psl_profile_enable(psl_ctx* ctx, int32_t on)
+{
+    if (!ctx) return PSL_ERR_ARG;
+    ctx->profiling = on != 0;
+    return PSL_OK;
+}
+
+psl_status psl_profile_read(psl_ctx* ctx, psl_profile* out)
+{
+    if (!ctx || !out) return PSL_ERR_ARG;
+    CU(cudaSetDevice(ctx->cfg.device));
+    CU(cudaStreamSynchronize(ctx->stream));
+    memset(out, 0, sizeof *out);
+    for (auto& br : ctx->brackets) {
+        float ms = 0.0f;
+        if (cudaEventElapsedTime(&ms, br.a, br.b) == cudaSuccess) {
+            out->ms[br.cls] += (double)ms;
+            out->launches[br.cls] += 1;
+        }
+        ctx->event_pool.push_back(br.a);
+        ctx->event_pool.push_back(br.b);
+    }
+    ctx->brackets.clear();
     return PSL_OK;
 }
 

@@ -14,7 +14,7 @@ def test_library_loads_and_exports_every_declared_symbol():
     lib = P.load_library()
     names = P.exported_symbols()
     assert {"psl_create", "psl_load_chunk", "psl_build_batches", "psl_get_batch"} <= set(names)  # north_star's four
-    assert len(names) == 14
+    assert len(names) == 16
     for n in names:
         assert hasattr(lib, n), n
 
