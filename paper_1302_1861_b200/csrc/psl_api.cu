@@ -28,7 +28,7 @@ constexpr uint64_t kStageBytes = 32ull << 20;  // pinned staging buffers for pag
 
 struct Layout {
     uint64_t total = 0;
-    uint64_t raw = 0, tiles = 0, tstats = 0, scan_sums = 0, scalars = 0, edges = 0, stats = 0, batch_off = 0;
+    uint64_t raw = 0, chunks = 0, sstats = 0, scan_sums = 0, scalars = 0, edges = 0, stats = 0, batch_off = 0;
     // ONTHEFLY
     uint64_t table = 0, out[10] = {0}, offsets = 0, counts = 0;
     // INDEX
@@ -41,7 +41,7 @@ struct Layout {
 struct Derived {
     uint32_t K = 0, n_batches = 0, n_pos = 0;
     uint32_t lo_bits = 0, B_lo = 0, B_hi = 0;
-    uint32_t tiles_cap = 0, tiles_b_cap = 0, max_chunks = 0;
+    uint32_t tiles_cap = 0, cols_cap = 0, max_chunks = 0;  // cols = table columns = segments over all launches
     uint64_t max_beam = 0;
     uint32_t max_seg = 0;
     uint32_t scan_blocks_cap = 0;
@@ -108,30 +108,35 @@ psl_status derive(const psl_config* c, Derived* d, char* err)
     d->n_batches = (uint32_t)(c->n_types * c->n_ebins);
     d->max_chunks = c->max_chunks ? c->max_chunks : 4096u;
     uint64_t tiles_cap = (c->max_records + kTile - 1) / kTile + d->max_chunks;
-    d->tiles_b_cap = (uint32_t)((c->max_records + kTile - 1) / kTile);
+    // ONTHEFLY builds in one launch over all chunks; INDEX counts chunk by chunk as the chunks land
+    uint64_t cols_cap = kMaxSegments;
+    if (c->mode == PSL_MODE_INDEX) {
+        cols_cap = (uint64_t)d->max_chunks * kMaxSegments;
+        if (cols_cap > tiles_cap) cols_cap = tiles_cap;
+    }
     if (c->mode == PSL_MODE_ONTHEFLY) {
         if (K > kMaxBuckets) { set_err(err, "ONTHEFLY mode handles at most %d keys (got %llu); use PSL_MODE_INDEX", kMaxBuckets, (unsigned long long)K); return PSL_ERR_ARG; }
-        if (K * tiles_cap >= (1ull << 32)) { set_err(err, "keys x tiles overflows 32 bits"); return PSL_ERR_CAPACITY; }
     } else {
         if (K > (uint64_t)kMaxBuckets * kMaxBuckets) { set_err(err, "INDEX mode handles at most %d keys", kMaxBuckets * kMaxBuckets); return PSL_ERR_ARG; }
         uint32_t bits = 0;
         while ((1ull << bits) < K) ++bits;  // K <= 2^bits
-        uint32_t lo = (bits + 1) / 2;
+        uint32_t lo = bits / 2;  // the smaller digit goes to pass A (its counters are the larger share of its shared memory)
         while ((((K - 1) >> lo) + 1) > (uint64_t)kMaxBuckets) ++lo;
         d->lo_bits = lo;
         d->B_lo = (uint32_t)((K < (1ull << lo)) ? K : (1ull << lo));
         if (d->B_lo < 1) d->B_lo = 1;
         d->B_hi = (uint32_t)(((K - 1) >> lo) + 1);
-        if ((uint64_t)d->B_lo * tiles_cap >= (1ull << 32) || (uint64_t)d->B_hi * d->tiles_b_cap >= (1ull << 32)) { set_err(err, "buckets x tiles overflows 32 bits"); return PSL_ERR_CAPACITY; }
+        if ((uint64_t)d->B_lo * cols_cap >= (1ull << 32)) { set_err(err, "buckets x segments overflows 32 bits"); return PSL_ERR_CAPACITY; }
         d->max_beam = c->max_beam_records ? c->max_beam_records : c->max_records;
         if (d->max_beam > c->max_records) d->max_beam = c->max_records;
         d->max_seg = d->n_batches * (uint32_t)c->n_ybins;
     }
     d->tiles_cap = (uint32_t)tiles_cap;
-    uint64_t Lmax = c->mode == PSL_MODE_ONTHEFLY ? K * tiles_cap
-                                                  : ((uint64_t)d->B_lo * tiles_cap > (uint64_t)d->B_hi * d->tiles_b_cap
-                                                         ? (uint64_t)d->B_lo * tiles_cap
-                                                         : (uint64_t)d->B_hi * d->tiles_b_cap);
+    d->cols_cap = (uint32_t)cols_cap;
+    uint64_t Lmax = c->mode == PSL_MODE_ONTHEFLY ? K * cols_cap
+                                                  : ((uint64_t)d->B_lo * cols_cap > (uint64_t)d->B_hi * kMaxSegments
+                                                         ? (uint64_t)d->B_lo * cols_cap
+                                                         : (uint64_t)d->B_hi * kMaxSegments);
     d->scan_blocks_cap = (uint32_t)((Lmax + kScanBlock - 1) / kScanBlock);
     return PSL_OK;
 }
@@ -149,21 +154,21 @@ void plan(const psl_config* c, const Derived& d, Layout* L)
     const uint64_t N = c->max_records;
     const bool proj = (c->flags & PSL_OUT_PROJ) != 0;
     L->raw = take(&cur, c->max_host_records * kRecBytes);
-    L->tiles = take(&cur, (uint64_t)d.tiles_cap * sizeof(TileDesc));
-    L->tstats = take(&cur, (uint64_t)d.tiles_cap * sizeof(TileStats));
+    L->chunks = take(&cur, (uint64_t)d.max_chunks * sizeof(ChunkDesc));
+    L->sstats = take(&cur, (uint64_t)d.cols_cap * sizeof(SegStats));
     L->scan_sums = take(&cur, (uint64_t)(d.scan_blocks_cap + 1) * 4);
     L->scalars = take(&cur, 64);
     L->edges = take(&cur, (uint64_t)(c->n_ebins + 1) * 4);
     L->stats = take(&cur, sizeof(DevStats));
     L->batch_off = take(&cur, (uint64_t)(d.n_batches + 1) * 4);
     if (c->mode == PSL_MODE_ONTHEFLY) {
-        L->table = take(&cur, (uint64_t)d.K * d.tiles_cap * 4);
+        L->table = take(&cur, (uint64_t)d.K * d.cols_cap * 4);
         for (int i = 0; i < 10; ++i) L->out[i] = ((i == 7 || i == 8) && !proj) ? 0 : take(&cur, N * 4);
         L->offsets = take(&cur, (uint64_t)(d.K + 1) * 4);
         L->counts = take(&cur, (uint64_t)d.K * 4);
     } else {
-        L->table_a = take(&cur, (uint64_t)d.B_lo * d.tiles_cap * 4);
-        L->table_b = take(&cur, (uint64_t)d.B_hi * d.tiles_b_cap * 4);
+        L->table_a = take(&cur, (uint64_t)d.B_lo * d.cols_cap * 4);
+        L->table_b = take(&cur, (uint64_t)d.B_hi * kMaxSegments * 4);
         L->aos = take(&cur, N * 32);
         L->hi16 = take(&cur, N * 2);
         for (int i = 0; i < 7; ++i) L->idx[i] = take(&cur, N * 4);
@@ -176,7 +181,7 @@ void plan(const psl_config* c, const Derived& d, Layout* L)
         L->beam_keys = take(&cur, d.max_beam * 4);
         L->beam_offsets = take(&cur, (uint64_t)(d.K + 1) * 4);
         L->beam_counts = take(&cur, (uint64_t)d.K * 4);
-        uint64_t bt = (d.max_beam + kTile - 1) / kTile + 1;
+        uint64_t bt = (d.max_beam + kBeamTile - 1) / kBeamTile + 1;
         L->lookback = take(&cur, bt * 8);
         L->bstats = take(&cur, bt * sizeof(BeamTileStats));
         L->beam_stats = take(&cur, sizeof(DevBeamStats));
@@ -207,9 +212,14 @@ struct psl_ctx {
     DevBeamStats* h_beam_stats = nullptr;
     uint32_t* h_scalars = nullptr;
     bool seg_pending = false;
+    // launch shapes: persistent CTAs per launch (= SMs x resident CTAs of the scatter kernel, one wave)
+    uint32_t S_otf = 0, S_a = 0, S_b = 0;
+    uint32_t sm_count_raw = 0, sm_scatter_otf = 0, sm_idx_a = 0, sm_count_b = 0, sm_idx_b = 0;  // dynamic smem bytes
+    struct ChunkLaunch { Span span; uint32_t n_seg; };
+    std::vector<ChunkLaunch> idx_launches;  // INDEX: the per-chunk count launches, replayed by pass A's scatter
     // state
     uint64_t n_records = 0, n_host_records = 0;
-    uint32_t n_tiles = 0, n_chunks = 0;
+    uint32_t n_tiles = 0, n_chunks = 0, n_cols = 0;
     bool ragged = false;  // a chunk with n % 4 != 0 was loaded: no more chunks may follow
     bool indexed = false;
     int result = RES_NONE;
@@ -385,18 +395,18 @@ cudaError_t allow_smem(Kern k, uint32_t bytes)
 }
 
 // exclusive scan of table (virtual order bucket-major, tile-minor); grand total -> *total_dev
-psl_status run_scan(psl_ctx* ctx, uint32_t* table, uint32_t B, uint32_t n_tiles, uint32_t stride, uint32_t* total_dev)
+psl_status run_scan(psl_ctx* ctx, uint32_t* table, uint32_t B, uint32_t n_cols, uint32_t stride, uint32_t* total_dev)
 {
-    uint64_t L64 = (uint64_t)B * n_tiles;
+    uint64_t L64 = (uint64_t)B * n_cols;
     uint32_t L = (uint32_t)L64;
     uint32_t nb = (uint32_t)((L64 + kScanBlock - 1) / kScanBlock);
     uint32_t* sums = at<uint32_t>(ctx, ctx->L.scan_sums);
     Prof prof(ctx, PSL_K_SCAN);
-    k_scan_reduce<<<nb, kScanThreads, 0, ctx->stream>>>(table, n_tiles, stride, L, sums);
+    k_scan_reduce<<<nb, kScanThreads, 0, ctx->stream>>>(table, n_cols, stride, L, sums);
     LAUNCHED();
     k_scan_sums<<<1, 1024, 0, ctx->stream>>>(sums, nb, total_dev);
     LAUNCHED();
-    k_scan_apply<<<nb, kScanThreads, 0, ctx->stream>>>(table, n_tiles, stride, L, sums);
+    k_scan_apply<<<nb, kScanThreads, 0, ctx->stream>>>(table, n_cols, stride, L, sums);
     LAUNCHED();
     return PSL_OK;
 }
@@ -428,27 +438,28 @@ psl_status build_onthefly(psl_ctx* ctx, const DevBeam& bm)
         CU(cudaMemsetAsync(batch_off, 0, (uint64_t)(d.n_batches + 1) * 4, ctx->stream));
         CU(cudaMemsetAsync(stats, 0, sizeof(DevStats), ctx->stream));
     } else {
-        const TileDesc* tiles = at<TileDesc>(ctx, L.tiles);
-        TileStats* ts = at<TileStats>(ctx, L.tstats);
-        uint32_t sm_count = tile_smem_bytes(kTile * kRecBytes, d.K, ctx->cfg.n_ebins + 1, false, false);
-        uint32_t sm_scatter = tile_smem_bytes(kTile * kRecBytes, d.K, ctx->cfg.n_ebins + 1, true, true);
+        const ChunkDesc* chunks = at<ChunkDesc>(ctx, L.chunks);
+        SegStats* ss = at<SegStats>(ctx, L.sstats);
+        const uint32_t S = nt < ctx->S_otf ? nt : ctx->S_otf;  // one persistent CTA per segment, one wave
+        const Span span = {0u, nt, 0u};
         {
             Prof prof(ctx, PSL_K_COUNT);
-            k_count_raw<false><<<nt, kThreads, sm_count, ctx->stream>>>(tiles, 0, ctx->grid, bm, d.K, 0, table, d.tiles_cap, ts);
+            k_count_raw<false><<<S, kThreads, ctx->sm_count_raw, ctx->stream>>>(chunks, ctx->n_chunks, span, ctx->grid, bm, d.K, 0,
+                                                                              table, d.cols_cap, ss);
             LAUNCHED();
         }
-        psl_status s = run_scan(ctx, table, d.K, nt, d.tiles_cap, scalar(ctx, SC_TOTAL));
+        psl_status s = run_scan(ctx, table, d.K, S, d.cols_cap, scalar(ctx, SC_TOTAL));
         if (s != PSL_OK) return s;
-        k_offsets_from_table<<<(d.K + 1 + 255) / 256, 256, 0, ctx->stream>>>(table, d.tiles_cap, d.K, scalar(ctx, SC_TOTAL),
+        k_offsets_from_table<<<(d.K + 1 + 255) / 256, 256, 0, ctx->stream>>>(table, d.cols_cap, d.K, scalar(ctx, SC_TOTAL),
                                                                            offsets, counts, d.n_pos, d.n_batches, batch_off);
         LAUNCHED();
         {
             Prof prof(ctx, PSL_K_SCATTER);
-            k_scatter_otf<<<nt, kThreads, sm_scatter, ctx->stream>>>(tiles, ctx->grid, bm, d.K, table, d.tiles_cap,
-                                                                    soa_out(ctx, L.out), ts);
+            k_scatter_otf<<<S, kThreads, ctx->sm_scatter_otf, ctx->stream>>>(chunks, ctx->n_chunks, span, ctx->grid, bm, d.K, table,
+                                                                            d.cols_cap, soa_out(ctx, L.out), ss);
             LAUNCHED();
         }
-        k_reduce_stats<<<1, 1024, 0, ctx->stream>>>(ts, nt, stats);
+        k_reduce_stats<<<1, 1024, 0, ctx->stream>>>(ss, S, stats);
         LAUNCHED();
     }
     CU(cudaMemcpyAsync(ctx->h_batch_off, batch_off, (uint64_t)(d.n_batches + 1) * 4, cudaMemcpyDeviceToHost, ctx->stream));
@@ -489,38 +500,42 @@ psl_status finalize_index(psl_ctx* ctx)
     } else {
         DevBeam none;
         memset(&none, 0, sizeof none);
-        const TileDesc* tiles = at<TileDesc>(ctx, L.tiles);
+        const ChunkDesc* chunks = at<ChunkDesc>(ctx, L.chunks);
         uint32_t* table_a = at<uint32_t>(ctx, L.table_a);
         uint32_t* table_b = at<uint32_t>(ctx, L.table_b);
         uint4* aos = at<uint4>(ctx, L.aos);
         uint16_t* hi16 = at<uint16_t>(ctx, L.hi16);
-        psl_status s = run_scan(ctx, table_a, d.B_lo, nt, d.tiles_cap, scalar(ctx, SC_NIDX));
+        psl_status s = run_scan(ctx, table_a, d.B_lo, ctx->n_cols, d.cols_cap, scalar(ctx, SC_NIDX));
         if (s != PSL_OK) return s;
-        uint32_t sm_a = tile_smem_bytes(kTile * kRecBytes, d.B_lo, ctx->cfg.n_ebins + 1, true, false);
         {
             Prof prof(ctx, PSL_K_INDEX_A);
-            k_scatter_idx_a<<<nt, kThreads, sm_a, ctx->stream>>>(tiles, ctx->grid, none, d.B_lo, d.lo_bits, table_a, d.tiles_cap, aos, hi16);
-            LAUNCHED();
+            for (const psl_ctx::ChunkLaunch& cl : ctx->idx_launches) {  // the same segments the counts were taken on
+                k_scatter_idx_a<<<cl.n_seg, kThreads, ctx->sm_idx_a, ctx->stream>>>(chunks, ctx->n_chunks, cl.span, ctx->grid, none,
+                                                                                  d.B_lo, d.lo_bits, table_a, d.cols_cap, aos, hi16);
+                LAUNCHED();
+            }
         }
+        // pass B runs over the n_idx <= n_records keyed records; the device knows n_idx, the host only the bound
         uint32_t ntb = (uint32_t)((ctx->n_records + kTile - 1) / kTile);
+        const uint32_t Sb = ntb < ctx->S_b ? ntb : ctx->S_b;
         {
             Prof prof(ctx, PSL_K_COUNT);
-            k_count_hi16<<<ntb, kThreads, d.B_hi * 4, ctx->stream>>>(hi16, scalar(ctx, SC_NIDX), d.B_hi, table_b, d.tiles_b_cap);
+            k_count_hi16<<<Sb, kThreads, ctx->sm_count_b, ctx->stream>>>(hi16, scalar(ctx, SC_NIDX), d.B_hi, table_b, kMaxSegments);
             LAUNCHED();
         }
-        s = run_scan(ctx, table_b, d.B_hi, ntb, d.tiles_b_cap, scalar(ctx, SC_TOTAL));
+        s = run_scan(ctx, table_b, d.B_hi, Sb, kMaxSegments, scalar(ctx, SC_TOTAL));
         if (s != PSL_OK) return s;
-        uint32_t sm_b = tile_smem_bytes(kTile * 32, d.B_hi, 0, true, true);
         {
             Prof prof(ctx, PSL_K_INDEX_B);
-            k_scatter_idx_b<<<ntb, kThreads, sm_b, ctx->stream>>>(aos, hi16, scalar(ctx, SC_NIDX), d.B_hi, table_b, d.tiles_b_cap, idx_out(ctx));
+            k_scatter_idx_b<<<Sb, kThreads, ctx->sm_idx_b, ctx->stream>>>(aos, scalar(ctx, SC_NIDX), d.B_hi, d.lo_bits, table_b,
+                                                                         kMaxSegments, idx_out(ctx));
             LAUNCHED();
         }
         k_offsets_by_search<<<(d.K + 1 + 255) / 256, 256, 0, ctx->stream>>>(at<uint32_t>(ctx, L.keyfull), scalar(ctx, SC_NIDX), d.K, idx_offsets);
         LAUNCHED();
         k_counts_from_offsets<<<(d.K + 1 + 255) / 256, 256, 0, ctx->stream>>>(idx_offsets, d.K, idx_counts, d.n_pos, d.n_batches, idx_batch);
         LAUNCHED();
-        k_reduce_stats<<<1, 1024, 0, ctx->stream>>>(at<TileStats>(ctx, L.tstats), nt, stats);
+        k_reduce_stats<<<1, 1024, 0, ctx->stream>>>(at<SegStats>(ctx, L.sstats), ctx->n_cols, stats);
         LAUNCHED();
     }
     CU(cudaMemcpyAsync(ctx->h_idx_offsets, idx_offsets, (uint64_t)(d.K + 1) * 4, cudaMemcpyDeviceToHost, ctx->stream));
@@ -585,7 +600,7 @@ psl_status build_beam_from_index(psl_ctx* ctx, const psl_beam* beam, const DevBe
     uint32_t* batch_off = at<uint32_t>(ctx, L.batch_off);
     uint32_t* beam_keys = at<uint32_t>(ctx, L.beam_keys);
     DevBeamStats* bstat = at<DevBeamStats>(ctx, L.beam_stats);
-    const uint32_t nt = (uint32_t)((M + kTile - 1) / kTile);
+    const uint32_t nt = (uint32_t)((M + kBeamTile - 1) / kBeamTile);
     CU(cudaMemsetAsync(scalar(ctx, SC_TILE_COUNTER), 0, 8, ctx->stream));  // tile counter + survivor count
     if (nt == 0) {
         CU(cudaMemsetAsync(bstat, 0, sizeof(DevBeamStats), ctx->stream));
@@ -606,7 +621,7 @@ psl_status build_beam_from_index(psl_ctx* ctx, const psl_beam* beam, const DevBe
         in.src = at<uint32_t>(ctx, L.idx[6]);
         {
             Prof prof(ctx, PSL_K_BEAM);
-            k_beam_compact<<<nt, kThreads, 11 * kTile * 4, ctx->stream>>>(st, in, ctx->grid, bm, soa_out(ctx, L.beam_out), beam_keys,
+            k_beam_compact<<<nt, kThreads, 11 * kBeamTile * 4, ctx->stream>>>(st, in, ctx->grid, bm, soa_out(ctx, L.beam_out), beam_keys,
                                                                          at<unsigned long long>(ctx, L.lookback),
                                                                          scalar(ctx, SC_TILE_COUNTER), at<BeamTileStats>(ctx, L.bstats),
                                                                          scalar(ctx, SC_BEAM_NSURV));
@@ -755,17 +770,36 @@ psl_status psl_create(const psl_config* cfg, psl_ctx** out)
         CUC(cudaMemcpyAsync(dev_edges, ctx->edges.data(), (uint64_t)(cfg->n_ebins + 1) * 4, cudaMemcpyHostToDevice, ctx->stream));
     ctx->grid = make_grid(ctx->cfg, d, dev_edges);
 
-    // dynamic shared memory opt-in for the tile kernels
+    // dynamic shared memory opt-in, and the launch width: SMs x resident CTAs of the scatter kernel (one wave)
     const uint32_t ne = cfg->n_ebins + 1;
+    int sms = 0;
+    CUC(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, cfg->device));
+    auto width = [&](int occ) {
+        uint32_t s = (uint32_t)sms * (uint32_t)(occ > 0 ? occ : 1);
+        return s > (uint32_t)kMaxSegments ? (uint32_t)kMaxSegments : s;
+    };
+    int occ = 0;
     if (cfg->mode == PSL_MODE_ONTHEFLY) {
-        CUC(allow_smem(k_count_raw<false>, tile_smem_bytes(kTile * kRecBytes, d.K, ne, false, false)));
-        CUC(allow_smem(k_scatter_otf, tile_smem_bytes(kTile * kRecBytes, d.K, ne, true, true)));
+        ctx->sm_count_raw = count_layout(kTile * kRecBytes, kStagesCount, d.K, ne).total;
+        ctx->sm_scatter_otf = part_layout(kTile * kRecBytes, kStagesRaw, d.K, ne, true).total;
+        CUC(allow_smem(k_count_raw<false>, ctx->sm_count_raw));
+        CUC(allow_smem(k_scatter_otf, ctx->sm_scatter_otf));
+        CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_scatter_otf, kThreads, ctx->sm_scatter_otf));
+        ctx->S_otf = width(occ);
     } else {
-        CUC(allow_smem(k_count_raw<true>, tile_smem_bytes(kTile * kRecBytes, d.B_lo, ne, false, false)));
-        CUC(allow_smem(k_scatter_idx_a, tile_smem_bytes(kTile * kRecBytes, d.B_lo, ne, true, false)));
-        CUC(allow_smem(k_count_hi16, d.B_hi * 4));
-        CUC(allow_smem(k_scatter_idx_b, tile_smem_bytes(kTile * 32, d.B_hi, 0, true, true)));
-        CUC(allow_smem(k_beam_compact, 11 * kTile * 4));
+        ctx->sm_count_raw = count_layout(kTile * kRecBytes, kStagesCount, d.B_lo, ne).total;
+        ctx->sm_idx_a = part_layout(kTile * kRecBytes, kStagesRaw, d.B_lo, ne, false).total;
+        ctx->sm_count_b = count_layout(0, 0, d.B_hi, 0).total;
+        ctx->sm_idx_b = part_layout(kTile * 32, kStagesKeyed, d.B_hi, 0, true).total;
+        CUC(allow_smem(k_count_raw<true>, ctx->sm_count_raw));
+        CUC(allow_smem(k_scatter_idx_a, ctx->sm_idx_a));
+        CUC(allow_smem(k_count_hi16, ctx->sm_count_b));
+        CUC(allow_smem(k_scatter_idx_b, ctx->sm_idx_b));
+        CUC(allow_smem(k_beam_compact, 11 * kBeamTile * 4));
+        CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_scatter_idx_a, kThreads, ctx->sm_idx_a));
+        ctx->S_a = width(occ);
+        CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_scatter_idx_b, kThreads, ctx->sm_idx_b));
+        ctx->S_b = width(occ);
     }
     CUC(cudaStreamSynchronize(ctx->stream));
 #undef CUC
@@ -781,7 +815,8 @@ psl_status psl_reset(psl_ctx* ctx)
     CU(cudaEventRecord(ctx->ev_main, ctx->stream));
     CU(cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_main, 0));
     ctx->n_records = ctx->n_host_records = 0;
-    ctx->n_tiles = ctx->n_chunks = 0;
+    ctx->n_tiles = ctx->n_chunks = ctx->n_cols = 0;
+    ctx->idx_launches.clear();
     ctx->ragged = false;
     ctx->indexed = false;
     ctx->result = RES_NONE;
@@ -841,19 +876,31 @@ psl_status psl_load_chunk(psl_ctx* ctx, const void* records, uint64_t n, int32_t
 
     const uint32_t nt = (uint32_t)((n + kTile - 1) / kTile);
     const uint32_t tile0 = ctx->n_tiles;
-    TileDesc* tiles = at<TileDesc>(ctx, ctx->L.tiles);
-    k_fill_tiles<<<(nt + 255) / 256, 256, 0, ctx->stream>>>(tiles, tile0, nt, dev_ptr, (uint32_t)ctx->n_records, (uint32_t)n);
+    ChunkDesc cd;
+    cd.ptr = dev_ptr;
+    cd.first_index = (uint32_t)ctx->n_records;
+    cd.n_records = (uint32_t)n;
+    cd.tile0 = tile0;
+    cd.pad = 0;
+    ChunkDesc* chunks = at<ChunkDesc>(ctx, ctx->L.chunks);
+    k_set_chunk<<<1, 1, 0, ctx->stream>>>(chunks + ctx->n_chunks, cd);  // the descriptor travels as a kernel argument
     LAUNCHED();
     if (ctx->cfg.mode == PSL_MODE_INDEX) {
         // a8 for pass A, chunk by chunk: overlaps the transfer of the next chunk
         DevBeam none;
         memset(&none, 0, sizeof none);
-        uint32_t sm = tile_smem_bytes(kTile * kRecBytes, ctx->d.B_lo, ctx->cfg.n_ebins + 1, false, false);
+        psl_ctx::ChunkLaunch cl;
+        cl.span = {tile0, nt, ctx->n_cols};
+        cl.n_seg = nt < ctx->S_a ? nt : ctx->S_a;
+        if (ctx->n_cols + cl.n_seg > ctx->d.cols_cap) { set_err(ctx->err, "load_chunk: out of table columns"); return PSL_ERR_CAPACITY; }
         Prof prof(ctx, PSL_K_COUNT);
-        k_count_raw<true><<<nt, kThreads, sm, ctx->stream>>>(tiles, tile0, ctx->grid, none, ctx->d.B_lo, (1u << ctx->d.lo_bits) - 1u,
-                                                            at<uint32_t>(ctx, ctx->L.table_a), ctx->d.tiles_cap,
-                                                            at<TileStats>(ctx, ctx->L.tstats));
+        k_count_raw<true><<<cl.n_seg, kThreads, ctx->sm_count_raw, ctx->stream>>>(chunks, ctx->n_chunks + 1, cl.span, ctx->grid, none,
+                                                                                ctx->d.B_lo, (1u << ctx->d.lo_bits) - 1u,
+                                                                                at<uint32_t>(ctx, ctx->L.table_a), ctx->d.cols_cap,
+                                                                                at<SegStats>(ctx, ctx->L.sstats));
         LAUNCHED();
+        ctx->idx_launches.push_back(cl);
+        ctx->n_cols += cl.n_seg;
     }
     ctx->n_records += n;
     if (host) ctx->n_host_records += n;

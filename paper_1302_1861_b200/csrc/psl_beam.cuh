@@ -53,6 +53,8 @@ __device__ __forceinline__ uint32_t seg_of(const uint32_t* __restrict__ vstart, 
     return lo;
 }
 
+constexpr int kBeamTile = 2048;                       // index records one CTA of the beam kernel compacts
+constexpr int kBeamRounds = kBeamTile / kThreads;      // 8
 constexpr int kBeamArrays = 12;  // E x y u v w wt xp yp src key + spare
 
 __global__ void __launch_bounds__(kThreads) k_beam_compact(SegTable seg, IdxIn in, const __grid_constant__ DevGrid g,
@@ -64,7 +66,7 @@ __global__ void __launch_bounds__(kThreads) k_beam_compact(SegTable seg, IdxIn i
                                                           uint32_t* __restrict__ n_surv_out)
 {
     extern __shared__ __align__(128) uint8_t smem[];
-    uint32_t* stage = reinterpret_cast<uint32_t*>(smem);  // [11][kTile]
+    uint32_t* stage = reinterpret_cast<uint32_t*>(smem);  // [11][kBeamTile]
     __shared__ uint32_t s_wc[2][kWarps];
     __shared__ uint32_t s_ctl[4];  // tile, seg_first, seg_last, exclusive prefix
     __shared__ double s_d[kWarps];
@@ -74,8 +76,8 @@ __global__ void __launch_bounds__(kThreads) k_beam_compact(SegTable seg, IdxIn i
     if (threadIdx.x == 0) s_ctl[0] = atomicAdd(tile_counter, 1u);  // tiles are handed out in order
     __syncthreads();
     const uint32_t tile = s_ctl[0];
-    const uint32_t v0 = tile * kTile;
-    const uint32_t cnt = min((uint32_t)kTile, seg.M - v0);
+    const uint32_t v0 = tile * kBeamTile;
+    const uint32_t cnt = min((uint32_t)kBeamTile, seg.M - v0);
     if (threadIdx.x == 0) s_ctl[1] = seg_of(seg.vstart, 0, seg.n_seg - 1, v0);
     if (threadIdx.x == 32) s_ctl[2] = seg_of(seg.vstart, 0, seg.n_seg - 1, v0 + cnt - 1);
     __syncthreads();
@@ -84,7 +86,7 @@ __global__ void __launch_bounds__(kThreads) k_beam_compact(SegTable seg, IdxIn i
     uint32_t run = 0, n_zero = 0;
     double sum_out = 0.0;
 #pragma unroll 1
-    for (int r = 0; r < kRounds; ++r) {
+    for (int r = 0; r < kBeamRounds; ++r) {
         uint32_t lv = r * kThreads + threadIdx.x;
         bool keep = false;
         float E = 0, x = 0, y = 0, u = 0, v = 0, wz = 0, wt = 0, xm = 0, ym = 0;
@@ -122,17 +124,17 @@ __global__ void __launch_bounds__(kThreads) k_beam_compact(SegTable seg, IdxIn i
         }
         if (keep) {
             uint32_t pos = run + pre + __popc(ballot & lanemask_lt());
-            stage[0 * kTile + pos] = __float_as_uint(E);
-            stage[1 * kTile + pos] = __float_as_uint(x);
-            stage[2 * kTile + pos] = __float_as_uint(y);
-            stage[3 * kTile + pos] = __float_as_uint(u);
-            stage[4 * kTile + pos] = __float_as_uint(v);
-            stage[5 * kTile + pos] = __float_as_uint(wz);
-            stage[6 * kTile + pos] = __float_as_uint(wt);
-            stage[7 * kTile + pos] = __float_as_uint(xm);
-            stage[8 * kTile + pos] = __float_as_uint(ym);
-            stage[9 * kTile + pos] = srci;
-            stage[10 * kTile + pos] = key;
+            stage[0 * kBeamTile + pos] = __float_as_uint(E);
+            stage[1 * kBeamTile + pos] = __float_as_uint(x);
+            stage[2 * kBeamTile + pos] = __float_as_uint(y);
+            stage[3 * kBeamTile + pos] = __float_as_uint(u);
+            stage[4 * kBeamTile + pos] = __float_as_uint(v);
+            stage[5 * kBeamTile + pos] = __float_as_uint(wz);
+            stage[6 * kBeamTile + pos] = __float_as_uint(wt);
+            stage[7 * kBeamTile + pos] = __float_as_uint(xm);
+            stage[8 * kBeamTile + pos] = __float_as_uint(ym);
+            stage[9 * kBeamTile + pos] = srci;
+            stage[10 * kBeamTile + pos] = key;
             sum_out += (double)wt;
         }
         run += tot;
@@ -183,19 +185,19 @@ __global__ void __launch_bounds__(kThreads) k_beam_compact(SegTable seg, IdxIn i
     // coalesced copy-out of the tile's survivors
     for (uint32_t j = threadIdx.x; j < total; j += kThreads) {
         size_t d = (size_t)gbase + j;
-        out.E[d] = __uint_as_float(stage[0 * kTile + j]);
-        out.x[d] = __uint_as_float(stage[1 * kTile + j]);
-        out.y[d] = __uint_as_float(stage[2 * kTile + j]);
-        out.u[d] = __uint_as_float(stage[3 * kTile + j]);
-        out.v[d] = __uint_as_float(stage[4 * kTile + j]);
-        out.w[d] = __uint_as_float(stage[5 * kTile + j]);
-        out.wt[d] = __uint_as_float(stage[6 * kTile + j]);
+        out.E[d] = __uint_as_float(stage[0 * kBeamTile + j]);
+        out.x[d] = __uint_as_float(stage[1 * kBeamTile + j]);
+        out.y[d] = __uint_as_float(stage[2 * kBeamTile + j]);
+        out.u[d] = __uint_as_float(stage[3 * kBeamTile + j]);
+        out.v[d] = __uint_as_float(stage[4 * kBeamTile + j]);
+        out.w[d] = __uint_as_float(stage[5 * kBeamTile + j]);
+        out.wt[d] = __uint_as_float(stage[6 * kBeamTile + j]);
         if (bm.out_proj) {
-            out.xp[d] = __uint_as_float(stage[7 * kTile + j]);
-            out.yp[d] = __uint_as_float(stage[8 * kTile + j]);
+            out.xp[d] = __uint_as_float(stage[7 * kBeamTile + j]);
+            out.yp[d] = __uint_as_float(stage[8 * kBeamTile + j]);
         }
-        out.src[d] = stage[9 * kTile + j];
-        out_key[d] = stage[10 * kTile + j];
+        out.src[d] = stage[9 * kBeamTile + j];
+        out_key[d] = stage[10 * kBeamTile + j];
     }
     if (threadIdx.x == 0) {
         BeamTileStats bs = {0, total, 0.0};

@@ -12,11 +12,12 @@
 
 namespace psl {
 
-constexpr int kTile = 2048;              // records per tile (= table granularity of every partition pass)
+constexpr int kTile = 1024;              // records per tile: the unit one CTA stages, ranks and writes at a time
 constexpr int kThreads = 256;            // threads per CTA in the tile kernels
 constexpr int kWarps = kThreads / 32;    // 8
-constexpr int kRounds = kTile / kThreads;  // 8 records per thread
-constexpr int kWarpSpan = kTile / kWarps;  // 256 consecutive records owned by one warp
+constexpr int kRounds = kTile / kThreads;  // 4 records per thread
+constexpr int kWarpSpan = kTile / kWarps;  // 128 consecutive records owned by one warp
+constexpr int kMaxSegments = 592;        // most CTAs (= table columns) one partition launch uses: 148 SMs x 4
 constexpr int kRecWords = 7;             // 28-byte packed record
 constexpr int kRecBytes = 28;
 constexpr int kMaxBuckets = 2048;        // most buckets one partition pass handles
@@ -47,13 +48,21 @@ struct DevBeam {
     uint32_t out_proj;
 };
 
+struct ChunkDesc {  // 24 bytes, one per psl_load_chunk; tiles never straddle chunks
+    const uint8_t* ptr;    // DEVICE, first record of the chunk
+    uint32_t first_index;  // load-order index of that record
+    uint32_t n_records;
+    uint32_t tile0;        // global id of the chunk's first tile
+    uint32_t pad;
+};
+
 struct TileDesc {  // 16 bytes
     const void* ptr;       // first record of the tile
     uint32_t first_index;  // load-order index of that record
     uint32_t count;        // 1..kTile
 };
 
-struct TileStats {  // 48 bytes, one per tile, reduced in a fixed order (deterministic doubles)
+struct SegStats {  // 48 bytes, one per table column (= one CTA's segment), reduced in a fixed order
     uint32_t n_invalid, n_outside, n_jaw, n_zero, n_surv, pad;
     double sum_in, sum_idx, sum_out;
 };

@@ -1,12 +1,16 @@
 // psl_partition.cuh -- the stable partition passes (histogram -> exclusive scan -> stable scatter).
 //
-// One pass splits a stream of records into B <= kMaxBuckets buckets, keeping input order inside a bucket:
-//   count   : each CTA histograms one tile of kTile records into table[bucket][tile]          (a8)
-//   scan    : ONE exclusive scan over the table read bucket-major, tile-minor                  (a9)
-//             => table[b][t] = (slots of all buckets < b) + (slots of bucket b in tiles < t)
-//   scatter : each CTA re-derives the buckets of its tile, ranks every record among the records of the
-//             same bucket that precede it in the tile (per-warp private counters + __match_any_sync, then
-//             a scan over the 8 warps), and writes it to table[b][tile] + rank                  (a10)
+// One pass splits a stream of records into B <= kMaxBuckets buckets, keeping input order inside a bucket.
+// The stream is cut into S <= kMaxSegments contiguous SEGMENTS of whole tiles, one per persistent CTA
+// (S = SMs x resident CTAs, so the grid is exactly one wave):
+//   count   : CTA s streams its segment through a ring of TMA-filled shared-memory stages and histograms it
+//             into a privatised shared-memory table; table[bucket][s] is written once at the end       (a8)
+//   scan    : ONE exclusive scan over the table read bucket-major, segment-minor                      (a9)
+//             => table[b][s] = (slots of all buckets < b) + (slots of bucket b in segments < s)
+//   scatter : CTA s walks the same segment tile by tile with the same ring, keeping the running first free
+//             slot of every bucket in registers.  Inside a tile every record is ranked among the records of
+//             its bucket that precede it (per-warp private counters + __match_any_sync, then a scan over the
+//             8 warps), staged in tile-sorted order in shared memory and written out in runs            (a10)
 // Ranks come from ordered prefix sums only -- atomics are used for counting, never for claiming slots -- so
 // the output is the unique stable order, bit-identical from run to run.
 //
@@ -24,6 +28,11 @@ constexpr int kScanThreads = 256;
 constexpr int kScanRows = 16;
 constexpr int kScanBlock = kScanThreads * kScanRows;  // 4096 table entries per scan CTA
 
+constexpr int kStagesCount = 4;   // ring depth of the histogram kernels (28 KB stages)
+constexpr int kStagesRaw = 3;     // ring depth of the scatter kernels that read raw records
+constexpr int kStagesKeyed = 2;   // ring depth of INDEX pass B (32 KB stages)
+constexpr int kHistBytes = 32768; // privatised histogram budget of the histogram kernels
+
 struct SoAOut {
     float *E, *x, *y, *u, *v, *w, *wt, *xp, *yp;
     uint32_t* src;
@@ -35,58 +44,60 @@ struct IdxOut {
     uint32_t* key;
 };
 
-// ---- shared-memory carve-up of the tile kernels (dynamic shared memory) --------------------------------
-struct TileSmem {
-    uint32_t* raw;     // staged input tile
-    uint16_t* cnt;     // [kWarps][Bp] per-warp running counts -> exclusive over warps
-    uint32_t* lstart;  // [B] first local (tile-sorted) slot of each bucket
-    uint32_t* gbase;   // [B] first global slot of each bucket for this tile
-    uint16_t* perm;    // [kTile] tile-sorted slot -> record in tile
-    uint16_t* pbkt;    // [kTile] tile-sorted slot -> bucket
-    float* edges;      // [n_ebins+1]
-    uint32_t* misc;    // 64 words: scan scratch
-    uint64_t* bar;     // mbarrier
+// which tiles a launch covers and which table columns its CTAs own: CTA s of the launch (gridDim.x CTAs)
+// takes tiles tile_begin + [s*n_tiles/S, (s+1)*n_tiles/S) and column col0 + s.
+struct Span {
+    uint32_t tile_begin, n_tiles, col0;
 };
 
 __host__ __device__ inline uint32_t round_up(uint32_t a, uint32_t m) { return (a + m - 1) / m * m; }
 
-__host__ __device__ inline uint32_t tile_smem_bytes(uint32_t in_bytes, uint32_t B, uint32_t n_edges, bool ranks,
-                                                    bool reorder)
+// ---- shared-memory carve-up of the scatter kernels (dynamic shared memory, offsets in bytes) ---------
+struct PartSmem {
+    uint32_t ring, stage_bytes, cnt, gcur, lstart, perm, pdest, edges, misc, desc, bars, total;
+};
+
+__host__ __device__ inline PartSmem part_layout(uint32_t tile_bytes, uint32_t stages, uint32_t B, uint32_t n_edges,
+                                                bool staged)
 {
-    uint32_t s = round_up(in_bytes, 128);
-    if (ranks) s += round_up(kWarps * round_up(B, 8) * 2, 16);
-    else s += round_up(B * 4, 16);  // plain histogram
-    if (ranks) s += 2 * round_up(B * 4, 16);
-    if (reorder) s += 2 * kTile * 2;
-    s += round_up(n_edges * 4, 16);
-    s += 64 * 4 + 16;
-    return s;
+    PartSmem L;
+    uint32_t p = 0;
+    L.stage_bytes = round_up(tile_bytes, 128);
+    L.ring = p;   p += stages * L.stage_bytes;
+    L.cnt = p;    p += round_up(kWarps * round_up(B, 8) * 2, 16);  // [kWarps][Bp] uint16
+    L.gcur = p;   p += round_up(B * 4, 16);                        // first global slot of each bucket, this tile
+    L.lstart = p; if (staged) p += round_up(B * 4, 16);            // first tile-sorted slot of each bucket
+    L.pdest = p;  if (staged) p += kTile * 4;                      // tile-sorted slot -> global slot
+    L.perm = p;   if (staged) p += kTile * 2;                      // tile-sorted slot -> record in tile
+    L.edges = p;  p += round_up(n_edges * 4, 16);
+    L.misc = p;   p += 64 * 4;                                     // scan scratch
+    L.desc = p;   p += stages * 16;                                // TileDesc per stage
+    L.bars = p;   p += stages * 8;                                 // "full" mbarrier per stage
+    L.total = p;
+    return L;
 }
 
-__device__ __forceinline__ TileSmem carve(uint8_t* base, uint32_t in_bytes, uint32_t B, uint32_t n_edges, bool ranks,
-                                          bool reorder)
+// ---- histogram kernels --------------------------------------------------------------------------------
+struct CountSmem {
+    uint32_t ring, stage_bytes, hist, edges, desc, bars, total, rlog;
+};
+
+// R = 2^rlog interleaved copies of the histogram (copy = lane mod R) keep the lanes of a warp on
+// different words; R is the largest power of two <= 32 with B * R * 4 <= kHistBytes.
+__host__ __device__ inline CountSmem count_layout(uint32_t tile_bytes, uint32_t stages, uint32_t B, uint32_t n_edges)
 {
-    TileSmem t;
-    uint8_t* p = base;
-    t.raw = reinterpret_cast<uint32_t*>(p);
-    p += round_up(in_bytes, 128);
-    t.cnt = reinterpret_cast<uint16_t*>(p);
-    if (ranks) p += round_up(kWarps * round_up(B, 8) * 2, 16);
-    else p += round_up(B * 4, 16);
-    t.lstart = reinterpret_cast<uint32_t*>(p);
-    if (ranks) p += round_up(B * 4, 16);
-    t.gbase = reinterpret_cast<uint32_t*>(p);
-    if (ranks) p += round_up(B * 4, 16);
-    t.perm = reinterpret_cast<uint16_t*>(p);
-    if (reorder) p += kTile * 2;
-    t.pbkt = reinterpret_cast<uint16_t*>(p);
-    if (reorder) p += kTile * 2;
-    t.edges = reinterpret_cast<float*>(p);
-    p += round_up(n_edges * 4, 16);
-    t.misc = reinterpret_cast<uint32_t*>(p);
-    p += 64 * 4;
-    t.bar = reinterpret_cast<uint64_t*>(p);
-    return t;
+    CountSmem L;
+    uint32_t p = 0;
+    L.rlog = 5;
+    while (L.rlog > 0 && (B << L.rlog) * 4u > (uint32_t)kHistBytes) --L.rlog;
+    L.stage_bytes = round_up(tile_bytes, 128);
+    L.ring = p;  p += stages * L.stage_bytes;
+    L.hist = p;  p += round_up((B << L.rlog) * 4, 16);
+    L.edges = p; p += round_up(n_edges * 4, 16);
+    L.desc = p;  p += stages * 16;
+    L.bars = p;  p += stages * 8;
+    L.total = p;
+    return L;
 }
 
 __device__ __forceinline__ void stage_edges(const DevGrid& g, float* s_edges)
@@ -95,142 +106,245 @@ __device__ __forceinline__ void stage_edges(const DevGrid& g, float* s_edges)
         for (int i = threadIdx.x; i <= g.n_ebins; i += blockDim.x) s_edges[i] = g.e_edges[i];
 }
 
-// After every warp has ranked its slice: turn cnt[w][b] into the exclusive prefix over warps, lstart[b]
-// into the exclusive prefix over buckets of the tile totals, and fetch gbase[b] = table[b][tile].
-// Returns the number of records of the tile that take part.  Contains __syncthreads.
-__device__ __forceinline__ uint32_t finish_ranks(const TileSmem& s, uint32_t B, uint32_t Bp, const uint32_t* table,
-                                                 uint32_t stride, uint32_t tile)
+// one entry of the chunk table (psl_load_chunk)
+__global__ void k_set_chunk(ChunkDesc* __restrict__ dst, ChunkDesc d) { *dst = d; }
+
+// tile id -> descriptor.  Raw records: binary search over the chunk table (tiles never straddle chunks).
+__device__ __forceinline__ TileDesc raw_tile(const ChunkDesc* __restrict__ chunks, uint32_t n_chunks, uint32_t t)
 {
-    __syncthreads();
-    const uint32_t ipt = (B + kThreads - 1) / kThreads;  // <= 8 buckets per thread, blocked
-    const uint32_t b0 = threadIdx.x * ipt;
-    uint32_t tot[kMaxBuckets / kThreads];
-    uint32_t mine = 0;
-#pragma unroll
-    for (uint32_t k = 0; k < kMaxBuckets / kThreads; ++k) {
-        tot[k] = 0;
-        uint32_t b = b0 + k;
-        if (k < ipt && b < B) {
-            uint32_t run = 0;
-#pragma unroll
-            for (int w = 0; w < kWarps; ++w) {
-                uint32_t c = s.cnt[w * Bp + b];
-                s.cnt[w * Bp + b] = (uint16_t)run;
-                run += c;
-            }
-            tot[k] = run;
-            mine += run;
-        }
+    uint32_t lo = 0, hi = n_chunks - 1;
+    while (lo < hi) {
+        uint32_t mid = (lo + hi + 1) >> 1;
+        if (__ldg(&chunks[mid].tile0) <= t) lo = mid; else hi = mid - 1;
     }
-    uint32_t total;
-    uint32_t ex = block_excl_scan(mine, s.misc, &total);
+    const ChunkDesc c = chunks[lo];
+    const uint32_t local = (t - c.tile0) * (uint32_t)kTile;
+    TileDesc d;
+    d.ptr = c.ptr + (size_t)local * kRecBytes;
+    d.first_index = c.first_index + local;
+    d.count = min((uint32_t)kTile, c.n_records - local);
+    return d;
+}
+
+// the segment of CTA s: tiles [t0, t1)
+__device__ __forceinline__ void segment_of(const Span& sp, uint32_t& t0, uint32_t& t1)
+{
+    const unsigned long long n = sp.n_tiles, S = gridDim.x, s = blockIdx.x;
+    t0 = sp.tile_begin + (uint32_t)(n * s / S);
+    t1 = sp.tile_begin + (uint32_t)(n * (s + 1) / S);
+}
+
+// ---- the ring: stage = i % STAGES, one "full" mbarrier per stage, refilled by thread 0 ------------------
+__device__ __forceinline__ bool bulk_ok(const void* src, uint32_t bytes)
+{
+    return ((reinterpret_cast<uintptr_t>(src) & 15u) == 0) && ((bytes & 15u) == 0) && bytes > 0;
+}
+
+// thread 0: start the copy of one tile into a free stage (tiles that cannot be bulk-copied -- a source that
+// is not 16-byte aligned, or the ragged last tile -- are fetched by all threads in ring_acquire instead)
+__device__ __forceinline__ void ring_issue(uint32_t* s_dst, uint64_t* bar, const void* src, uint32_t bytes)
+{
+    if (bulk_ok(src, bytes)) {
+        mbar_expect_tx(bar, bytes);
+        tma_load_1d(s_dst, src, bytes, bar);
+    }
+}
+
+// all threads: wait until the stage holds its tile.  `phase` is this thread's parity bit for the stage.
+__device__ __forceinline__ void ring_acquire(uint32_t* s_dst, uint64_t* bar, uint32_t& phase_bits, uint32_t stage,
+                                             const void* src, uint32_t bytes)
+{
+    if (bulk_ok(src, bytes)) {
+        mbar_wait(bar, (phase_bits >> stage) & 1u);
+        phase_bits ^= 1u << stage;
+    } else {
+        const uint32_t* g = reinterpret_cast<const uint32_t*>(src);
+        for (uint32_t i = threadIdx.x; i < bytes / 4; i += blockDim.x) s_dst[i] = __ldg(g + i);
+        __syncthreads();
+    }
+}
+
+// After every warp has ranked its slice of the tile: thread t owns buckets 8t..8t+7 (one 16-byte row piece
+// per warp).  Turns cnt[w][b] into the exclusive prefix over warps, publishes gcur[b] = first global slot
+// of bucket b for this tile and advances the thread's running slots grun[8].  With STAGED also lstart[b] =
+// exclusive prefix over buckets of the tile totals; returns the number of records that take part.
+// Must be called by all threads after a __syncthreads; ends with a __syncthreads.
+template <bool STAGED>
+__device__ __forceinline__ uint32_t finish_ranks(uint16_t* cnt, uint32_t B, uint32_t Bp, uint32_t* gcur, uint32_t* lstart,
+                                                 uint32_t* misc, uint32_t (&grun)[8])
+{
+    const uint32_t b0 = threadIdx.x * 8;
+    uint32_t t8[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    uint32_t mine = 0;
+    if (b0 < Bp) {
+        uint4 run = make_uint4(0, 0, 0, 0);  // 8 packed uint16 running sums (no carry: a tile has <= 1024 records)
 #pragma unroll
-    for (uint32_t k = 0; k < kMaxBuckets / kThreads; ++k) {
-        uint32_t b = b0 + k;
-        if (k < ipt && b < B) {
-            s.lstart[b] = ex;
-            ex += tot[k];
-            s.gbase[b] = table[(size_t)b * stride + tile];
+        for (int w = 0; w < kWarps; ++w) {
+            uint4* p = reinterpret_cast<uint4*>(cnt + w * Bp + b0);
+            uint4 c = *p;
+            *p = run;
+            run.x += c.x; run.y += c.y; run.z += c.z; run.w += c.w;
+        }
+        t8[0] = run.x & 0xFFFFu; t8[1] = run.x >> 16; t8[2] = run.y & 0xFFFFu; t8[3] = run.y >> 16;
+        t8[4] = run.z & 0xFFFFu; t8[5] = run.z >> 16; t8[6] = run.w & 0xFFFFu; t8[7] = run.w >> 16;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) mine += t8[k];
+    }
+    uint32_t total = 0, ex = 0;
+    if (STAGED) ex = block_excl_scan(mine, misc, &total);
+    if (b0 < Bp) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            if (b0 + k < B) {
+                if (STAGED) lstart[b0 + k] = ex;
+                ex += t8[k];
+                gcur[b0 + k] = grun[k];
+                grun[k] += t8[k];
+            }
         }
     }
     __syncthreads();
     return total;
 }
 
-// ------------------------------------------------------------------------------------------------------
-// count over raw records.  IDX = false: ONTHEFLY, bucket = key of survivors (jaws applied).
-//                          IDX = true : INDEX pass A, bucket = key & lo_mask of valid in-grid records.
-// Also writes the tile's statistics (every record falls in exactly one class).
-// ------------------------------------------------------------------------------------------------------
-template <bool IDX>
-__global__ void __launch_bounds__(kThreads) k_count_raw(const TileDesc* __restrict__ tiles, uint32_t tile0,
-                                                       const __grid_constant__ DevGrid g,
-                                                       const __grid_constant__ DevBeam bm, uint32_t B,
-                                                       uint32_t lo_mask, uint32_t* __restrict__ table,
-                                                       uint32_t stride, TileStats* __restrict__ tstats)
+// a warp clears its own row of the counter matrix (only that warp ever touches it outside finish_ranks)
+__device__ __forceinline__ void zero_row(uint16_t* row, uint32_t Bp)
 {
-    extern __shared__ __align__(128) uint8_t smem[];
-    TileSmem s = carve(smem, kTile * kRecBytes, B, g.n_ebins + 1, false, false);
-    uint32_t* hist = reinterpret_cast<uint32_t*>(s.cnt);
-    const uint32_t tile = tile0 + blockIdx.x;
-    const TileDesc td = tiles[tile];
+    uint4* p = reinterpret_cast<uint4*>(row);
+    for (uint32_t i = lane_id(); i < Bp / 8; i += 32) p[i] = make_uint4(0, 0, 0, 0);
+}
 
-    if (threadIdx.x == 0) {
-        mbar_init(s.bar, 1);
-        mbar_fence_init();
-    }
-    for (uint32_t b = threadIdx.x; b < B; b += kThreads) hist[b] = 0;
-    stage_edges(g, s.edges);
-    __syncthreads();
-    load_tile_bytes(s.raw, td.ptr, td.count * kRecBytes, s.bar, 0);
-
+// ------------------------------------------------------------------------------------------------------
+// per-segment statistics: per-thread running values, reduced once per CTA in a fixed order
+// ------------------------------------------------------------------------------------------------------
+struct ThreadStats {
     uint32_t n_inv = 0, n_out = 0, n_jaw = 0, n_zero = 0, n_surv = 0;
     double sum_in = 0.0, sum_idx = 0.0;
-#pragma unroll 2
-    for (int r = 0; r < kRounds; ++r) {
-        int idx = r * kThreads + threadIdx.x;
-        uint32_t bucket = kNone;
-        if (idx < (int)td.count) {
-            Rec rec = rec_from_smem(s.raw, idx);
-            uint32_t key;
-            int cls = classify_raw(g, bm, rec, s.edges, key);
-            if (cls != C_INVALID) sum_in += (double)rec.wt;
-            if (cls != C_INVALID && cls != C_OUTSIDE) sum_idx += (double)rec.wt;
-            n_inv += cls == C_INVALID;
-            n_out += cls == C_OUTSIDE;
-            n_jaw += cls == C_JAW;
-            n_zero += cls == C_ZERO;
-            n_surv += cls == C_SURVIVOR;
-            if (cls == C_SURVIVOR) bucket = IDX ? (key & lo_mask) : key;
-        }
-        // warp-aggregated shared-memory histogram: one atomic per distinct bucket per warp-round
-        uint32_t active = __ballot_sync(0xFFFFFFFFu, bucket != kNone);
-        if (bucket != kNone) {
-            uint32_t peers = __match_any_sync(active, bucket);
-            if ((int)lane_id() == __ffs(peers) - 1) atomicAdd(&hist[bucket], (uint32_t)__popc(peers));
-        }
-    }
-    __syncthreads();
-    for (uint32_t b = threadIdx.x; b < B; b += kThreads) table[(size_t)b * stride + tile] = hist[b];
+};
 
-    // tile statistics, reduced in a fixed order
-    n_inv = __reduce_add_sync(0xFFFFFFFFu, n_inv);
-    n_out = __reduce_add_sync(0xFFFFFFFFu, n_out);
-    n_jaw = __reduce_add_sync(0xFFFFFFFFu, n_jaw);
-    n_zero = __reduce_add_sync(0xFFFFFFFFu, n_zero);
-    n_surv = __reduce_add_sync(0xFFFFFFFFu, n_surv);
-    sum_in = warp_sum_double(sum_in);
-    sum_idx = warp_sum_double(sum_idx);
+__device__ __forceinline__ void write_seg_stats(ThreadStats t, SegStats* __restrict__ dst)
+{
     __shared__ uint32_t s_n[kWarps][5];
     __shared__ double s_d[kWarps][2];
+    t.n_inv = __reduce_add_sync(0xFFFFFFFFu, t.n_inv);
+    t.n_out = __reduce_add_sync(0xFFFFFFFFu, t.n_out);
+    t.n_jaw = __reduce_add_sync(0xFFFFFFFFu, t.n_jaw);
+    t.n_zero = __reduce_add_sync(0xFFFFFFFFu, t.n_zero);
+    t.n_surv = __reduce_add_sync(0xFFFFFFFFu, t.n_surv);
+    t.sum_in = warp_sum_double(t.sum_in);
+    t.sum_idx = warp_sum_double(t.sum_idx);
     if (lane_id() == 0) {
         uint32_t w = warp_id();
-        s_n[w][0] = n_inv; s_n[w][1] = n_out; s_n[w][2] = n_jaw; s_n[w][3] = n_zero; s_n[w][4] = n_surv;
-        s_d[w][0] = sum_in; s_d[w][1] = sum_idx;
+        s_n[w][0] = t.n_inv; s_n[w][1] = t.n_out; s_n[w][2] = t.n_jaw; s_n[w][3] = t.n_zero; s_n[w][4] = t.n_surv;
+        s_d[w][0] = t.sum_in; s_d[w][1] = t.sum_idx;
     }
     __syncthreads();
     if (threadIdx.x == 0) {
-        TileStats ts = {0, 0, 0, 0, 0, 0, 0.0, 0.0, 0.0};
+        SegStats ts = {0, 0, 0, 0, 0, 0, 0.0, 0.0, 0.0};
         for (int w = 0; w < kWarps; ++w) {
             ts.n_invalid += s_n[w][0]; ts.n_outside += s_n[w][1]; ts.n_jaw += s_n[w][2];
             ts.n_zero += s_n[w][3]; ts.n_surv += s_n[w][4];
             ts.sum_in += s_d[w][0]; ts.sum_idx += s_d[w][1];
         }
-        tstats[tile] = ts;
+        *dst = ts;
     }
 }
 
 // ------------------------------------------------------------------------------------------------------
-// exclusive scan of the table read bucket-major / tile-minor (virtual index v = b * n_tiles + t lives at
-// table[b * stride + t]).  Three small kernels: per-CTA sums, scan of the sums, in-place scan.
+// count over raw records.  IDX = false: ONTHEFLY, bucket = key of survivors (jaws applied).
+//                          IDX = true : INDEX pass A, bucket = key & lo_mask of valid in-grid records.
+// Also writes the segment's statistics (every record falls in exactly one class).
 // ------------------------------------------------------------------------------------------------------
-__device__ __forceinline__ size_t table_phys(uint32_t v, uint32_t n_tiles, uint32_t stride)
+template <bool IDX>
+__global__ void __launch_bounds__(kThreads, 2) k_count_raw(const ChunkDesc* __restrict__ chunks, uint32_t n_chunks,
+                                                          Span sp, const __grid_constant__ DevGrid g,
+                                                          const __grid_constant__ DevBeam bm, uint32_t B,
+                                                          uint32_t lo_mask, uint32_t* __restrict__ table,
+                                                          uint32_t stride, SegStats* __restrict__ sstats)
 {
-    uint32_t b = v / n_tiles;
-    return (size_t)b * stride + (v - b * n_tiles);
+    extern __shared__ __align__(128) uint8_t smem[];
+    const CountSmem L = count_layout(kTile * kRecBytes, kStagesCount, B, g.n_ebins + 1);
+    uint32_t* hist = reinterpret_cast<uint32_t*>(smem + L.hist);
+    float* s_edges = reinterpret_cast<float*>(smem + L.edges);
+    TileDesc* s_desc = reinterpret_cast<TileDesc*>(smem + L.desc);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + L.bars);
+    const uint32_t rmask = (1u << L.rlog) - 1u;
+
+    uint32_t t0, t1;
+    segment_of(sp, t0, t1);
+    const uint32_t n = t1 - t0;
+
+    if (threadIdx.x == 0) {
+        for (int k = 0; k < kStagesCount; ++k) mbar_init(&bars[k], 1);
+        mbar_fence_init();
+        for (uint32_t k = 0; k < (uint32_t)kStagesCount && k < n; ++k) {
+            TileDesc d = raw_tile(chunks, n_chunks, t0 + k);
+            s_desc[k] = d;
+            ring_issue(reinterpret_cast<uint32_t*>(smem + L.ring + k * L.stage_bytes), &bars[k], d.ptr, d.count * kRecBytes);
+        }
+    }
+    for (uint32_t i = threadIdx.x; i < (B << L.rlog); i += kThreads) hist[i] = 0;
+    stage_edges(g, s_edges);
+    __syncthreads();
+
+    ThreadStats st;
+    uint32_t phase_bits = 0;
+    for (uint32_t i = 0; i < n; ++i) {
+        const uint32_t stage = i % kStagesCount;
+        uint32_t* raw = reinterpret_cast<uint32_t*>(smem + L.ring + stage * L.stage_bytes);
+        const TileDesc td = s_desc[stage];
+        ring_acquire(raw, &bars[stage], phase_bits, stage, td.ptr, td.count * kRecBytes);
+#pragma unroll
+        for (int r = 0; r < kRounds; ++r) {
+            const int idx = r * kThreads + threadIdx.x;
+            if (idx < (int)td.count) {
+                Rec rec = rec_from_smem(raw, idx);
+                uint32_t key;
+                int cls = classify_raw(g, bm, rec, s_edges, key);
+                if (cls != C_INVALID) {
+                    double wd = (double)rec.wt;
+                    st.sum_in += wd;
+                    if (cls != C_OUTSIDE) st.sum_idx += wd;
+                }
+                st.n_inv += cls == C_INVALID;
+                st.n_out += cls == C_OUTSIDE;
+                st.n_jaw += cls == C_JAW;
+                st.n_zero += cls == C_ZERO;
+                if (cls == C_SURVIVOR) {
+                    st.n_surv += 1;
+                    uint32_t bucket = IDX ? (key & lo_mask) : key;
+                    atomicAdd(&hist[(bucket << L.rlog) + (lane_id() & rmask)], 1u);
+                }
+            }
+        }
+        __syncthreads();  // every thread is done with the stage
+        if (threadIdx.x == 0 && i + kStagesCount < n) {
+            TileDesc d = raw_tile(chunks, n_chunks, t0 + i + kStagesCount);
+            s_desc[stage] = d;
+            ring_issue(raw, &bars[stage], d.ptr, d.count * kRecBytes);
+        }
+    }
+    __syncthreads();
+    const uint32_t col = sp.col0 + blockIdx.x;
+    for (uint32_t b = threadIdx.x; b < B; b += kThreads) {
+        uint32_t c = 0;
+        for (uint32_t r = 0; r <= rmask; ++r) c += hist[(b << L.rlog) + ((r + lane_id()) & rmask)];
+        table[(size_t)b * stride + col] = c;
+    }
+    write_seg_stats(st, &sstats[col]);
 }
 
-__global__ void __launch_bounds__(kScanThreads) k_scan_reduce(const uint32_t* __restrict__ table, uint32_t n_tiles,
+// ------------------------------------------------------------------------------------------------------
+// exclusive scan of the table read bucket-major / column-minor (virtual index v = b * n_cols + c lives at
+// table[b * stride + c]).  Three small kernels: per-CTA sums, scan of the sums, in-place scan.
+// ------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ size_t table_phys(uint32_t v, uint32_t n_cols, uint32_t stride)
+{
+    uint32_t b = v / n_cols;
+    return (size_t)b * stride + (v - b * n_cols);
+}
+
+__global__ void __launch_bounds__(kScanThreads) k_scan_reduce(const uint32_t* __restrict__ table, uint32_t n_cols,
                                                              uint32_t stride, uint32_t L,
                                                              uint32_t* __restrict__ block_sums)
 {
@@ -240,7 +354,7 @@ __global__ void __launch_bounds__(kScanThreads) k_scan_reduce(const uint32_t* __
 #pragma unroll 4
     for (int r = 0; r < kScanRows; ++r) {
         uint32_t v = base + r * kScanThreads + threadIdx.x;
-        if (v < L) acc += table[table_phys(v, n_tiles, stride)];
+        if (v < L) acc += table[table_phys(v, n_cols, stride)];
     }
     acc = __reduce_add_sync(0xFFFFFFFFu, acc);
     if (lane_id() == 0) s_w[warp_id()] = acc;
@@ -270,7 +384,7 @@ __global__ void __launch_bounds__(1024) k_scan_sums(uint32_t* __restrict__ block
     if (threadIdx.x == 0) *total_out = carry;
 }
 
-__global__ void __launch_bounds__(kScanThreads) k_scan_apply(uint32_t* __restrict__ table, uint32_t n_tiles,
+__global__ void __launch_bounds__(kScanThreads) k_scan_apply(uint32_t* __restrict__ table, uint32_t n_cols,
                                                             uint32_t stride, uint32_t L,
                                                             const uint32_t* __restrict__ block_sums)
 {
@@ -282,7 +396,7 @@ __global__ void __launch_bounds__(kScanThreads) k_scan_apply(uint32_t* __restric
         size_t p = 0;
         uint32_t x = 0;
         if (v < L) {
-            p = table_phys(v, n_tiles, stride);
+            p = table_phys(v, n_cols, stride);
             x = table[p];
         }
         uint32_t tot;
@@ -307,85 +421,138 @@ __global__ void k_offsets_from_table(const uint32_t* __restrict__ table, uint32_
     if (k % n_pos == 0 && k / n_pos <= n_batches) batch_offsets[k / n_pos] = o;
 }
 
+// prologue shared by the scatter kernels: barriers, first STAGES copies, zeroed counters, running slots
+template <int STAGES, typename DescFn>
+__device__ __forceinline__ void scatter_prologue(uint8_t* smem, const PartSmem& L, uint32_t B, uint32_t Bp, uint32_t n,
+                                                 uint32_t t0, uint32_t rec_bytes, DescFn desc_of,
+                                                 const uint32_t* __restrict__ table, uint32_t stride, uint32_t col,
+                                                 uint32_t (&grun)[8])
+{
+    TileDesc* s_desc = reinterpret_cast<TileDesc*>(smem + L.desc);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + L.bars);
+    if (threadIdx.x == 0) {
+        for (int k = 0; k < STAGES; ++k) mbar_init(&bars[k], 1);
+        mbar_fence_init();
+        for (uint32_t k = 0; k < (uint32_t)STAGES && k < n; ++k) {
+            TileDesc d = desc_of(t0 + k);
+            s_desc[k] = d;
+            ring_issue(reinterpret_cast<uint32_t*>(smem + L.ring + k * L.stage_bytes), &bars[k], d.ptr, d.count * rec_bytes);
+        }
+    }
+    uint32_t* cz = reinterpret_cast<uint32_t*>(smem + L.cnt);
+    for (uint32_t i = threadIdx.x; i < kWarps * Bp / 2; i += kThreads) cz[i] = 0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        uint32_t b = threadIdx.x * 8 + k;
+        grun[k] = b < B ? table[(size_t)b * stride + col] : 0u;
+    }
+}
+
 // ------------------------------------------------------------------------------------------------------
 // ONTHEFLY scatter: raw records -> transport-ready SoA (a1-a4, a6, a7, a10 fused).
-// The tile is staged once in shared memory; survivors are ordered inside the tile by (key, input order) so
-// that consecutive threads write consecutive slots of a key (block-local staging before the global scatter).
+// Survivors are ordered inside the tile by (key, input order) so that consecutive threads write consecutive
+// slots of a key (block-local staging before the global scatter).
 // ------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kThreads) k_scatter_otf(const TileDesc* __restrict__ tiles,
-                                                         const __grid_constant__ DevGrid g,
-                                                         const __grid_constant__ DevBeam bm, uint32_t B,
-                                                         const uint32_t* __restrict__ table, uint32_t stride,
-                                                         SoAOut out, TileStats* __restrict__ tstats)
+__global__ void __launch_bounds__(kThreads, 2) k_scatter_otf(const ChunkDesc* __restrict__ chunks, uint32_t n_chunks,
+                                                            Span sp, const __grid_constant__ DevGrid g,
+                                                            const __grid_constant__ DevBeam bm, uint32_t B,
+                                                            const uint32_t* __restrict__ table, uint32_t stride,
+                                                            SoAOut out, SegStats* __restrict__ sstats)
 {
     extern __shared__ __align__(128) uint8_t smem[];
     const uint32_t Bp = round_up(B, 8);
-    TileSmem s = carve(smem, kTile * kRecBytes, B, g.n_ebins + 1, true, true);
-    const uint32_t tile = blockIdx.x;
-    const TileDesc td = tiles[tile];
+    const PartSmem L = part_layout(kTile * kRecBytes, kStagesRaw, B, g.n_ebins + 1, true);
+    uint16_t* cnt = reinterpret_cast<uint16_t*>(smem + L.cnt);
+    uint32_t* gcur = reinterpret_cast<uint32_t*>(smem + L.gcur);
+    uint32_t* lstart = reinterpret_cast<uint32_t*>(smem + L.lstart);
+    uint32_t* pdest = reinterpret_cast<uint32_t*>(smem + L.pdest);
+    uint16_t* perm = reinterpret_cast<uint16_t*>(smem + L.perm);
+    float* s_edges = reinterpret_cast<float*>(smem + L.edges);
+    uint32_t* misc = reinterpret_cast<uint32_t*>(smem + L.misc);
+    TileDesc* s_desc = reinterpret_cast<TileDesc*>(smem + L.desc);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + L.bars);
     const uint32_t w = warp_id();
+    const uint32_t col = sp.col0 + blockIdx.x;
 
-    if (threadIdx.x == 0) {
-        mbar_init(s.bar, 1);
-        mbar_fence_init();
-    }
-    for (uint32_t i = threadIdx.x; i < kWarps * Bp / 2; i += kThreads) reinterpret_cast<uint32_t*>(s.cnt)[i] = 0;
-    stage_edges(g, s.edges);
-    __syncthreads();
-    load_tile_bytes(s.raw, td.ptr, td.count * kRecBytes, s.bar, 0);
-
-    // pass 1 over the tile: bucket and stable rank inside the warp's slice
-    uint32_t packed[kRounds];  // bucket << 9 | rank   (bucket < 2^11... stored in 22 bits, rank < 2^9)
-#pragma unroll
-    for (int r = 0; r < kRounds; ++r) {
-        int idx = w * kWarpSpan + r * 32 + lane_id();
-        uint32_t bucket = kNone;
-        if (idx < (int)td.count) {
-            Rec rec = rec_from_smem(s.raw, idx);
-            uint32_t key;
-            if (classify_raw(g, bm, rec, s.edges, key) == C_SURVIVOR) bucket = key;
-        }
-        uint32_t rank = warp_rank(bucket, s.cnt + w * Bp);
-        packed[r] = bucket == kNone ? kNone : ((bucket << 9) | rank);
-    }
-    uint32_t n_part = finish_ranks(s, B, Bp, table, stride, tile);
-
-    // tile-sorted order
-#pragma unroll
-    for (int r = 0; r < kRounds; ++r) {
-        if (packed[r] != kNone) {
-            uint32_t bucket = packed[r] >> 9, rank = packed[r] & 511u;
-            uint32_t p = s.lstart[bucket] + s.cnt[w * Bp + bucket] + rank;
-            s.perm[p] = (uint16_t)(w * kWarpSpan + r * 32 + lane_id());
-            s.pbkt[p] = (uint16_t)bucket;
-        }
-    }
+    uint32_t t0, t1;
+    segment_of(sp, t0, t1);
+    const uint32_t n = t1 - t0;
+    uint32_t grun[8];
+    auto desc_of = [&](uint32_t t) { return raw_tile(chunks, n_chunks, t); };
+    scatter_prologue<kStagesRaw>(smem, L, B, Bp, n, t0, kRecBytes, desc_of, table, stride, col, grun);
+    stage_edges(g, s_edges);
     __syncthreads();
 
-    // write-out: thread j takes tile-sorted slot j
     double sum_out = 0.0;
-    for (uint32_t j = threadIdx.x; j < n_part; j += kThreads) {
-        uint32_t i = s.perm[j], bucket = s.pbkt[j];
-        uint32_t dest = s.gbase[bucket] + (j - s.lstart[bucket]);
-        Rec rec = rec_from_smem(s.raw, (int)i);
-        float q = q_of(rec.u, rec.v), wz, tx, ty;
-        slopes(rec.u, rec.v, q, wz, tx, ty);
-        float xm = __fadd_rn(rec.x, __fmul_rn(tx, bm.dzM));
-        float ym = __fadd_rn(rec.y, __fmul_rn(ty, bm.dzM));
-        float wt = final_weight(bm, rec.wt, xm, ym);
-        out.E[dest] = rec.E;
-        out.x[dest] = rec.x;
-        out.y[dest] = rec.y;
-        out.u[dest] = rec.u;
-        out.v[dest] = rec.v;
-        out.w[dest] = wz;
-        out.wt[dest] = wt;
-        out.src[dest] = td.first_index + i;
-        if (bm.out_proj) {
-            out.xp[dest] = xm;
-            out.yp[dest] = ym;
+    uint32_t phase_bits = 0;
+    for (uint32_t i = 0; i < n; ++i) {
+        const uint32_t stage = i % kStagesRaw;
+        uint32_t* raw = reinterpret_cast<uint32_t*>(smem + L.ring + stage * L.stage_bytes);
+        const TileDesc td = s_desc[stage];
+        ring_acquire(raw, &bars[stage], phase_bits, stage, td.ptr, td.count * kRecBytes);
+
+        // bucket and stable rank inside the warp's slice of the tile
+        uint32_t packed[kRounds];  // bucket << 9 | rank   (bucket < 2^11, rank < 2^7)
+#pragma unroll
+        for (int r = 0; r < kRounds; ++r) {
+            int idx = w * kWarpSpan + r * 32 + lane_id();
+            uint32_t bucket = kNone;
+            if (idx < (int)td.count) {
+                Rec rec = rec_from_smem(raw, idx);
+                uint32_t key;
+                if (classify_raw(g, bm, rec, s_edges, key) == C_SURVIVOR) bucket = key;
+            }
+            uint32_t rank = warp_rank(bucket, cnt + w * Bp);
+            packed[r] = bucket == kNone ? kNone : ((bucket << 9) | rank);
         }
-        sum_out += (double)wt;
+        __syncthreads();
+        const uint32_t n_part = finish_ranks<true>(cnt, B, Bp, gcur, lstart, misc, grun);
+
+        // tile-sorted order
+#pragma unroll
+        for (int r = 0; r < kRounds; ++r) {
+            if (packed[r] != kNone) {
+                uint32_t bucket = packed[r] >> 9, rank = packed[r] & 511u;
+                uint32_t rel = cnt[w * Bp + bucket] + rank;  // among the tile's records of this bucket
+                uint32_t p = lstart[bucket] + rel;
+                perm[p] = (uint16_t)(w * kWarpSpan + r * 32 + lane_id());
+                pdest[p] = gcur[bucket] + rel;
+            }
+        }
+        __syncwarp();
+        zero_row(cnt + w * Bp, Bp);
+        __syncthreads();
+
+        // write-out: thread j takes tile-sorted slot j
+        for (uint32_t j = threadIdx.x; j < n_part; j += kThreads) {
+            const uint32_t irec = perm[j];
+            const uint32_t dest = pdest[j];
+            Rec rec = rec_from_smem(raw, (int)irec);
+            float q = q_of(rec.u, rec.v), wz, tx, ty;
+            slopes(rec.u, rec.v, q, wz, tx, ty);
+            float xm = __fadd_rn(rec.x, __fmul_rn(tx, bm.dzM));
+            float ym = __fadd_rn(rec.y, __fmul_rn(ty, bm.dzM));
+            float wt = final_weight(bm, rec.wt, xm, ym);
+            out.E[dest] = rec.E;
+            out.x[dest] = rec.x;
+            out.y[dest] = rec.y;
+            out.u[dest] = rec.u;
+            out.v[dest] = rec.v;
+            out.w[dest] = wz;
+            out.wt[dest] = wt;
+            out.src[dest] = td.first_index + irec;
+            if (bm.out_proj) {
+                out.xp[dest] = xm;
+                out.yp[dest] = ym;
+            }
+            sum_out += (double)wt;
+        }
+        __syncthreads();  // the stage and perm/pdest are free again
+        if (threadIdx.x == 0 && i + kStagesRaw < n) {
+            TileDesc d = raw_tile(chunks, n_chunks, t0 + i + kStagesRaw);
+            s_desc[stage] = d;
+            ring_issue(raw, &bars[stage], d.ptr, d.count * kRecBytes);
+        }
     }
     sum_out = warp_sum_double(sum_out);
     __shared__ double s_d[kWarps];
@@ -394,161 +561,221 @@ __global__ void __launch_bounds__(kThreads) k_scatter_otf(const TileDesc* __rest
     if (threadIdx.x == 0) {
         double t = 0.0;
         for (int k = 0; k < kWarps; ++k) t += s_d[k];
-        tstats[tile].sum_out = t;
+        sstats[col].sum_out = t;
     }
 }
 
 // ------------------------------------------------------------------------------------------------------
 // INDEX pass A: raw records -> 32-byte keyed records {key, E, x, y, u, v, wt, src}, stably partitioned by
-// the low digit of the key.  One record = one full 32-byte sector, written by its own thread.
+// the low digit of the key.  One record = one full 32-byte sector, written by its own thread (no staging).
 // Also writes the high digit of every record (uint16) to hi16[] in the new order, which is all pass B's
 // count needs to read.
 // ------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kThreads) k_scatter_idx_a(const TileDesc* __restrict__ tiles,
-                                                           const __grid_constant__ DevGrid g,
-                                                           const __grid_constant__ DevBeam bm, uint32_t B,
-                                                           uint32_t lo_bits, const uint32_t* __restrict__ table,
-                                                           uint32_t stride, uint4* __restrict__ aos,
-                                                           uint16_t* __restrict__ hi16)
+__global__ void __launch_bounds__(kThreads, 2) k_scatter_idx_a(const ChunkDesc* __restrict__ chunks, uint32_t n_chunks,
+                                                              Span sp, const __grid_constant__ DevGrid g,
+                                                              const __grid_constant__ DevBeam bm, uint32_t B,
+                                                              uint32_t lo_bits, const uint32_t* __restrict__ table,
+                                                              uint32_t stride, uint4* __restrict__ aos,
+                                                              uint16_t* __restrict__ hi16)
 {
     extern __shared__ __align__(128) uint8_t smem[];
     const uint32_t Bp = round_up(B, 8);
-    TileSmem s = carve(smem, kTile * kRecBytes, B, g.n_ebins + 1, true, false);
-    const uint32_t tile = blockIdx.x;
-    const TileDesc td = tiles[tile];
+    const PartSmem L = part_layout(kTile * kRecBytes, kStagesRaw, B, g.n_ebins + 1, false);
+    uint16_t* cnt = reinterpret_cast<uint16_t*>(smem + L.cnt);
+    uint32_t* gcur = reinterpret_cast<uint32_t*>(smem + L.gcur);
+    float* s_edges = reinterpret_cast<float*>(smem + L.edges);
+    uint32_t* misc = reinterpret_cast<uint32_t*>(smem + L.misc);
+    TileDesc* s_desc = reinterpret_cast<TileDesc*>(smem + L.desc);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + L.bars);
     const uint32_t w = warp_id();
     const uint32_t lo_mask = (1u << lo_bits) - 1u;
 
-    if (threadIdx.x == 0) {
-        mbar_init(s.bar, 1);
-        mbar_fence_init();
-    }
-    for (uint32_t i = threadIdx.x; i < kWarps * Bp / 2; i += kThreads) reinterpret_cast<uint32_t*>(s.cnt)[i] = 0;
-    stage_edges(g, s.edges);
+    uint32_t t0, t1;
+    segment_of(sp, t0, t1);
+    const uint32_t n = t1 - t0;
+    uint32_t grun[8];
+    auto desc_of = [&](uint32_t t) { return raw_tile(chunks, n_chunks, t); };
+    scatter_prologue<kStagesRaw>(smem, L, B, Bp, n, t0, kRecBytes, desc_of, table, stride, sp.col0 + blockIdx.x, grun);
+    stage_edges(g, s_edges);
     __syncthreads();
-    load_tile_bytes(s.raw, td.ptr, td.count * kRecBytes, s.bar, 0);
 
-    uint32_t packed[kRounds];  // key << 9 | rank   (key < 2^22)
-#pragma unroll
-    for (int r = 0; r < kRounds; ++r) {
-        int idx = w * kWarpSpan + r * 32 + lane_id();
-        uint32_t key = kNone;
-        if (idx < (int)td.count) {
-            Rec rec = rec_from_smem(s.raw, idx);
-            if (classify_raw(g, bm, rec, s.edges, key) != C_SURVIVOR) key = kNone;
-        }
-        uint32_t rank = warp_rank(key == kNone ? kNone : (key & lo_mask), s.cnt + w * Bp);
-        packed[r] = key == kNone ? kNone : ((key << 9) | rank);
-    }
-    finish_ranks(s, B, Bp, table, stride, tile);
+    uint32_t phase_bits = 0;
+    for (uint32_t i = 0; i < n; ++i) {
+        const uint32_t stage = i % kStagesRaw;
+        uint32_t* raw = reinterpret_cast<uint32_t*>(smem + L.ring + stage * L.stage_bytes);
+        const TileDesc td = s_desc[stage];
+        ring_acquire(raw, &bars[stage], phase_bits, stage, td.ptr, td.count * kRecBytes);
 
+        uint32_t packed[kRounds];  // key << 9 | rank   (key < 2^22)
 #pragma unroll
-    for (int r = 0; r < kRounds; ++r) {
-        if (packed[r] != kNone) {
-            uint32_t key = packed[r] >> 9, rank = packed[r] & 511u, bucket = key & lo_mask;
-            uint32_t dest = s.gbase[bucket] + s.cnt[w * Bp + bucket] + rank;
+        for (int r = 0; r < kRounds; ++r) {
             int idx = w * kWarpSpan + r * 32 + lane_id();
-            const uint32_t* p = s.raw + idx * kRecWords;
-            aos[2 * (size_t)dest + 0] = make_uint4(key, p[1], p[2], p[3]);
-            aos[2 * (size_t)dest + 1] = make_uint4(p[4], p[5], p[6], td.first_index + idx);
-            hi16[dest] = (uint16_t)(key >> lo_bits);
+            uint32_t key = kNone;
+            if (idx < (int)td.count) {
+                Rec rec = rec_from_smem(raw, idx);
+                if (classify_raw(g, bm, rec, s_edges, key) != C_SURVIVOR) key = kNone;
+            }
+            uint32_t rank = warp_rank(key == kNone ? kNone : (key & lo_mask), cnt + w * Bp);
+            packed[r] = key == kNone ? kNone : ((key << 9) | rank);
+        }
+        __syncthreads();
+        finish_ranks<false>(cnt, B, Bp, gcur, nullptr, misc, grun);
+
+#pragma unroll
+        for (int r = 0; r < kRounds; ++r) {
+            if (packed[r] != kNone) {
+                uint32_t key = packed[r] >> 9, rank = packed[r] & 511u, bucket = key & lo_mask;
+                uint32_t dest = gcur[bucket] + cnt[w * Bp + bucket] + rank;
+                int idx = w * kWarpSpan + r * 32 + lane_id();
+                const uint32_t* p = raw + idx * kRecWords;
+                aos[2 * (size_t)dest + 0] = make_uint4(key, p[1], p[2], p[3]);
+                aos[2 * (size_t)dest + 1] = make_uint4(p[4], p[5], p[6], td.first_index + idx);
+                hi16[dest] = (uint16_t)(key >> lo_bits);
+            }
+        }
+        __syncwarp();
+        zero_row(cnt + w * Bp, Bp);
+        __syncthreads();  // the stage is free again
+        if (threadIdx.x == 0 && i + kStagesRaw < n) {
+            TileDesc d = raw_tile(chunks, n_chunks, t0 + i + kStagesRaw);
+            s_desc[stage] = d;
+            ring_issue(raw, &bars[stage], d.ptr, d.count * kRecBytes);
         }
     }
 }
 
-// INDEX pass B count: histogram of the uint16 high digits, tile by tile of the pass-A output.
+// tiles of the pass-A output: n = *n_ptr keyed records, contiguous
+__device__ __forceinline__ TileDesc keyed_tile(const uint4* aos, uint32_t n, uint32_t t)
+{
+    TileDesc d;
+    d.ptr = aos + 2 * (size_t)t * kTile;
+    d.first_index = t * kTile;
+    d.count = min((uint32_t)kTile, n - t * (uint32_t)kTile);
+    return d;
+}
+
+// INDEX pass B count: histogram of the uint16 high digits over the CTA's segment of the pass-A output.
 __global__ void __launch_bounds__(kThreads) k_count_hi16(const uint16_t* __restrict__ hi16,
                                                         const uint32_t* __restrict__ n_ptr, uint32_t B,
                                                         uint32_t* __restrict__ table, uint32_t stride)
 {
     extern __shared__ __align__(128) uint8_t smem[];
     uint32_t* hist = reinterpret_cast<uint32_t*>(smem);
-    const uint32_t tile = blockIdx.x;
+    const CountSmem L = count_layout(0, 0, B, 0);
+    const uint32_t rmask = (1u << L.rlog) - 1u;
     const uint32_t n = *n_ptr;
-    const uint32_t first = tile * kTile;
-    const uint32_t count = first < n ? min((uint32_t)kTile, n - first) : 0u;
-    for (uint32_t b = threadIdx.x; b < B; b += kThreads) hist[b] = 0;
+    Span sp = {0u, (n + kTile - 1) / kTile, 0u};
+    uint32_t t0, t1;
+    segment_of(sp, t0, t1);
+    for (uint32_t i = threadIdx.x; i < (B << L.rlog); i += kThreads) hist[i] = 0;
     __syncthreads();
+    // 8 digits per 16-byte load; the segment starts on a tile boundary, so the loads are aligned
+    const uint32_t first = t0 * kTile, last = min(n, t1 * (uint32_t)kTile);
+    const uint4* v = reinterpret_cast<const uint4*>(hi16 + first);
+    const uint32_t n8 = (last - first) / 8;
+    for (uint32_t i = threadIdx.x; i < n8; i += kThreads) {
+        uint4 d = __ldg(v + i);
+        uint32_t wds[4] = {d.x, d.y, d.z, d.w};
 #pragma unroll
-    for (int r = 0; r < kRounds; ++r) {
-        uint32_t idx = r * kThreads + threadIdx.x;
-        uint32_t bucket = idx < count ? (uint32_t)hi16[first + idx] : kNone;
-        uint32_t active = __ballot_sync(0xFFFFFFFFu, bucket != kNone);
-        if (bucket != kNone) {
-            uint32_t peers = __match_any_sync(active, bucket);
-            if ((int)lane_id() == __ffs(peers) - 1) atomicAdd(&hist[bucket], (uint32_t)__popc(peers));
+        for (int k = 0; k < 4; ++k) {
+            atomicAdd(&hist[((wds[k] & 0xFFFFu) << L.rlog) + (lane_id() & rmask)], 1u);
+            atomicAdd(&hist[((wds[k] >> 16) << L.rlog) + (lane_id() & rmask)], 1u);
         }
     }
+    for (uint32_t i = first + n8 * 8 + threadIdx.x; i < last; i += kThreads)
+        atomicAdd(&hist[((uint32_t)hi16[i] << L.rlog) + (lane_id() & rmask)], 1u);
     __syncthreads();
-    for (uint32_t b = threadIdx.x; b < B; b += kThreads) table[(size_t)b * stride + tile] = hist[b];
+    for (uint32_t b = threadIdx.x; b < B; b += kThreads) {
+        uint32_t c = 0;
+        for (uint32_t r = 0; r <= rmask; ++r) c += hist[(b << L.rlog) + ((r + lane_id()) & rmask)];
+        table[(size_t)b * stride + blockIdx.x] = c;
+    }
 }
 
 // ------------------------------------------------------------------------------------------------------
 // INDEX pass B scatter: keyed records (sorted by low digit) -> SoA index sorted by the full key, plus the
 // full key of every slot (used once, by binary search, to build offsets[K+1]).
 // ------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kThreads) k_scatter_idx_b(const uint4* __restrict__ aos,
-                                                           const uint16_t* __restrict__ hi16,
-                                                           const uint32_t* __restrict__ n_ptr, uint32_t B,
-                                                           const uint32_t* __restrict__ table, uint32_t stride,
-                                                           IdxOut out)
+__global__ void __launch_bounds__(kThreads, 2) k_scatter_idx_b(const uint4* __restrict__ aos,
+                                                              const uint32_t* __restrict__ n_ptr, uint32_t B,
+                                                              uint32_t lo_bits, const uint32_t* __restrict__ table,
+                                                              uint32_t stride, IdxOut out)
 {
     extern __shared__ __align__(128) uint8_t smem[];
     const uint32_t Bp = round_up(B, 8);
-    TileSmem s = carve(smem, kTile * 32, B, 0, true, true);
-    const uint32_t tile = blockIdx.x;
-    const uint32_t n = *n_ptr;
-    const uint32_t first = tile * kTile;
-    if (first >= n) return;
-    const uint32_t count = min((uint32_t)kTile, n - first);
+    const PartSmem L = part_layout(kTile * 32, kStagesKeyed, B, 0, true);
+    uint16_t* cnt = reinterpret_cast<uint16_t*>(smem + L.cnt);
+    uint32_t* gcur = reinterpret_cast<uint32_t*>(smem + L.gcur);
+    uint32_t* lstart = reinterpret_cast<uint32_t*>(smem + L.lstart);
+    uint32_t* pdest = reinterpret_cast<uint32_t*>(smem + L.pdest);
+    uint16_t* perm = reinterpret_cast<uint16_t*>(smem + L.perm);
+    uint32_t* misc = reinterpret_cast<uint32_t*>(smem + L.misc);
+    TileDesc* s_desc = reinterpret_cast<TileDesc*>(smem + L.desc);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + L.bars);
     const uint32_t w = warp_id();
+    const uint32_t n_rec = *n_ptr;
 
-    if (threadIdx.x == 0) {
-        mbar_init(s.bar, 1);
-        mbar_fence_init();
-    }
-    for (uint32_t i = threadIdx.x; i < kWarps * Bp / 2; i += kThreads) reinterpret_cast<uint32_t*>(s.cnt)[i] = 0;
+    Span sp = {0u, (n_rec + kTile - 1) / kTile, 0u};
+    uint32_t t0, t1;
+    segment_of(sp, t0, t1);
+    const uint32_t n = t1 - t0;
+    uint32_t grun[8];
+    auto desc_of = [&](uint32_t t) { return keyed_tile(aos, n_rec, t); };
+    scatter_prologue<kStagesKeyed>(smem, L, B, Bp, n, t0, 32u, desc_of, table, stride, blockIdx.x, grun);
     __syncthreads();
-    if (threadIdx.x == 0) {  // 32-byte records from a 256-byte-aligned array: always bulk-copyable
-        mbar_expect_tx(s.bar, count * 32);
-        tma_load_1d(s.raw, aos + 2 * (size_t)first, count * 32, s.bar);
-    }
 
-    uint32_t packed[kRounds];
-#pragma unroll
-    for (int r = 0; r < kRounds; ++r) {
-        uint32_t idx = w * kWarpSpan + r * 32 + lane_id();
-        uint32_t bucket = idx < count ? (uint32_t)hi16[first + idx] : kNone;
-        uint32_t rank = warp_rank(bucket, s.cnt + w * Bp);
-        packed[r] = bucket == kNone ? kNone : ((bucket << 9) | rank);
-    }
-    uint32_t n_part = finish_ranks(s, B, Bp, table, stride, tile);
+    uint32_t phase_bits = 0;
+    for (uint32_t i = 0; i < n; ++i) {
+        const uint32_t stage = i % kStagesKeyed;
+        uint32_t* raw = reinterpret_cast<uint32_t*>(smem + L.ring + stage * L.stage_bytes);
+        const TileDesc td = s_desc[stage];
+        ring_acquire(raw, &bars[stage], phase_bits, stage, td.ptr, td.count * 32u);
 
+        uint32_t packed[kRounds];
 #pragma unroll
-    for (int r = 0; r < kRounds; ++r) {
-        if (packed[r] != kNone) {
-            uint32_t bucket = packed[r] >> 9, rank = packed[r] & 511u;
-            uint32_t p = s.lstart[bucket] + s.cnt[w * Bp + bucket] + rank;
-            s.perm[p] = (uint16_t)(w * kWarpSpan + r * 32 + lane_id());
-            s.pbkt[p] = (uint16_t)bucket;
+        for (int r = 0; r < kRounds; ++r) {
+            uint32_t idx = w * kWarpSpan + r * 32 + lane_id();
+            uint32_t bucket = idx < td.count ? (raw[idx * 8] >> lo_bits) : kNone;
+            uint32_t rank = warp_rank(bucket, cnt + w * Bp);
+            packed[r] = bucket == kNone ? kNone : ((bucket << 9) | rank);
         }
-    }
-    mbar_wait(s.bar, 0);
-    __syncthreads();
+        __syncthreads();
+        const uint32_t n_part = finish_ranks<true>(cnt, B, Bp, gcur, lstart, misc, grun);
 
-    const uint4* s_rec = reinterpret_cast<const uint4*>(s.raw);
-    for (uint32_t j = threadIdx.x; j < n_part; j += kThreads) {
-        uint32_t i = s.perm[j], bucket = s.pbkt[j];
-        uint32_t dest = s.gbase[bucket] + (j - s.lstart[bucket]);
-        uint4 a = s_rec[2 * i + 0], b = s_rec[2 * i + 1];
-        out.key[dest] = a.x;
-        out.E[dest] = __uint_as_float(a.y);
-        out.x[dest] = __uint_as_float(a.z);
-        out.y[dest] = __uint_as_float(a.w);
-        out.u[dest] = __uint_as_float(b.x);
-        out.v[dest] = __uint_as_float(b.y);
-        out.wt[dest] = __uint_as_float(b.z);
-        out.src[dest] = b.w;
+#pragma unroll
+        for (int r = 0; r < kRounds; ++r) {
+            if (packed[r] != kNone) {
+                uint32_t bucket = packed[r] >> 9, rank = packed[r] & 511u;
+                uint32_t rel = cnt[w * Bp + bucket] + rank;
+                uint32_t p = lstart[bucket] + rel;
+                perm[p] = (uint16_t)(w * kWarpSpan + r * 32 + lane_id());
+                pdest[p] = gcur[bucket] + rel;
+            }
+        }
+        __syncwarp();
+        zero_row(cnt + w * Bp, Bp);
+        __syncthreads();
+
+        const uint4* s_rec = reinterpret_cast<const uint4*>(raw);
+        for (uint32_t j = threadIdx.x; j < n_part; j += kThreads) {
+            const uint32_t irec = perm[j];
+            const uint32_t dest = pdest[j];
+            uint4 a = s_rec[2 * irec + 0], b = s_rec[2 * irec + 1];
+            out.key[dest] = a.x;
+            out.E[dest] = __uint_as_float(a.y);
+            out.x[dest] = __uint_as_float(a.z);
+            out.y[dest] = __uint_as_float(a.w);
+            out.u[dest] = __uint_as_float(b.x);
+            out.v[dest] = __uint_as_float(b.y);
+            out.wt[dest] = __uint_as_float(b.z);
+            out.src[dest] = b.w;
+        }
+        __syncthreads();
+        if (threadIdx.x == 0 && i + kStagesKeyed < n) {
+            TileDesc d = keyed_tile(aos, n_rec, t0 + i + kStagesKeyed);
+            s_desc[stage] = d;
+            ring_issue(raw, &bars[stage], d.ptr, d.count * 32u);
+        }
     }
 }
 
@@ -576,34 +803,21 @@ __global__ void k_counts_from_offsets(const uint32_t* __restrict__ offsets, uint
     if (k % n_pos == 0 && k / n_pos <= n_batches) batch_offsets[k / n_pos] = o;
 }
 
-// describe the tiles of one chunk: tile t covers records [t*kTile, ...) of the chunk
-__global__ void k_fill_tiles(TileDesc* __restrict__ tiles, uint32_t tile0, uint32_t n_tiles, const uint8_t* base,
-                             uint32_t first_index, uint32_t n_records)
-{
-    uint32_t t = blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= n_tiles) return;
-    TileDesc d;
-    d.ptr = base + (size_t)t * kTile * kRecBytes;
-    d.first_index = first_index + t * kTile;
-    d.count = min((uint32_t)kTile, n_records - t * kTile);
-    tiles[tile0 + t] = d;
-}
-
-// fixed-order reduction of the per-tile statistics into one record (single CTA)
+// fixed-order reduction of the per-segment statistics into one record (single CTA)
 struct DevStats {
     unsigned long long n_invalid, n_outside, n_jaw, n_zero, n_surv;
     double sum_in, sum_idx, sum_out;
 };
 
-__global__ void __launch_bounds__(1024) k_reduce_stats(const TileStats* __restrict__ ts, uint32_t n_tiles,
+__global__ void __launch_bounds__(1024) k_reduce_stats(const SegStats* __restrict__ ts, uint32_t n_cols,
                                                        DevStats* __restrict__ out)
 {
     __shared__ unsigned long long s_n[32][5];
     __shared__ double s_d[32][3];
     unsigned long long n[5] = {0, 0, 0, 0, 0};
     double d[3] = {0.0, 0.0, 0.0};
-    for (uint32_t t = threadIdx.x; t < n_tiles; t += 1024) {
-        TileStats x = ts[t];
+    for (uint32_t t = threadIdx.x; t < n_cols; t += 1024) {
+        SegStats x = ts[t];
         n[0] += x.n_invalid; n[1] += x.n_outside; n[2] += x.n_jaw; n[3] += x.n_zero; n[4] += x.n_surv;
         d[0] += x.sum_in; d[1] += x.sum_idx; d[2] += x.sum_out;
     }
