@@ -191,6 +191,47 @@ void plan(const psl_config* c, const Derived& d, Layout* L)
 
 enum ResultKind { RES_NONE = 0, RES_OTF = 1, RES_INDEX = 2, RES_BEAM = 3 };
 
+// ---- kernel variants: the features a configuration / beam does not use are compiled out ------------------
+using CountFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, uint32_t, uint32_t*, uint32_t, SegStats*);
+using ScatterOtfFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, const uint32_t*, uint32_t, SoAOut, SegStats*);
+using ScatterIdxAFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, uint32_t, const uint32_t*, uint32_t, uint4*, uint16_t*);
+
+template <bool POS, bool EDGES>
+CountFn count_otf_pe(int beam)
+{
+    return beam == 0 ? k_count_raw<false, POS, EDGES, 0> : (beam == 1 ? k_count_raw<false, POS, EDGES, 1> : k_count_raw<false, POS, EDGES, 2>);
+}
+CountFn count_otf_fn(bool pos, bool edges, int beam)
+{
+    return pos ? (edges ? count_otf_pe<true, true>(beam) : count_otf_pe<true, false>(beam))
+               : (edges ? count_otf_pe<false, true>(beam) : count_otf_pe<false, false>(beam));
+}
+CountFn count_idx_fn(bool pos, bool edges)
+{
+    return pos ? (edges ? k_count_raw<true, true, true, 0> : k_count_raw<true, true, false, 0>)
+               : (edges ? k_count_raw<true, false, true, 0> : k_count_raw<true, false, false, 0>);
+}
+template <bool POS, bool EDGES, bool PROJ>
+ScatterOtfFn scatter_otf_pep(int beam)
+{
+    return beam == 0 ? k_scatter_otf<POS, EDGES, 0, PROJ> : (beam == 1 ? k_scatter_otf<POS, EDGES, 1, PROJ> : k_scatter_otf<POS, EDGES, 2, PROJ>);
+}
+template <bool POS, bool EDGES>
+ScatterOtfFn scatter_otf_pe(int beam, bool proj)
+{
+    return proj ? scatter_otf_pep<POS, EDGES, true>(beam) : scatter_otf_pep<POS, EDGES, false>(beam);
+}
+ScatterOtfFn scatter_otf_fn(bool pos, bool edges, int beam, bool proj)
+{
+    return pos ? (edges ? scatter_otf_pe<true, true>(beam, proj) : scatter_otf_pe<true, false>(beam, proj))
+               : (edges ? scatter_otf_pe<false, true>(beam, proj) : scatter_otf_pe<false, false>(beam, proj));
+}
+ScatterIdxAFn scatter_idx_a_fn(bool pos, bool edges)
+{
+    return pos ? (edges ? k_scatter_idx_a<true, true> : k_scatter_idx_a<true, false>)
+               : (edges ? k_scatter_idx_a<false, true> : k_scatter_idx_a<false, false>);
+}
+
 }  // namespace
 
 struct psl_ctx {
@@ -442,10 +483,12 @@ psl_status build_onthefly(psl_ctx* ctx, const DevBeam& bm)
         SegStats* ss = at<SegStats>(ctx, L.sstats);
         const uint32_t S = nt < ctx->S_otf ? nt : ctx->S_otf;  // one persistent CTA per segment, one wave
         const Span span = {0u, nt, 0u};
+        const bool pos = ctx->grid.has_pos != 0, edges = ctx->grid.ebin_mode != 0, proj = bm.has_map || bm.out_proj;
+        const int bv = beam_variant(bm);
         {
             Prof prof(ctx, PSL_K_COUNT);
-            k_count_raw<false><<<S, kThreads, ctx->sm_count_raw, ctx->stream>>>(chunks, ctx->n_chunks, span, ctx->grid, bm, d.K, 0,
-                                                                              table, d.cols_cap, ss);
+            count_otf_fn(pos, edges, bv)<<<S, kThreads, ctx->sm_count_raw, ctx->stream>>>(chunks, ctx->n_chunks, span, ctx->grid, bm, d.K, 0,
+                                                                                        table, d.cols_cap, ss);
             LAUNCHED();
         }
         psl_status s = run_scan(ctx, table, d.K, S, d.cols_cap, scalar(ctx, SC_TOTAL));
@@ -455,8 +498,8 @@ psl_status build_onthefly(psl_ctx* ctx, const DevBeam& bm)
         LAUNCHED();
         {
             Prof prof(ctx, PSL_K_SCATTER);
-            k_scatter_otf<<<S, kThreads, ctx->sm_scatter_otf, ctx->stream>>>(chunks, ctx->n_chunks, span, ctx->grid, bm, d.K, table,
-                                                                            d.cols_cap, soa_out(ctx, L.out), ss);
+            scatter_otf_fn(pos, edges, bv, proj)<<<S, kThreads, ctx->sm_scatter_otf, ctx->stream>>>(chunks, ctx->n_chunks, span, ctx->grid, bm,
+                                                                                                   d.K, table, d.cols_cap, soa_out(ctx, L.out), ss);
             LAUNCHED();
         }
         k_reduce_stats<<<1, 1024, 0, ctx->stream>>>(ss, S, stats);
@@ -510,8 +553,8 @@ psl_status finalize_index(psl_ctx* ctx)
         {
             Prof prof(ctx, PSL_K_INDEX_A);
             for (const psl_ctx::ChunkLaunch& cl : ctx->idx_launches) {  // the same segments the counts were taken on
-                k_scatter_idx_a<<<cl.n_seg, kThreads, ctx->sm_idx_a, ctx->stream>>>(chunks, ctx->n_chunks, cl.span, ctx->grid, none,
-                                                                                  d.B_lo, d.lo_bits, table_a, d.cols_cap, aos, hi16);
+                scatter_idx_a_fn(ctx->grid.has_pos != 0, ctx->grid.ebin_mode != 0)<<<cl.n_seg, kThreads, ctx->sm_idx_a, ctx->stream>>>(
+                    chunks, ctx->n_chunks, cl.span, ctx->grid, none, d.B_lo, d.lo_bits, table_a, d.cols_cap, aos, hi16);
                 LAUNCHED();
             }
         }
@@ -782,21 +825,26 @@ psl_status psl_create(const psl_config* cfg, psl_ctx** out)
     if (cfg->mode == PSL_MODE_ONTHEFLY) {
         ctx->sm_count_raw = count_layout(kTile * kRecBytes, kStagesCount, d.K, ne).total;
         ctx->sm_scatter_otf = part_layout(kTile * kRecBytes, kStagesRaw, d.K, ne, true).total;
-        CUC(allow_smem(k_count_raw<false>, ctx->sm_count_raw));
-        CUC(allow_smem(k_scatter_otf, ctx->sm_scatter_otf));
-        CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_scatter_otf, kThreads, ctx->sm_scatter_otf));
+        const bool pos = d.n_pos > 1, edges = cfg->ebin_mode == PSL_EBIN_EDGES;
+        for (int bv = 0; bv < 3; ++bv) {
+            CUC(allow_smem(count_otf_fn(pos, edges, bv), ctx->sm_count_raw));
+            CUC(allow_smem(scatter_otf_fn(pos, edges, bv, false), ctx->sm_scatter_otf));
+            CUC(allow_smem(scatter_otf_fn(pos, edges, bv, true), ctx->sm_scatter_otf));
+        }
+        CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, scatter_otf_fn(pos, edges, 2, true), kThreads, ctx->sm_scatter_otf));
         ctx->S_otf = width(occ);
     } else {
         ctx->sm_count_raw = count_layout(kTile * kRecBytes, kStagesCount, d.B_lo, ne).total;
         ctx->sm_idx_a = part_layout(kTile * kRecBytes, kStagesRaw, d.B_lo, ne, false).total;
         ctx->sm_count_b = count_layout(0, 0, d.B_hi, 0).total;
         ctx->sm_idx_b = part_layout(kTile * 32, kStagesKeyed, d.B_hi, 0, true).total;
-        CUC(allow_smem(k_count_raw<true>, ctx->sm_count_raw));
-        CUC(allow_smem(k_scatter_idx_a, ctx->sm_idx_a));
+        const bool pos = d.n_pos > 1, edges = cfg->ebin_mode == PSL_EBIN_EDGES;
+        CUC(allow_smem(count_idx_fn(pos, edges), ctx->sm_count_raw));
+        CUC(allow_smem(scatter_idx_a_fn(pos, edges), ctx->sm_idx_a));
         CUC(allow_smem(k_count_hi16, ctx->sm_count_b));
         CUC(allow_smem(k_scatter_idx_b, ctx->sm_idx_b));
         CUC(allow_smem(k_beam_compact, 11 * kBeamTile * 4));
-        CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_scatter_idx_a, kThreads, ctx->sm_idx_a));
+        CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, scatter_idx_a_fn(pos, edges), kThreads, ctx->sm_idx_a));
         ctx->S_a = width(occ);
         CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_scatter_idx_b, kThreads, ctx->sm_idx_b));
         ctx->S_b = width(occ);
@@ -894,10 +942,9 @@ psl_status psl_load_chunk(psl_ctx* ctx, const void* records, uint64_t n, int32_t
         cl.n_seg = nt < ctx->S_a ? nt : ctx->S_a;
         if (ctx->n_cols + cl.n_seg > ctx->d.cols_cap) { set_err(ctx->err, "load_chunk: out of table columns"); return PSL_ERR_CAPACITY; }
         Prof prof(ctx, PSL_K_COUNT);
-        k_count_raw<true><<<cl.n_seg, kThreads, ctx->sm_count_raw, ctx->stream>>>(chunks, ctx->n_chunks + 1, cl.span, ctx->grid, none,
-                                                                                ctx->d.B_lo, (1u << ctx->d.lo_bits) - 1u,
-                                                                                at<uint32_t>(ctx, ctx->L.table_a), ctx->d.cols_cap,
-                                                                                at<SegStats>(ctx, ctx->L.sstats));
+        count_idx_fn(ctx->grid.has_pos != 0, ctx->grid.ebin_mode != 0)<<<cl.n_seg, kThreads, ctx->sm_count_raw, ctx->stream>>>(
+            chunks, ctx->n_chunks + 1, cl.span, ctx->grid, none, ctx->d.B_lo, (1u << ctx->d.lo_bits) - 1u,
+            at<uint32_t>(ctx, ctx->L.table_a), ctx->d.cols_cap, at<SegStats>(ctx, ctx->L.sstats));
         LAUNCHED();
         ctx->idx_launches.push_back(cl);
         ctx->n_cols += cl.n_seg;

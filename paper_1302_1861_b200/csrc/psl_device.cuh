@@ -149,32 +149,70 @@ __device__ __forceinline__ float final_weight(const DevBeam& b, float wt, float 
 }
 
 // Steps 1-4 (+6, +8 when a beam is given) for one raw record.  Returns the class; key is valid for every
-// class except C_INVALID / C_OUTSIDE.
-__device__ __forceinline__ int classify_raw(const DevGrid& g, const DevBeam& b, const Rec& r, const float* s_edges,
-                                            uint32_t& key)
+// class except C_INVALID / C_OUTSIDE.  Straight-line code (selects, no data-dependent branches) so that the
+// records a thread owns are classified in an interleaved instruction stream.  Compile-time features:
+//   POS   the grid has position bins (a3)            EDGES  energy bins from the edge table (a2)
+//   BEAM  0: nothing rejects a valid in-grid record  1: jaws only (a6)  2: run-time jaws / PSL_DROP_ZERO_WEIGHT
+template <bool POS, bool EDGES, int BEAM>
+__device__ __forceinline__ int classify(const DevGrid& g, const DevBeam& b, const Rec& r, const float* s_edges, uint32_t& key)
 {
-    key = kNone;
-    float q = q_of(r.u, r.v);
-    if (!rec_valid(r, q)) return C_INVALID;
+    const float q = q_of(r.u, r.v);
+    // q > 0 already implies finite u and v (an infinite or NaN cosine makes q -inf or NaN)
+    const bool valid = ((uint32_t)r.type <= 2u) & is_finite(r.E) & is_finite(r.x) & is_finite(r.y) & is_finite(r.wt) &
+                       (r.E > 0.0f) & (q > 0.0f);
     int ix = 0, iy = 0;
-    if (g.has_pos) {
-        if (!axis_bin(r.x, g.inv_dx, g.ix0, g.n_xbins, ix)) return C_OUTSIDE;
-        if (!axis_bin(r.y, g.inv_dy, g.iy0, g.n_ybins, iy)) return C_OUTSIDE;
+    bool inside = true;
+    if (POS) {
+        const bool okx = axis_bin(r.x, g.inv_dx, g.ix0, g.n_xbins, ix);
+        const bool oky = axis_bin(r.y, g.inv_dy, g.iy0, g.n_ybins, iy);
+        inside = okx & oky;
     }
-    int ie = energy_bin(g, r.E, s_edges);
-    key = (uint32_t)(type_division(g, r.type) * g.n_ebins + ie) * g.n_pos + (uint32_t)(iy * g.n_xbins + ix);
-    if (!b.has_beam) return C_SURVIVOR;
-    if (b.has_jaws || b.drop_zero) {
+    int ie;
+    if (!EDGES) {
+        // floor((E - e_min) / dE) clamped into [0, n_ebins - 1]; one IEEE division
+        float t = floorf(__fdiv_rn(__fsub_rn(r.E, g.e_min), g.dE));
+        ie = (int)fminf(fmaxf(t, 0.0f), (float)(g.n_ebins - 1));
+    } else {
+        int lo = 1, hi = g.n_ebins;  // first k in [1, n_ebins) with edges[k] > E
+        while (lo < hi) {
+            int mid = (lo + hi) >> 1;
+            if (s_edges[mid] <= r.E) lo = mid + 1; else hi = mid;
+        }
+        ie = lo - 1;
+    }
+    const int td = min(r.type, g.n_types - 1);  // n_types == 2 merges electrons and positrons
+    uint32_t k = (uint32_t)(td * g.n_ebins + ie);
+    if (POS) k = k * g.n_pos + (uint32_t)(iy * g.n_xbins + ix);
+    key = k;
+    int cls = C_SURVIVOR;
+    if (BEAM == 1) {
         float w, tx, ty;
         slopes(r.u, r.v, q, w, tx, ty);
-        if (b.has_jaws && !jaw_pass(b, r.x, r.y, tx, ty)) return C_JAW;
-        if (b.drop_zero) {
-            float xm = __fadd_rn(r.x, __fmul_rn(tx, b.dzM));
-            float ym = __fadd_rn(r.y, __fmul_rn(ty, b.dzM));
-            if (final_weight(b, r.wt, xm, ym) == 0.0f) return C_ZERO;
+        if (!jaw_pass(b, r.x, r.y, tx, ty)) cls = C_JAW;
+    }
+    if (BEAM == 2) {
+        if (valid && inside && (b.has_jaws || b.drop_zero)) {
+            float w, tx, ty;
+            slopes(r.u, r.v, q, w, tx, ty);
+            if (b.has_jaws && !jaw_pass(b, r.x, r.y, tx, ty)) {
+                cls = C_JAW;
+            } else if (b.drop_zero) {
+                float xm = __fadd_rn(r.x, __fmul_rn(tx, b.dzM));
+                float ym = __fadd_rn(r.y, __fmul_rn(ty, b.dzM));
+                if (final_weight(b, r.wt, xm, ym) == 0.0f) cls = C_ZERO;
+            }
         }
     }
-    return C_SURVIVOR;
+    if (!inside) cls = C_OUTSIDE;
+    if (!valid) cls = C_INVALID;
+    return cls;
+}
+
+// which BEAM variant of classify() a beam needs
+__host__ __device__ inline int beam_variant(const DevBeam& b)
+{
+    if (!b.has_beam || (!b.has_jaws && !b.drop_zero)) return 0;
+    return b.drop_zero ? 2 : 1;
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -28,10 +28,10 @@ constexpr int kScanThreads = 256;
 constexpr int kScanRows = 16;
 constexpr int kScanBlock = kScanThreads * kScanRows;  // 4096 table entries per scan CTA
 
-constexpr int kStagesCount = 4;   // ring depth of the histogram kernels (28 KB stages)
+constexpr int kStagesCount = 3;   // ring depth of the histogram kernels (28 KB stages)
 constexpr int kStagesRaw = 3;     // ring depth of the scatter kernels that read raw records
 constexpr int kStagesKeyed = 2;   // ring depth of INDEX pass B (32 KB stages)
-constexpr int kHistBytes = 32768; // privatised histogram budget of the histogram kernels
+constexpr int kHistBytes = 16384; // privatised histogram budget of the histogram kernels
 
 struct SoAOut {
     float *E, *x, *y, *u, *v, *w, *wt, *xp, *yp;
@@ -255,7 +255,7 @@ __device__ __forceinline__ void write_seg_stats(ThreadStats t, SegStats* __restr
 //                          IDX = true : INDEX pass A, bucket = key & lo_mask of valid in-grid records.
 // Also writes the segment's statistics (every record falls in exactly one class).
 // ------------------------------------------------------------------------------------------------------
-template <bool IDX>
+template <bool IDX, bool POS, bool EDGES, int BEAM>
 __global__ void __launch_bounds__(kThreads, 2) k_count_raw(const ChunkDesc* __restrict__ chunks, uint32_t n_chunks,
                                                           Span sp, const __grid_constant__ DevGrid g,
                                                           const __grid_constant__ DevBeam bm, uint32_t B,
@@ -294,27 +294,30 @@ __global__ void __launch_bounds__(kThreads, 2) k_count_raw(const ChunkDesc* __re
         uint32_t* raw = reinterpret_cast<uint32_t*>(smem + L.ring + stage * L.stage_bytes);
         const TileDesc td = s_desc[stage];
         ring_acquire(raw, &bars[stage], phase_bits, stage, td.ptr, td.count * kRecBytes);
+        // all of the thread's records first, then straight-line classification: independent chains interleave
+        Rec rec[kRounds];
+        bool have[kRounds];
 #pragma unroll
         for (int r = 0; r < kRounds; ++r) {
             const int idx = r * kThreads + threadIdx.x;
-            if (idx < (int)td.count) {
-                Rec rec = rec_from_smem(raw, idx);
-                uint32_t key;
-                int cls = classify_raw(g, bm, rec, s_edges, key);
-                if (cls != C_INVALID) {
-                    double wd = (double)rec.wt;
-                    st.sum_in += wd;
-                    if (cls != C_OUTSIDE) st.sum_idx += wd;
-                }
-                st.n_inv += cls == C_INVALID;
-                st.n_out += cls == C_OUTSIDE;
-                st.n_jaw += cls == C_JAW;
-                st.n_zero += cls == C_ZERO;
-                if (cls == C_SURVIVOR) {
-                    st.n_surv += 1;
-                    uint32_t bucket = IDX ? (key & lo_mask) : key;
-                    atomicAdd(&hist[(bucket << L.rlog) + (lane_id() & rmask)], 1u);
-                }
+            have[r] = idx < (int)td.count;
+            rec[r] = rec_from_smem(raw, have[r] ? idx : 0);
+        }
+#pragma unroll
+        for (int r = 0; r < kRounds; ++r) {
+            uint32_t key;
+            const int cls = classify<POS, EDGES, BEAM>(g, bm, rec[r], s_edges, key);
+            const bool valid = have[r] & (cls != C_INVALID);
+            st.sum_in += (double)(valid ? rec[r].wt : 0.0f);
+            if (POS) st.sum_idx += (double)((valid & (cls != C_OUTSIDE)) ? rec[r].wt : 0.0f);
+            st.n_inv += have[r] & (cls == C_INVALID);
+            if (POS) st.n_out += have[r] & (cls == C_OUTSIDE);
+            if (BEAM != 0) st.n_jaw += have[r] & (cls == C_JAW);
+            if (BEAM == 2) st.n_zero += have[r] & (cls == C_ZERO);
+            if (have[r] & (cls == C_SURVIVOR)) {
+                st.n_surv += 1;
+                const uint32_t bucket = IDX ? (key & lo_mask) : key;
+                atomicAdd(&hist[(bucket << L.rlog) + (lane_id() & rmask)], 1u);
             }
         }
         __syncthreads();  // every thread is done with the stage
@@ -331,6 +334,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_count_raw(const ChunkDesc* __re
         for (uint32_t r = 0; r <= rmask; ++r) c += hist[(b << L.rlog) + ((r + lane_id()) & rmask)];
         table[(size_t)b * stride + col] = c;
     }
+    if (!POS) st.sum_idx = st.sum_in;  // no grid to fall out of
     write_seg_stats(st, &sstats[col]);
 }
 
@@ -453,6 +457,8 @@ __device__ __forceinline__ void scatter_prologue(uint8_t* smem, const PartSmem& 
 // Survivors are ordered inside the tile by (key, input order) so that consecutive threads write consecutive
 // slots of a key (block-local staging before the global scatter).
 // ------------------------------------------------------------------------------------------------------
+// PROJ: the ray slopes are needed at write-out (a fluence map to look up, or PSL_OUT_PROJ).
+template <bool POS, bool EDGES, int BEAM, bool PROJ>
 __global__ void __launch_bounds__(kThreads, 2) k_scatter_otf(const ChunkDesc* __restrict__ chunks, uint32_t n_chunks,
                                                             Span sp, const __grid_constant__ DevGrid g,
                                                             const __grid_constant__ DevBeam bm, uint32_t B,
@@ -493,17 +499,26 @@ __global__ void __launch_bounds__(kThreads, 2) k_scatter_otf(const ChunkDesc* __
 
         // bucket and stable rank inside the warp's slice of the tile
         uint32_t packed[kRounds];  // bucket << 9 | rank   (bucket < 2^11, rank < 2^7)
+        {
+            Rec rec[kRounds];
 #pragma unroll
-        for (int r = 0; r < kRounds; ++r) {
-            int idx = w * kWarpSpan + r * 32 + lane_id();
-            uint32_t bucket = kNone;
-            if (idx < (int)td.count) {
-                Rec rec = rec_from_smem(raw, idx);
-                uint32_t key;
-                if (classify_raw(g, bm, rec, s_edges, key) == C_SURVIVOR) bucket = key;
+            for (int r = 0; r < kRounds; ++r) {
+                int idx = w * kWarpSpan + r * 32 + lane_id();
+                rec[r] = rec_from_smem(raw, idx < (int)td.count ? idx : 0);
             }
-            uint32_t rank = warp_rank(bucket, cnt + w * Bp);
-            packed[r] = bucket == kNone ? kNone : ((bucket << 9) | rank);
+#pragma unroll
+            for (int r = 0; r < kRounds; ++r) {  // straight-line: the four classifications interleave
+                int idx = w * kWarpSpan + r * 32 + lane_id();
+                uint32_t key;
+                int cls = classify<POS, EDGES, BEAM>(g, bm, rec[r], s_edges, key);
+                packed[r] = (idx < (int)td.count && cls == C_SURVIVOR) ? key : kNone;
+            }
+#pragma unroll
+            for (int r = 0; r < kRounds; ++r) {  // ranks: round r before round r + 1
+                uint32_t bucket = packed[r];
+                uint32_t rank = warp_rank(bucket, cnt + w * Bp);
+                packed[r] = bucket == kNone ? kNone : ((bucket << 9) | rank);
+            }
         }
         __syncthreads();
         const uint32_t n_part = finish_ranks<true>(cnt, B, Bp, gcur, lstart, misc, grun);
@@ -528,11 +543,17 @@ __global__ void __launch_bounds__(kThreads, 2) k_scatter_otf(const ChunkDesc* __
             const uint32_t irec = perm[j];
             const uint32_t dest = pdest[j];
             Rec rec = rec_from_smem(raw, (int)irec);
-            float q = q_of(rec.u, rec.v), wz, tx, ty;
-            slopes(rec.u, rec.v, q, wz, tx, ty);
-            float xm = __fadd_rn(rec.x, __fmul_rn(tx, bm.dzM));
-            float ym = __fadd_rn(rec.y, __fmul_rn(ty, bm.dzM));
-            float wt = final_weight(bm, rec.wt, xm, ym);
+            float q = q_of(rec.u, rec.v), wz, xm = 0.0f, ym = 0.0f, wt;
+            if (PROJ) {
+                float tx, ty;
+                slopes(rec.u, rec.v, q, wz, tx, ty);
+                xm = __fadd_rn(rec.x, __fmul_rn(tx, bm.dzM));
+                ym = __fadd_rn(rec.y, __fmul_rn(ty, bm.dzM));
+                wt = final_weight(bm, rec.wt, xm, ym);
+            } else {  // no map, no projected outputs: the weight is wt or wt * mu
+                wz = __fsqrt_rn(q);
+                wt = bm.has_beam ? __fmul_rn(rec.wt, bm.mu) : rec.wt;
+            }
             out.E[dest] = rec.E;
             out.x[dest] = rec.x;
             out.y[dest] = rec.y;
@@ -541,7 +562,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_scatter_otf(const ChunkDesc* __
             out.w[dest] = wz;
             out.wt[dest] = wt;
             out.src[dest] = td.first_index + irec;
-            if (bm.out_proj) {
+            if (PROJ && bm.out_proj) {
                 out.xp[dest] = xm;
                 out.yp[dest] = ym;
             }
@@ -571,6 +592,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_scatter_otf(const ChunkDesc* __
 // Also writes the high digit of every record (uint16) to hi16[] in the new order, which is all pass B's
 // count needs to read.
 // ------------------------------------------------------------------------------------------------------
+template <bool POS, bool EDGES>
 __global__ void __launch_bounds__(kThreads, 2) k_scatter_idx_a(const ChunkDesc* __restrict__ chunks, uint32_t n_chunks,
                                                               Span sp, const __grid_constant__ DevGrid g,
                                                               const __grid_constant__ DevBeam bm, uint32_t B,
@@ -607,16 +629,26 @@ __global__ void __launch_bounds__(kThreads, 2) k_scatter_idx_a(const ChunkDesc* 
         ring_acquire(raw, &bars[stage], phase_bits, stage, td.ptr, td.count * kRecBytes);
 
         uint32_t packed[kRounds];  // key << 9 | rank   (key < 2^22)
+        {
+            Rec rec[kRounds];
 #pragma unroll
-        for (int r = 0; r < kRounds; ++r) {
-            int idx = w * kWarpSpan + r * 32 + lane_id();
-            uint32_t key = kNone;
-            if (idx < (int)td.count) {
-                Rec rec = rec_from_smem(raw, idx);
-                if (classify_raw(g, bm, rec, s_edges, key) != C_SURVIVOR) key = kNone;
+            for (int r = 0; r < kRounds; ++r) {
+                int idx = w * kWarpSpan + r * 32 + lane_id();
+                rec[r] = rec_from_smem(raw, idx < (int)td.count ? idx : 0);
             }
-            uint32_t rank = warp_rank(key == kNone ? kNone : (key & lo_mask), cnt + w * Bp);
-            packed[r] = key == kNone ? kNone : ((key << 9) | rank);
+#pragma unroll
+            for (int r = 0; r < kRounds; ++r) {
+                int idx = w * kWarpSpan + r * 32 + lane_id();
+                uint32_t key;
+                int cls = classify<POS, EDGES, 0>(g, bm, rec[r], s_edges, key);
+                packed[r] = (idx < (int)td.count && cls == C_SURVIVOR) ? key : kNone;
+            }
+#pragma unroll
+            for (int r = 0; r < kRounds; ++r) {
+                uint32_t key = packed[r];
+                uint32_t rank = warp_rank(key == kNone ? kNone : (key & lo_mask), cnt + w * Bp);
+                packed[r] = key == kNone ? kNone : ((key << 9) | rank);
+            }
         }
         __syncthreads();
         finish_ranks<false>(cnt, B, Bp, gcur, nullptr, misc, grun);
