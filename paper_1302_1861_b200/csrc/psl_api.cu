@@ -14,6 +14,7 @@
 #include <vector>
 
 #include "psl_beam.cuh"
+#include "psl_bigtile.cuh"
 #include "psl_device.cuh"
 #include "psl_partition.cuh"
 
@@ -226,6 +227,22 @@ ScatterOtfFn scatter_otf_fn(bool pos, bool edges, int beam, bool proj)
     return pos ? (edges ? scatter_otf_pe<true, true>(beam, proj) : scatter_otf_pe<true, false>(beam, proj))
                : (edges ? scatter_otf_pe<false, true>(beam, proj) : scatter_otf_pe<false, false>(beam, proj));
 }
+template <bool POS, bool EDGES, bool PROJ>
+ScatterOtfFn scatter_big_pep(int beam)
+{
+    return beam == 0 ? k_scatter_otf_big<POS, EDGES, 0, PROJ> : (beam == 1 ? k_scatter_otf_big<POS, EDGES, 1, PROJ> : k_scatter_otf_big<POS, EDGES, 2, PROJ>);
+}
+template <bool POS, bool EDGES>
+ScatterOtfFn scatter_big_pe(int beam, bool proj)
+{
+    return proj ? scatter_big_pep<POS, EDGES, true>(beam) : scatter_big_pep<POS, EDGES, false>(beam);
+}
+// the 4096-record-tile scatter (keys <= kBigMaxKeys)
+ScatterOtfFn scatter_big_fn(bool pos, bool edges, int beam, bool proj)
+{
+    return pos ? (edges ? scatter_big_pe<true, true>(beam, proj) : scatter_big_pe<true, false>(beam, proj))
+               : (edges ? scatter_big_pe<false, true>(beam, proj) : scatter_big_pe<false, false>(beam, proj));
+}
 ScatterIdxAFn scatter_idx_a_fn(bool pos, bool edges)
 {
     return pos ? (edges ? k_scatter_idx_a<true, true> : k_scatter_idx_a<true, false>)
@@ -255,6 +272,7 @@ struct psl_ctx {
     bool seg_pending = false;
     // launch shapes: persistent CTAs per launch (= SMs x resident CTAs of the scatter kernel, one wave)
     uint32_t S_otf = 0, S_a = 0, S_b = 0;
+    bool big_tiles = false;  // ONTHEFLY with few keys: the 4096-record-tile scatter
     uint32_t sm_count_raw = 0, sm_scatter_otf = 0, sm_idx_a = 0, sm_count_b = 0, sm_idx_b = 0;  // dynamic smem bytes
     struct ChunkLaunch { Span span; uint32_t n_seg; };
     std::vector<ChunkLaunch> idx_launches;  // INDEX: the per-chunk count launches, replayed by pass A's scatter
@@ -498,8 +516,12 @@ psl_status build_onthefly(psl_ctx* ctx, const DevBeam& bm)
         LAUNCHED();
         {
             Prof prof(ctx, PSL_K_SCATTER);
-            scatter_otf_fn(pos, edges, bv, proj)<<<S, kThreads, ctx->sm_scatter_otf, ctx->stream>>>(chunks, ctx->n_chunks, span, ctx->grid, bm,
-                                                                                                   d.K, table, d.cols_cap, soa_out(ctx, L.out), ss);
+            if (ctx->big_tiles)
+                scatter_big_fn(pos, edges, bv, proj)<<<S, kBigThreads, ctx->sm_scatter_otf, ctx->stream>>>(chunks, ctx->n_chunks, span, ctx->grid, bm,
+                                                                                                          d.K, table, d.cols_cap, soa_out(ctx, L.out), ss);
+            else
+                scatter_otf_fn(pos, edges, bv, proj)<<<S, kThreads, ctx->sm_scatter_otf, ctx->stream>>>(chunks, ctx->n_chunks, span, ctx->grid, bm,
+                                                                                                       d.K, table, d.cols_cap, soa_out(ctx, L.out), ss);
             LAUNCHED();
         }
         k_reduce_stats<<<1, 1024, 0, ctx->stream>>>(ss, S, stats);
@@ -824,14 +846,19 @@ psl_status psl_create(const psl_config* cfg, psl_ctx** out)
     int occ = 0;
     if (cfg->mode == PSL_MODE_ONTHEFLY) {
         ctx->sm_count_raw = count_layout(kTile * kRecBytes, kStagesCount, d.K, ne).total;
-        ctx->sm_scatter_otf = part_layout(kTile * kRecBytes, kStagesRaw, d.K, ne, true).total;
+        ctx->big_tiles = round_up(d.K, 8) <= (uint32_t)kBigMaxKeys;
+        ctx->sm_scatter_otf = ctx->big_tiles ? big_layout(d.K, ne).total : part_layout(kTile * kRecBytes, kStagesRaw, d.K, ne, true).total;
         const bool pos = d.n_pos > 1, edges = cfg->ebin_mode == PSL_EBIN_EDGES;
         for (int bv = 0; bv < 3; ++bv) {
             CUC(allow_smem(count_otf_fn(pos, edges, bv), ctx->sm_count_raw));
-            CUC(allow_smem(scatter_otf_fn(pos, edges, bv, false), ctx->sm_scatter_otf));
-            CUC(allow_smem(scatter_otf_fn(pos, edges, bv, true), ctx->sm_scatter_otf));
+            for (int pj = 0; pj < 2; ++pj)
+                CUC(allow_smem(ctx->big_tiles ? scatter_big_fn(pos, edges, bv, pj != 0) : scatter_otf_fn(pos, edges, bv, pj != 0),
+                               ctx->sm_scatter_otf));
         }
-        CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, scatter_otf_fn(pos, edges, 2, true), kThreads, ctx->sm_scatter_otf));
+        if (ctx->big_tiles)
+            CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, scatter_big_fn(pos, edges, 2, true), kBigThreads, ctx->sm_scatter_otf));
+        else
+            CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, scatter_otf_fn(pos, edges, 2, true), kThreads, ctx->sm_scatter_otf));
         ctx->S_otf = width(occ);
     } else {
         ctx->sm_count_raw = count_layout(kTile * kRecBytes, kStagesCount, d.B_lo, ne).total;

@@ -328,25 +328,19 @@ __device__ __forceinline__ double warp_sum_double(double v)
 
 // Stable rank of a record inside its warp's slice of the tile: records of one warp arrive in rounds of 32
 // consecutive records; `cnt` is the warp's private running count per bucket.  Lanes with bucket == kNone
-// take no part.  Must be called by all 32 lanes.
+// match among themselves and touch no counter.  Must be called by all 32 lanes (full-mask collectives only).
 __device__ __forceinline__ uint32_t warp_rank(uint32_t bucket, uint16_t* cnt)
 {
-    uint32_t rank = 0;
-    uint32_t active = __ballot_sync(0xFFFFFFFFu, bucket != kNone);
-    if (bucket != kNone) {
-        uint32_t peers = __match_any_sync(active, bucket);
-        int leader = __ffs(peers) - 1;
-        uint32_t before = __popc(peers & lanemask_lt());
-        uint32_t base = 0;
-        if ((int)lane_id() == leader) {
-            base = cnt[bucket];
-            cnt[bucket] = (uint16_t)(base + __popc(peers));
-        }
-        base = __shfl_sync(peers, base, leader);
-        rank = base + before;
+    const uint32_t peers = __match_any_sync(0xFFFFFFFFu, bucket);
+    const int leader = __ffs(peers) - 1;
+    uint32_t base = 0;
+    if ((int)lane_id() == leader && bucket != kNone) {
+        base = cnt[bucket];
+        cnt[bucket] = (uint16_t)(base + __popc(peers));
     }
+    base = __shfl_sync(0xFFFFFFFFu, base, leader);
     __syncwarp();
-    return rank;
+    return base + __popc(peers & lanemask_lt());
 }
 
 }  // namespace psl

@@ -169,7 +169,7 @@ __device__ __forceinline__ void ring_acquire(uint32_t* s_dst, uint64_t* bar, uin
 // of bucket b for this tile and advances the thread's running slots grun[8].  With STAGED also lstart[b] =
 // exclusive prefix over buckets of the tile totals; returns the number of records that take part.
 // Must be called by all threads after a __syncthreads; ends with a __syncthreads.
-template <bool STAGED>
+template <bool STAGED, int NW = kWarps>
 __device__ __forceinline__ uint32_t finish_ranks(uint16_t* cnt, uint32_t B, uint32_t Bp, uint32_t* gcur, uint32_t* lstart,
                                                  uint32_t* misc, uint32_t (&grun)[8])
 {
@@ -179,7 +179,7 @@ __device__ __forceinline__ uint32_t finish_ranks(uint16_t* cnt, uint32_t B, uint
     if (b0 < Bp) {
         uint4 run = make_uint4(0, 0, 0, 0);  // 8 packed uint16 running sums (no carry: a tile has <= 1024 records)
 #pragma unroll
-        for (int w = 0; w < kWarps; ++w) {
+        for (int w = 0; w < NW; ++w) {
             uint4* p = reinterpret_cast<uint4*>(cnt + w * Bp + b0);
             uint4 c = *p;
             *p = run;
@@ -191,7 +191,17 @@ __device__ __forceinline__ uint32_t finish_ranks(uint16_t* cnt, uint32_t B, uint
         for (int k = 0; k < 8; ++k) mine += t8[k];
     }
     uint32_t total = 0, ex = 0;
-    if (STAGED) ex = block_excl_scan(mine, misc, &total);
+    if (STAGED) {
+        if (Bp <= 256) {  // every bucket belongs to a thread of warp 0: a warp scan, no barrier
+            if (warp_id() == 0) {
+                uint32_t inc = warp_incl_scan(mine);
+                ex = inc - mine;
+                if (lane_id() == 31) misc[32] = inc;
+            }
+        } else {
+            ex = block_excl_scan(mine, misc, &total);
+        }
+    }
     if (b0 < Bp) {
 #pragma unroll
         for (int k = 0; k < 8; ++k) {
@@ -204,6 +214,7 @@ __device__ __forceinline__ uint32_t finish_ranks(uint16_t* cnt, uint32_t B, uint
         }
     }
     __syncthreads();
+    if (STAGED && Bp <= 256) total = misc[32];
     return total;
 }
 
