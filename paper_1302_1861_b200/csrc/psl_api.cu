@@ -15,6 +15,7 @@
 
 #include "psl_beam.cuh"
 #include "psl_bigtile.cuh"
+#include "psl_index.cuh"
 #include "psl_device.cuh"
 #include "psl_partition.cuh"
 
@@ -33,7 +34,7 @@ struct Layout {
     // ONTHEFLY
     uint64_t table = 0, out[10] = {0}, offsets = 0, counts = 0;
     // INDEX
-    uint64_t table_a = 0, table_b = 0, aos = 0, hi16 = 0, idx[7] = {0}, keyfull = 0, idx_offsets = 0, idx_counts = 0,
+    uint64_t table_a = 0, table_b = 0, aos = 0, idx[7] = {0}, keyfull = 0, idx_offsets = 0, idx_counts = 0,
              idx_batch_off = 0;
     uint64_t seg = 0, beam_out[10] = {0}, beam_keys = 0, beam_offsets = 0, beam_counts = 0, lookback = 0, bstats = 0,
              beam_stats = 0;
@@ -118,11 +119,10 @@ psl_status derive(const psl_config* c, Derived* d, char* err)
     if (c->mode == PSL_MODE_ONTHEFLY) {
         if (K > kMaxBuckets) { set_err(err, "ONTHEFLY mode handles at most %d keys (got %llu); use PSL_MODE_INDEX", kMaxBuckets, (unsigned long long)K); return PSL_ERR_ARG; }
     } else {
-        if (K > (uint64_t)kMaxBuckets * kMaxBuckets) { set_err(err, "INDEX mode handles at most %d keys", kMaxBuckets * kMaxBuckets); return PSL_ERR_ARG; }
-        uint32_t bits = 0;
-        while ((1ull << bits) < K) ++bits;  // K <= 2^bits
-        uint32_t lo = bits / 2;  // the smaller digit goes to pass A (its counters are the larger share of its shared memory)
-        while ((((K - 1) >> lo) + 1) > (uint64_t)kMaxBuckets) ++lo;
+        if (K > (uint64_t)kIdxMaxHi * kIdxMaxLo) { set_err(err, "INDEX mode handles at most %d keys", kIdxMaxHi * kIdxMaxLo); return PSL_ERR_ARG; }
+        // key = hi * 2^lo_bits + lo: pass B wants few buckets (<= 256, long output runs), pass A takes the rest
+        uint32_t lo = 0;
+        while ((((K - 1) >> lo) + 1) > (uint64_t)kIdxMaxHi) ++lo;
         d->lo_bits = lo;
         d->B_lo = (uint32_t)((K < (1ull << lo)) ? K : (1ull << lo));
         if (d->B_lo < 1) d->B_lo = 1;
@@ -171,7 +171,6 @@ void plan(const psl_config* c, const Derived& d, Layout* L)
         L->table_a = take(&cur, (uint64_t)d.B_lo * d.cols_cap * 4);
         L->table_b = take(&cur, (uint64_t)d.B_hi * kMaxSegments * 4);
         L->aos = take(&cur, N * 32);
-        L->hi16 = take(&cur, N * 2);
         for (int i = 0; i < 7; ++i) L->idx[i] = take(&cur, N * 4);
         L->keyfull = take(&cur, N * 4);
         L->idx_offsets = take(&cur, (uint64_t)(d.K + 1) * 4);
@@ -195,7 +194,7 @@ enum ResultKind { RES_NONE = 0, RES_OTF = 1, RES_INDEX = 2, RES_BEAM = 3 };
 // ---- kernel variants: the features a configuration / beam does not use are compiled out ------------------
 using CountFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, uint32_t, uint32_t*, uint32_t, SegStats*);
 using ScatterOtfFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, const uint32_t*, uint32_t, SoAOut, SegStats*);
-using ScatterIdxAFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, uint32_t, const uint32_t*, uint32_t, uint4*, uint16_t*);
+using ScatterIdxAFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, uint32_t, const uint32_t*, uint32_t, uint4*);
 
 template <bool POS, bool EDGES>
 CountFn count_otf_pe(int beam)
@@ -569,14 +568,13 @@ psl_status finalize_index(psl_ctx* ctx)
         uint32_t* table_a = at<uint32_t>(ctx, L.table_a);
         uint32_t* table_b = at<uint32_t>(ctx, L.table_b);
         uint4* aos = at<uint4>(ctx, L.aos);
-        uint16_t* hi16 = at<uint16_t>(ctx, L.hi16);
         psl_status s = run_scan(ctx, table_a, d.B_lo, ctx->n_cols, d.cols_cap, scalar(ctx, SC_NIDX));
         if (s != PSL_OK) return s;
         {
             Prof prof(ctx, PSL_K_INDEX_A);
             for (const psl_ctx::ChunkLaunch& cl : ctx->idx_launches) {  // the same segments the counts were taken on
                 scatter_idx_a_fn(ctx->grid.has_pos != 0, ctx->grid.ebin_mode != 0)<<<cl.n_seg, kThreads, ctx->sm_idx_a, ctx->stream>>>(
-                    chunks, ctx->n_chunks, cl.span, ctx->grid, none, d.B_lo, d.lo_bits, table_a, d.cols_cap, aos, hi16);
+                    chunks, ctx->n_chunks, cl.span, ctx->grid, none, d.B_lo, d.lo_bits, table_a, d.cols_cap, aos);
                 LAUNCHED();
             }
         }
@@ -585,14 +583,14 @@ psl_status finalize_index(psl_ctx* ctx)
         const uint32_t Sb = ntb < ctx->S_b ? ntb : ctx->S_b;
         {
             Prof prof(ctx, PSL_K_COUNT);
-            k_count_hi16<<<Sb, kThreads, ctx->sm_count_b, ctx->stream>>>(hi16, scalar(ctx, SC_NIDX), d.B_hi, table_b, kMaxSegments);
+            k_count_keys<<<Sb, kThreads, ctx->sm_count_b, ctx->stream>>>(aos, scalar(ctx, SC_NIDX), d.B_hi, d.lo_bits, table_b, kMaxSegments);
             LAUNCHED();
         }
         s = run_scan(ctx, table_b, d.B_hi, Sb, kMaxSegments, scalar(ctx, SC_TOTAL));
         if (s != PSL_OK) return s;
         {
             Prof prof(ctx, PSL_K_INDEX_B);
-            k_scatter_idx_b<<<Sb, kThreads, ctx->sm_idx_b, ctx->stream>>>(aos, scalar(ctx, SC_NIDX), d.B_hi, d.lo_bits, table_b,
+            k_scatter_idx_b<<<Sb, kBigThreads, ctx->sm_idx_b, ctx->stream>>>(aos, scalar(ctx, SC_NIDX), d.B_hi, d.lo_bits, table_b,
                                                                          kMaxSegments, idx_out(ctx));
             LAUNCHED();
         }
@@ -862,18 +860,18 @@ psl_status psl_create(const psl_config* cfg, psl_ctx** out)
         ctx->S_otf = width(occ);
     } else {
         ctx->sm_count_raw = count_layout(kTile * kRecBytes, kStagesCount, d.B_lo, ne).total;
-        ctx->sm_idx_a = part_layout(kTile * kRecBytes, kStagesRaw, d.B_lo, ne, false).total;
+        ctx->sm_idx_a = idx_a_layout(d.B_lo, ne).total;
         ctx->sm_count_b = count_layout(0, 0, d.B_hi, 0).total;
-        ctx->sm_idx_b = part_layout(kTile * 32, kStagesKeyed, d.B_hi, 0, true).total;
+        ctx->sm_idx_b = idx_b_layout(d.B_hi).total;
         const bool pos = d.n_pos > 1, edges = cfg->ebin_mode == PSL_EBIN_EDGES;
         CUC(allow_smem(count_idx_fn(pos, edges), ctx->sm_count_raw));
         CUC(allow_smem(scatter_idx_a_fn(pos, edges), ctx->sm_idx_a));
-        CUC(allow_smem(k_count_hi16, ctx->sm_count_b));
+        CUC(allow_smem(k_count_keys, ctx->sm_count_b));
         CUC(allow_smem(k_scatter_idx_b, ctx->sm_idx_b));
         CUC(allow_smem(k_beam_compact, 11 * kBeamTile * 4));
         CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, scatter_idx_a_fn(pos, edges), kThreads, ctx->sm_idx_a));
         ctx->S_a = width(occ);
-        CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_scatter_idx_b, kThreads, ctx->sm_idx_b));
+        CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_scatter_idx_b, kBigThreads, ctx->sm_idx_b));
         ctx->S_b = width(occ);
     }
     CUC(cudaStreamSynchronize(ctx->stream));

@@ -30,7 +30,6 @@ constexpr int kScanBlock = kScanThreads * kScanRows;  // 4096 table entries per 
 
 constexpr int kStagesCount = 3;   // ring depth of the histogram kernels (28 KB stages)
 constexpr int kStagesRaw = 3;     // ring depth of the scatter kernels that read raw records
-constexpr int kStagesKeyed = 2;   // ring depth of INDEX pass B (32 KB stages)
 constexpr int kHistBytes = 16384; // privatised histogram budget of the histogram kernels
 
 struct SoAOut {
@@ -597,97 +596,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_scatter_otf(const ChunkDesc* __
     }
 }
 
-// ------------------------------------------------------------------------------------------------------
-// INDEX pass A: raw records -> 32-byte keyed records {key, E, x, y, u, v, wt, src}, stably partitioned by
-// the low digit of the key.  One record = one full 32-byte sector, written by its own thread (no staging).
-// Also writes the high digit of every record (uint16) to hi16[] in the new order, which is all pass B's
-// count needs to read.
-// ------------------------------------------------------------------------------------------------------
-template <bool POS, bool EDGES>
-__global__ void __launch_bounds__(kThreads, 2) k_scatter_idx_a(const ChunkDesc* __restrict__ chunks, uint32_t n_chunks,
-                                                              Span sp, const __grid_constant__ DevGrid g,
-                                                              const __grid_constant__ DevBeam bm, uint32_t B,
-                                                              uint32_t lo_bits, const uint32_t* __restrict__ table,
-                                                              uint32_t stride, uint4* __restrict__ aos,
-                                                              uint16_t* __restrict__ hi16)
-{
-    extern __shared__ __align__(128) uint8_t smem[];
-    const uint32_t Bp = round_up(B, 8);
-    const PartSmem L = part_layout(kTile * kRecBytes, kStagesRaw, B, g.n_ebins + 1, false);
-    uint16_t* cnt = reinterpret_cast<uint16_t*>(smem + L.cnt);
-    uint32_t* gcur = reinterpret_cast<uint32_t*>(smem + L.gcur);
-    float* s_edges = reinterpret_cast<float*>(smem + L.edges);
-    uint32_t* misc = reinterpret_cast<uint32_t*>(smem + L.misc);
-    TileDesc* s_desc = reinterpret_cast<TileDesc*>(smem + L.desc);
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + L.bars);
-    const uint32_t w = warp_id();
-    const uint32_t lo_mask = (1u << lo_bits) - 1u;
-
-    uint32_t t0, t1;
-    segment_of(sp, t0, t1);
-    const uint32_t n = t1 - t0;
-    uint32_t grun[8];
-    auto desc_of = [&](uint32_t t) { return raw_tile(chunks, n_chunks, t); };
-    scatter_prologue<kStagesRaw>(smem, L, B, Bp, n, t0, kRecBytes, desc_of, table, stride, sp.col0 + blockIdx.x, grun);
-    stage_edges(g, s_edges);
-    __syncthreads();
-
-    uint32_t phase_bits = 0;
-    for (uint32_t i = 0; i < n; ++i) {
-        const uint32_t stage = i % kStagesRaw;
-        uint32_t* raw = reinterpret_cast<uint32_t*>(smem + L.ring + stage * L.stage_bytes);
-        const TileDesc td = s_desc[stage];
-        ring_acquire(raw, &bars[stage], phase_bits, stage, td.ptr, td.count * kRecBytes);
-
-        uint32_t packed[kRounds];  // key << 9 | rank   (key < 2^22)
-        {
-            Rec rec[kRounds];
-#pragma unroll
-            for (int r = 0; r < kRounds; ++r) {
-                int idx = w * kWarpSpan + r * 32 + lane_id();
-                rec[r] = rec_from_smem(raw, idx < (int)td.count ? idx : 0);
-            }
-#pragma unroll
-            for (int r = 0; r < kRounds; ++r) {
-                int idx = w * kWarpSpan + r * 32 + lane_id();
-                uint32_t key;
-                int cls = classify<POS, EDGES, 0>(g, bm, rec[r], s_edges, key);
-                packed[r] = (idx < (int)td.count && cls == C_SURVIVOR) ? key : kNone;
-            }
-#pragma unroll
-            for (int r = 0; r < kRounds; ++r) {
-                uint32_t key = packed[r];
-                uint32_t rank = warp_rank(key == kNone ? kNone : (key & lo_mask), cnt + w * Bp);
-                packed[r] = key == kNone ? kNone : ((key << 9) | rank);
-            }
-        }
-        __syncthreads();
-        finish_ranks<false>(cnt, B, Bp, gcur, nullptr, misc, grun);
-
-#pragma unroll
-        for (int r = 0; r < kRounds; ++r) {
-            if (packed[r] != kNone) {
-                uint32_t key = packed[r] >> 9, rank = packed[r] & 511u, bucket = key & lo_mask;
-                uint32_t dest = gcur[bucket] + cnt[w * Bp + bucket] + rank;
-                int idx = w * kWarpSpan + r * 32 + lane_id();
-                const uint32_t* p = raw + idx * kRecWords;
-                aos[2 * (size_t)dest + 0] = make_uint4(key, p[1], p[2], p[3]);
-                aos[2 * (size_t)dest + 1] = make_uint4(p[4], p[5], p[6], td.first_index + idx);
-                hi16[dest] = (uint16_t)(key >> lo_bits);
-            }
-        }
-        __syncwarp();
-        zero_row(cnt + w * Bp, Bp);
-        __syncthreads();  // the stage is free again
-        if (threadIdx.x == 0 && i + kStagesRaw < n) {
-            TileDesc d = raw_tile(chunks, n_chunks, t0 + i + kStagesRaw);
-            s_desc[stage] = d;
-            ring_issue(raw, &bars[stage], d.ptr, d.count * kRecBytes);
-        }
-    }
-}
-
-// tiles of the pass-A output: n = *n_ptr keyed records, contiguous
+// tiles of the pass-A output: n keyed records (32 bytes each), contiguous
 __device__ __forceinline__ TileDesc keyed_tile(const uint4* aos, uint32_t n, uint32_t t)
 {
     TileDesc d;
@@ -695,131 +604,6 @@ __device__ __forceinline__ TileDesc keyed_tile(const uint4* aos, uint32_t n, uin
     d.first_index = t * kTile;
     d.count = min((uint32_t)kTile, n - t * (uint32_t)kTile);
     return d;
-}
-
-// INDEX pass B count: histogram of the uint16 high digits over the CTA's segment of the pass-A output.
-__global__ void __launch_bounds__(kThreads) k_count_hi16(const uint16_t* __restrict__ hi16,
-                                                        const uint32_t* __restrict__ n_ptr, uint32_t B,
-                                                        uint32_t* __restrict__ table, uint32_t stride)
-{
-    extern __shared__ __align__(128) uint8_t smem[];
-    uint32_t* hist = reinterpret_cast<uint32_t*>(smem);
-    const CountSmem L = count_layout(0, 0, B, 0);
-    const uint32_t rmask = (1u << L.rlog) - 1u;
-    const uint32_t n = *n_ptr;
-    Span sp = {0u, (n + kTile - 1) / kTile, 0u};
-    uint32_t t0, t1;
-    segment_of(sp, t0, t1);
-    for (uint32_t i = threadIdx.x; i < (B << L.rlog); i += kThreads) hist[i] = 0;
-    __syncthreads();
-    // 8 digits per 16-byte load; the segment starts on a tile boundary, so the loads are aligned
-    const uint32_t first = t0 * kTile, last = min(n, t1 * (uint32_t)kTile);
-    const uint4* v = reinterpret_cast<const uint4*>(hi16 + first);
-    const uint32_t n8 = (last - first) / 8;
-    for (uint32_t i = threadIdx.x; i < n8; i += kThreads) {
-        uint4 d = __ldg(v + i);
-        uint32_t wds[4] = {d.x, d.y, d.z, d.w};
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            atomicAdd(&hist[((wds[k] & 0xFFFFu) << L.rlog) + (lane_id() & rmask)], 1u);
-            atomicAdd(&hist[((wds[k] >> 16) << L.rlog) + (lane_id() & rmask)], 1u);
-        }
-    }
-    for (uint32_t i = first + n8 * 8 + threadIdx.x; i < last; i += kThreads)
-        atomicAdd(&hist[((uint32_t)hi16[i] << L.rlog) + (lane_id() & rmask)], 1u);
-    __syncthreads();
-    for (uint32_t b = threadIdx.x; b < B; b += kThreads) {
-        uint32_t c = 0;
-        for (uint32_t r = 0; r <= rmask; ++r) c += hist[(b << L.rlog) + ((r + lane_id()) & rmask)];
-        table[(size_t)b * stride + blockIdx.x] = c;
-    }
-}
-
-// ------------------------------------------------------------------------------------------------------
-// INDEX pass B scatter: keyed records (sorted by low digit) -> SoA index sorted by the full key, plus the
-// full key of every slot (used once, by binary search, to build offsets[K+1]).
-// ------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kThreads, 2) k_scatter_idx_b(const uint4* __restrict__ aos,
-                                                              const uint32_t* __restrict__ n_ptr, uint32_t B,
-                                                              uint32_t lo_bits, const uint32_t* __restrict__ table,
-                                                              uint32_t stride, IdxOut out)
-{
-    extern __shared__ __align__(128) uint8_t smem[];
-    const uint32_t Bp = round_up(B, 8);
-    const PartSmem L = part_layout(kTile * 32, kStagesKeyed, B, 0, true);
-    uint16_t* cnt = reinterpret_cast<uint16_t*>(smem + L.cnt);
-    uint32_t* gcur = reinterpret_cast<uint32_t*>(smem + L.gcur);
-    uint32_t* lstart = reinterpret_cast<uint32_t*>(smem + L.lstart);
-    uint32_t* pdest = reinterpret_cast<uint32_t*>(smem + L.pdest);
-    uint16_t* perm = reinterpret_cast<uint16_t*>(smem + L.perm);
-    uint32_t* misc = reinterpret_cast<uint32_t*>(smem + L.misc);
-    TileDesc* s_desc = reinterpret_cast<TileDesc*>(smem + L.desc);
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + L.bars);
-    const uint32_t w = warp_id();
-    const uint32_t n_rec = *n_ptr;
-
-    Span sp = {0u, (n_rec + kTile - 1) / kTile, 0u};
-    uint32_t t0, t1;
-    segment_of(sp, t0, t1);
-    const uint32_t n = t1 - t0;
-    uint32_t grun[8];
-    auto desc_of = [&](uint32_t t) { return keyed_tile(aos, n_rec, t); };
-    scatter_prologue<kStagesKeyed>(smem, L, B, Bp, n, t0, 32u, desc_of, table, stride, blockIdx.x, grun);
-    __syncthreads();
-
-    uint32_t phase_bits = 0;
-    for (uint32_t i = 0; i < n; ++i) {
-        const uint32_t stage = i % kStagesKeyed;
-        uint32_t* raw = reinterpret_cast<uint32_t*>(smem + L.ring + stage * L.stage_bytes);
-        const TileDesc td = s_desc[stage];
-        ring_acquire(raw, &bars[stage], phase_bits, stage, td.ptr, td.count * 32u);
-
-        uint32_t packed[kRounds];
-#pragma unroll
-        for (int r = 0; r < kRounds; ++r) {
-            uint32_t idx = w * kWarpSpan + r * 32 + lane_id();
-            uint32_t bucket = idx < td.count ? (raw[idx * 8] >> lo_bits) : kNone;
-            uint32_t rank = warp_rank(bucket, cnt + w * Bp);
-            packed[r] = bucket == kNone ? kNone : ((bucket << 9) | rank);
-        }
-        __syncthreads();
-        const uint32_t n_part = finish_ranks<true>(cnt, B, Bp, gcur, lstart, misc, grun);
-
-#pragma unroll
-        for (int r = 0; r < kRounds; ++r) {
-            if (packed[r] != kNone) {
-                uint32_t bucket = packed[r] >> 9, rank = packed[r] & 511u;
-                uint32_t rel = cnt[w * Bp + bucket] + rank;
-                uint32_t p = lstart[bucket] + rel;
-                perm[p] = (uint16_t)(w * kWarpSpan + r * 32 + lane_id());
-                pdest[p] = gcur[bucket] + rel;
-            }
-        }
-        __syncwarp();
-        zero_row(cnt + w * Bp, Bp);
-        __syncthreads();
-
-        const uint4* s_rec = reinterpret_cast<const uint4*>(raw);
-        for (uint32_t j = threadIdx.x; j < n_part; j += kThreads) {
-            const uint32_t irec = perm[j];
-            const uint32_t dest = pdest[j];
-            uint4 a = s_rec[2 * irec + 0], b = s_rec[2 * irec + 1];
-            out.key[dest] = a.x;
-            out.E[dest] = __uint_as_float(a.y);
-            out.x[dest] = __uint_as_float(a.z);
-            out.y[dest] = __uint_as_float(a.w);
-            out.u[dest] = __uint_as_float(b.x);
-            out.v[dest] = __uint_as_float(b.y);
-            out.wt[dest] = __uint_as_float(b.z);
-            out.src[dest] = b.w;
-        }
-        __syncthreads();
-        if (threadIdx.x == 0 && i + kStagesKeyed < n) {
-            TileDesc d = keyed_tile(aos, n_rec, t0 + i + kStagesKeyed);
-            s_desc[stage] = d;
-            ring_issue(raw, &bars[stage], d.ptr, d.count * 32u);
-        }
-    }
 }
 
 // offsets[k] = number of sorted slots whose key is < k (binary search; k = 0..K).  keys[0..n) ascending.
