@@ -206,15 +206,19 @@ def run_reference(args):
 # ------------------------------------------------------------------------------------------------------
 # the CUDA arm
 # ------------------------------------------------------------------------------------------------------
-def algorithmic_bytes(cls, n, n_idx, m_sel, n_surv_beams, proj):
+def algorithmic_bytes(cls, n, n_idx, m_sel, n_surv_beams, proj, index_mode=False):
     """algorithmic bytes one step's launches of kernel class `cls` must move"""
     out_b = SOA_BYTES + (8 if proj else 0)
     if cls == "count":
-        return RECORD_BYTES * n                       # one read of every packed record
+        # one read of every packed record; INDEX mode adds pass B's histogram, which reads the 4-byte key of every
+        # keyed record
+        return RECORD_BYTES * n + (4 * n_idx if index_mode else 0)
     if cls == "scatter":
         return RECORD_BYTES * n + out_b * n_surv_beams  # read every record, write the survivors' SoA
-    if cls in ("index_a", "index_b"):
-        return RECORD_BYTES * (n if cls == "index_a" else n_idx) + RECORD_BYTES * n_idx  # the record moves once per pass
+    if cls == "index_a":
+        return RECORD_BYTES * n + 32 * n_idx          # packed records in, 32-byte keyed records out
+    if cls == "index_b":
+        return 32 * n_idx + 32 * n_idx                # keyed records in, 7 SoA arrays + the key per slot out
     if cls == "beam":
         return RECORD_BYTES * m_sel + out_b * n_surv_beams  # only the ROI-selected bins are read
     return 0
@@ -244,7 +248,7 @@ def run_ours(args):
 
     # inputs: generated once into pinned host memory (the e2e source), copied once to the device (the resident source)
     host = torch.empty(n * RECORD_BYTES, dtype=torch.uint8).pin_memory()
-    W.generate_into(w.gen, first_record, n, host.data_ptr())
+    W.generate_into(w.gen, first_record, n, host.data_ptr(), threads=os.cpu_count() or 1)
     resident = host.to(dev)
     host_chunks = [host[f * RECORD_BYTES:(f + c) * RECORD_BYTES] for f, c in chunks]
     dev_chunks = [resident[f * RECORD_BYTES:(f + c) * RECORD_BYTES] for f, c in chunks]
@@ -327,6 +331,18 @@ def run_ours(args):
     # INDEX mode adds the one-off offsets[K+1] copy that drives the ROI segment list
     d2h_bytes = len(beams) * ((2 * K + 1) * 4 + (n_batches + 1) * 4 + 64) + ((K + 1) * 4 if w.mode == 1 else 0)
     if not args.no_e2e:
+        # the host-link ceiling, measured here: plain pinned cudaMemcpyAsync of the same chunks into one device buffer
+        land = torch.empty(max(c for _, c in chunks) * RECORD_BYTES, dtype=torch.uint8, device=dev)
+        for rep_ in range(2):
+            torch.cuda.synchronize()
+            c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            c0.record()
+            for hc in host_chunks:
+                land[:hc.numel()].copy_(hc, non_blocking=True)
+            c1.record()
+            torch.cuda.synchronize()
+            h2d_peak = n * RECORD_BYTES / (c0.elapsed_time(c1) * 1e-3) / 1e9
+        del land
         for _ in range(3):
             step(host_chunks, True)
         e2e_steps = max(3, min(args.steps, 10 if n > 50_000_000 else args.steps))
@@ -336,6 +352,8 @@ def run_ours(args):
                "d2h_bytes_per_step": d2h_bytes,
                "steps": e2e_steps, "ms_per_step": ms_e / e2e_steps,
                "h2d_gbs": n * RECORD_BYTES * e2e_steps / (ms_e * 1e-3) / 1e9,
+               "h2d_peak_gbs": h2d_peak,  # plain pinned copies of the same chunks, same run
+               "h2d_frac": n * RECORD_BYTES * e2e_steps / (ms_e * 1e-3) / 1e9 / h2d_peak,
                "source": "pinned host memory, %d chunk(s) per step through psl_load_chunk(PSL_MEM_PINNED)" % len(chunks)}
     clocks = sampler.finish()
 
@@ -348,7 +366,7 @@ def run_ours(args):
             if brackets:
                 kernels[cls] = {"ms_per_step": tot_ms / args.steps, "launches_per_step": brackets / args.steps}
             continue
-        per_step_bytes = algorithmic_bytes(cls, n, n_idx, m_sel_all, surv_all, proj)
+        per_step_bytes = algorithmic_bytes(cls, n, n_idx, m_sel_all, surv_all, proj, w.mode == 1)
         kernels[cls] = {"ms_per_step": tot_ms / args.steps, "launches_per_step": brackets / args.steps,
                         "avg_launch_ms": tot_ms / brackets,
                         "algorithmic_bytes_per_step": per_step_bytes,

@@ -192,7 +192,7 @@ void plan(const psl_config* c, const Derived& d, Layout* L)
 enum ResultKind { RES_NONE = 0, RES_OTF = 1, RES_INDEX = 2, RES_BEAM = 3 };
 
 // ---- kernel variants: the features a configuration / beam does not use are compiled out ------------------
-using CountFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, uint32_t, uint32_t*, uint32_t, SegStats*);
+using CountFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, uint32_t, uint32_t*, uint32_t, SegStats*, uint32_t);
 using ScatterOtfFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, const uint32_t*, uint32_t, SoAOut, SegStats*);
 using ScatterIdxAFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, uint32_t, const uint32_t*, uint32_t, uint4*);
 
@@ -272,6 +272,7 @@ struct psl_ctx {
     // launch shapes: persistent CTAs per launch (= SMs x resident CTAs of the scatter kernel, one wave)
     uint32_t S_otf = 0, S_a = 0, S_b = 0;
     bool big_tiles = false;  // ONTHEFLY with few keys: the 4096-record-tile scatter
+    uint32_t count_stages = kStagesCount, count_split = 1;
     uint32_t sm_count_raw = 0, sm_scatter_otf = 0, sm_idx_a = 0, sm_count_b = 0, sm_idx_b = 0;  // dynamic smem bytes
     struct ChunkLaunch { Span span; uint32_t n_seg; };
     std::vector<ChunkLaunch> idx_launches;  // INDEX: the per-chunk count launches, replayed by pass A's scatter
@@ -499,16 +500,17 @@ psl_status build_onthefly(psl_ctx* ctx, const DevBeam& bm)
         const ChunkDesc* chunks = at<ChunkDesc>(ctx, L.chunks);
         SegStats* ss = at<SegStats>(ctx, L.sstats);
         const uint32_t S = nt < ctx->S_otf ? nt : ctx->S_otf;  // one persistent CTA per segment, one wave
-        const Span span = {0u, nt, 0u};
+        const Span span = {0u, nt, 0u, ctx->count_split};
+        const uint32_t n_cols = S * ctx->count_split;
         const bool pos = ctx->grid.has_pos != 0, edges = ctx->grid.ebin_mode != 0, proj = bm.has_map || bm.out_proj;
         const int bv = beam_variant(bm);
         {
             Prof prof(ctx, PSL_K_COUNT);
-            count_otf_fn(pos, edges, bv)<<<S, kThreads, ctx->sm_count_raw, ctx->stream>>>(chunks, ctx->n_chunks, span, ctx->grid, bm, d.K, 0,
-                                                                                        table, d.cols_cap, ss);
+            count_otf_fn(pos, edges, bv)<<<n_cols, kThreads, ctx->sm_count_raw, ctx->stream>>>(chunks, ctx->n_chunks, span, ctx->grid, bm, d.K, 0,
+                                                                                             table, d.cols_cap, ss, ctx->count_stages);
             LAUNCHED();
         }
-        psl_status s = run_scan(ctx, table, d.K, S, d.cols_cap, scalar(ctx, SC_TOTAL));
+        psl_status s = run_scan(ctx, table, d.K, n_cols, d.cols_cap, scalar(ctx, SC_TOTAL));
         if (s != PSL_OK) return s;
         k_offsets_from_table<<<(d.K + 1 + 255) / 256, 256, 0, ctx->stream>>>(table, d.cols_cap, d.K, scalar(ctx, SC_TOTAL),
                                                                            offsets, counts, d.n_pos, d.n_batches, batch_off);
@@ -523,7 +525,7 @@ psl_status build_onthefly(psl_ctx* ctx, const DevBeam& bm)
                                                                                                        d.K, table, d.cols_cap, soa_out(ctx, L.out), ss);
             LAUNCHED();
         }
-        k_reduce_stats<<<1, 1024, 0, ctx->stream>>>(ss, S, stats);
+        k_reduce_stats<<<1, 1024, 0, ctx->stream>>>(ss, n_cols, stats);
         LAUNCHED();
     }
     CU(cudaMemcpyAsync(ctx->h_batch_off, batch_off, (uint64_t)(d.n_batches + 1) * 4, cudaMemcpyDeviceToHost, ctx->stream));
@@ -843,7 +845,8 @@ psl_status psl_create(const psl_config* cfg, psl_ctx** out)
     };
     int occ = 0;
     if (cfg->mode == PSL_MODE_ONTHEFLY) {
-        ctx->sm_count_raw = count_layout(kTile * kRecBytes, kStagesCount, d.K, ne).total;
+        ctx->count_stages = d.K * 4 > 8192 ? 2 : kStagesCount;
+        ctx->sm_count_raw = count_layout(kTile * kRecBytes, ctx->count_stages, d.K, ne).total;
         ctx->big_tiles = round_up(d.K, 8) <= (uint32_t)kBigMaxKeys;
         ctx->sm_scatter_otf = ctx->big_tiles ? big_layout(d.K, ne).total : part_layout(kTile * kRecBytes, kStagesRaw, d.K, ne, true).total;
         const bool pos = d.n_pos > 1, edges = cfg->ebin_mode == PSL_EBIN_EDGES;
@@ -858,8 +861,10 @@ psl_status psl_create(const psl_config* cfg, psl_ctx** out)
         else
             CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, scatter_otf_fn(pos, edges, 2, true), kThreads, ctx->sm_scatter_otf));
         ctx->S_otf = width(occ);
+        ctx->count_split = ctx->big_tiles ? 2 : 1;  // one scatter CTA per SM, two histogram CTAs
     } else {
-        ctx->sm_count_raw = count_layout(kTile * kRecBytes, kStagesCount, d.B_lo, ne).total;
+        ctx->count_stages = d.B_lo * 4 > 8192 ? 2 : kStagesCount;
+        ctx->sm_count_raw = count_layout(kTile * kRecBytes, ctx->count_stages, d.B_lo, ne).total;
         ctx->sm_idx_a = idx_a_layout(d.B_lo, ne).total;
         ctx->sm_count_b = count_layout(0, 0, d.B_hi, 0).total;
         ctx->sm_idx_b = idx_b_layout(d.B_hi).total;
@@ -963,13 +968,13 @@ psl_status psl_load_chunk(psl_ctx* ctx, const void* records, uint64_t n, int32_t
         DevBeam none;
         memset(&none, 0, sizeof none);
         psl_ctx::ChunkLaunch cl;
-        cl.span = {tile0, nt, ctx->n_cols};
+        cl.span = {tile0, nt, ctx->n_cols, 1u};
         cl.n_seg = nt < ctx->S_a ? nt : ctx->S_a;
         if (ctx->n_cols + cl.n_seg > ctx->d.cols_cap) { set_err(ctx->err, "load_chunk: out of table columns"); return PSL_ERR_CAPACITY; }
         Prof prof(ctx, PSL_K_COUNT);
         count_idx_fn(ctx->grid.has_pos != 0, ctx->grid.ebin_mode != 0)<<<cl.n_seg, kThreads, ctx->sm_count_raw, ctx->stream>>>(
             chunks, ctx->n_chunks + 1, cl.span, ctx->grid, none, ctx->d.B_lo, (1u << ctx->d.lo_bits) - 1u,
-            at<uint32_t>(ctx, ctx->L.table_a), ctx->d.cols_cap, at<SegStats>(ctx, ctx->L.sstats));
+            at<uint32_t>(ctx, ctx->L.table_a), ctx->d.cols_cap, at<SegStats>(ctx, ctx->L.sstats), ctx->count_stages);
         LAUNCHED();
         ctx->idx_launches.push_back(cl);
         ctx->n_cols += cl.n_seg;

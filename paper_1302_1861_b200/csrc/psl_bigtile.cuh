@@ -73,7 +73,7 @@ __global__ void __launch_bounds__(kBigThreads, 1) k_scatter_otf_big(const ChunkD
     TileDesc* s_desc = reinterpret_cast<TileDesc*>(smem + L.desc);
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + L.bars);
     const uint32_t w = warp_id();
-    const uint32_t col = sp.col0 + blockIdx.x;
+    const uint32_t col = sp.col0 + blockIdx.x * sp.split;
 
     uint32_t t0, t1;
     segment_of(sp, t0, t1);

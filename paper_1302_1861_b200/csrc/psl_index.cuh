@@ -57,7 +57,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_scatter_idx_a(const ChunkDesc* 
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + L.bars);
     const uint32_t w = warp_id();
     const uint32_t lo_mask = (1u << lo_bits) - 1u;
-    const uint32_t col = sp.col0 + blockIdx.x;
+    const uint32_t col = sp.col0 + blockIdx.x * sp.split;
 
     uint32_t t0, t1;
     segment_of(sp, t0, t1);
@@ -153,7 +153,7 @@ __global__ void __launch_bounds__(kThreads) k_count_keys(const uint4* __restrict
     const CountSmem L = count_layout(0, 0, B, 0);
     const uint32_t rmask = (1u << L.rlog) - 1u;
     const uint32_t n = *n_ptr;
-    Span sp = {0u, (n + kTile - 1) / kTile, 0u};
+    Span sp = {0u, (n + kTile - 1) / kTile, 0u, 1u};
     uint32_t t0, t1;
     segment_of(sp, t0, t1);
     for (uint32_t i = threadIdx.x; i < (B << L.rlog); i += kThreads) hist[i] = 0;
@@ -218,7 +218,7 @@ __global__ void __launch_bounds__(kBigThreads, 1) k_scatter_idx_b(const uint4* _
     const uint32_t w = warp_id();
     const uint32_t n_rec = *n_ptr;
 
-    Span sp = {0u, (n_rec + kTile - 1) / kTile, 0u};
+    Span sp = {0u, (n_rec + kTile - 1) / kTile, 0u, 1u};
     uint32_t t0, t1;
     segment_of(sp, t0, t1);
     const uint32_t n = t1 - t0;

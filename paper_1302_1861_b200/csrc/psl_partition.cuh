@@ -28,7 +28,7 @@ constexpr int kScanThreads = 256;
 constexpr int kScanRows = 16;
 constexpr int kScanBlock = kScanThreads * kScanRows;  // 4096 table entries per scan CTA
 
-constexpr int kStagesCount = 3;   // ring depth of the histogram kernels (28 KB stages)
+constexpr int kStagesCount = 3;   // ring depth of the histogram kernels (28 KB stages; 2 when the histogram is large)
 constexpr int kStagesRaw = 3;     // ring depth of the scatter kernels that read raw records
 constexpr int kHistBytes = 16384; // privatised histogram budget of the histogram kernels
 
@@ -45,8 +45,10 @@ struct IdxOut {
 
 // which tiles a launch covers and which table columns its CTAs own: CTA s of the launch (gridDim.x CTAs)
 // takes tiles tile_begin + [s*n_tiles/S, (s+1)*n_tiles/S) and column col0 + s.
+// The histogram kernel may run `split` CTAs per segment (each on a contiguous part of it, with a table column
+// of its own: gridDim.x = S * split); the scatter CTA of segment s then starts from column col0 + s * split.
 struct Span {
-    uint32_t tile_begin, n_tiles, col0;
+    uint32_t tile_begin, n_tiles, col0, split;
 };
 
 __host__ __device__ inline uint32_t round_up(uint32_t a, uint32_t m) { return (a + m - 1) / m * m; }
@@ -131,6 +133,15 @@ __device__ __forceinline__ void segment_of(const Span& sp, uint32_t& t0, uint32_
     const unsigned long long n = sp.n_tiles, S = gridDim.x, s = blockIdx.x;
     t0 = sp.tile_begin + (uint32_t)(n * s / S);
     t1 = sp.tile_begin + (uint32_t)(n * (s + 1) / S);
+}
+
+// the part of its segment a histogram CTA takes when sp.split CTAs share a segment
+__device__ __forceinline__ void split_segment_of(const Span& sp, uint32_t& t0, uint32_t& t1)
+{
+    const unsigned long long n = sp.n_tiles, S = gridDim.x / sp.split, s = blockIdx.x / sp.split, h = blockIdx.x % sp.split;
+    const uint32_t a = (uint32_t)(n * s / S), b = (uint32_t)(n * (s + 1) / S);
+    t0 = sp.tile_begin + a + (uint32_t)((unsigned long long)(b - a) * h / sp.split);
+    t1 = sp.tile_begin + a + (uint32_t)((unsigned long long)(b - a) * (h + 1) / sp.split);
 }
 
 // ---- the ring: stage = i % STAGES, one "full" mbarrier per stage, refilled by thread 0 ------------------
@@ -270,10 +281,11 @@ __global__ void __launch_bounds__(kThreads, 2) k_count_raw(const ChunkDesc* __re
                                                           Span sp, const __grid_constant__ DevGrid g,
                                                           const __grid_constant__ DevBeam bm, uint32_t B,
                                                           uint32_t lo_mask, uint32_t* __restrict__ table,
-                                                          uint32_t stride, SegStats* __restrict__ sstats)
+                                                          uint32_t stride, SegStats* __restrict__ sstats,
+                                                          uint32_t n_stages)
 {
     extern __shared__ __align__(128) uint8_t smem[];
-    const CountSmem L = count_layout(kTile * kRecBytes, kStagesCount, B, g.n_ebins + 1);
+    const CountSmem L = count_layout(kTile * kRecBytes, n_stages, B, g.n_ebins + 1);
     uint32_t* hist = reinterpret_cast<uint32_t*>(smem + L.hist);
     float* s_edges = reinterpret_cast<float*>(smem + L.edges);
     TileDesc* s_desc = reinterpret_cast<TileDesc*>(smem + L.desc);
@@ -281,13 +293,13 @@ __global__ void __launch_bounds__(kThreads, 2) k_count_raw(const ChunkDesc* __re
     const uint32_t rmask = (1u << L.rlog) - 1u;
 
     uint32_t t0, t1;
-    segment_of(sp, t0, t1);
+    split_segment_of(sp, t0, t1);
     const uint32_t n = t1 - t0;
 
     if (threadIdx.x == 0) {
-        for (int k = 0; k < kStagesCount; ++k) mbar_init(&bars[k], 1);
+        for (uint32_t k = 0; k < n_stages; ++k) mbar_init(&bars[k], 1);
         mbar_fence_init();
-        for (uint32_t k = 0; k < (uint32_t)kStagesCount && k < n; ++k) {
+        for (uint32_t k = 0; k < n_stages && k < n; ++k) {
             TileDesc d = raw_tile(chunks, n_chunks, t0 + k);
             s_desc[k] = d;
             ring_issue(reinterpret_cast<uint32_t*>(smem + L.ring + k * L.stage_bytes), &bars[k], d.ptr, d.count * kRecBytes);
@@ -300,7 +312,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_count_raw(const ChunkDesc* __re
     ThreadStats st;
     uint32_t phase_bits = 0;
     for (uint32_t i = 0; i < n; ++i) {
-        const uint32_t stage = i % kStagesCount;
+        const uint32_t stage = i % n_stages;
         uint32_t* raw = reinterpret_cast<uint32_t*>(smem + L.ring + stage * L.stage_bytes);
         const TileDesc td = s_desc[stage];
         ring_acquire(raw, &bars[stage], phase_bits, stage, td.ptr, td.count * kRecBytes);
@@ -331,8 +343,8 @@ __global__ void __launch_bounds__(kThreads, 2) k_count_raw(const ChunkDesc* __re
             }
         }
         __syncthreads();  // every thread is done with the stage
-        if (threadIdx.x == 0 && i + kStagesCount < n) {
-            TileDesc d = raw_tile(chunks, n_chunks, t0 + i + kStagesCount);
+        if (threadIdx.x == 0 && i + n_stages < n) {
+            TileDesc d = raw_tile(chunks, n_chunks, t0 + i + n_stages);
             s_desc[stage] = d;
             ring_issue(raw, &bars[stage], d.ptr, d.count * kRecBytes);
         }
@@ -488,7 +500,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_scatter_otf(const ChunkDesc* __
     TileDesc* s_desc = reinterpret_cast<TileDesc*>(smem + L.desc);
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + L.bars);
     const uint32_t w = warp_id();
-    const uint32_t col = sp.col0 + blockIdx.x;
+    const uint32_t col = sp.col0 + blockIdx.x * sp.split;
 
     uint32_t t0, t1;
     segment_of(sp, t0, t1);

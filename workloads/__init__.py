@@ -108,10 +108,22 @@ def generate(gp: GenParams, first: int, n: int, out: Optional[np.ndarray] = None
     return out[:n]
 
 
-def generate_into(gp: GenParams, first: int, n: int, address: int) -> None:
-    """Same stream written straight to ``address`` (e.g. a pinned torch buffer), 28*n bytes."""
+def generate_into(gp: GenParams, first: int, n: int, address: int, threads: int = 0) -> None:
+    """Same stream written straight to ``address`` (e.g. a pinned torch buffer), 28*n bytes.  The generator is
+    counter-based, so ``threads`` > 1 fills disjoint sub-ranges concurrently (ctypes releases the GIL)."""
     c = gp._c()
-    _load().wl_generate(ctypes.byref(c), first, n, ctypes.c_void_p(address))
+    lib = _load()
+    if threads <= 1 or n < 1_000_000:
+        lib.wl_generate(ctypes.byref(c), first, n, ctypes.c_void_p(address))
+        return
+    from concurrent.futures import ThreadPoolExecutor
+
+    piece = (n + threads - 1) // threads
+    piece += (-piece) % 4
+    jobs = [(f, min(piece, n - f)) for f in range(0, n, piece)]
+    with ThreadPoolExecutor(max_workers=threads) as ex:
+        list(ex.map(lambda j: lib.wl_generate(ctypes.byref(c), first + j[0], j[1],
+                                              ctypes.c_void_p(address + RECORD_DTYPE.itemsize * j[0])), jobs))
 
 
 # ----------------------------------------------------------------------------------------
