@@ -26,6 +26,7 @@ namespace {
 thread_local char g_err[256] = "";
 
 constexpr uint64_t kAlign = 256;
+constexpr uint64_t kScanSmallMax = 131072;  // table entries the single-CTA scan takes
 constexpr uint64_t kStageBytes = 32ull << 20;  // pinned staging buffers for pageable sources (two of them)
 
 struct Layout {
@@ -270,11 +271,14 @@ struct psl_ctx {
     uint32_t* h_scalars = nullptr;
     bool seg_pending = false;
     // launch shapes: persistent CTAs per launch (= SMs x resident CTAs of the scatter kernel, one wave)
-    uint32_t S_otf = 0, S_a = 0, S_b = 0;
+    uint32_t S_otf = 0, S_otf_small = 0, S_a = 0, S_b = 0;
+    uint32_t sm_scatter_small = 0;
     bool big_tiles = false;  // ONTHEFLY with few keys: the 4096-record-tile scatter
     uint32_t count_stages = kStagesCount, count_split = 1;
     uint32_t sm_count_raw = 0, sm_scatter_otf = 0, sm_idx_a = 0, sm_count_b = 0, sm_idx_b = 0;  // dynamic smem bytes
     struct ChunkLaunch { Span span; uint32_t n_seg; };
+    std::vector<ChunkDesc> pending_chunks;  // ONTHEFLY: chunk descriptors not yet on the device
+    uint32_t chunks_uploaded = 0;
     std::vector<ChunkLaunch> idx_launches;  // INDEX: the per-chunk count launches, replayed by pass A's scatter
     // state
     uint64_t n_records = 0, n_host_records = 0;
@@ -497,31 +501,51 @@ psl_status build_onthefly(psl_ctx* ctx, const DevBeam& bm)
         CU(cudaMemsetAsync(batch_off, 0, (uint64_t)(d.n_batches + 1) * 4, ctx->stream));
         CU(cudaMemsetAsync(stats, 0, sizeof(DevStats), ctx->stream));
     } else {
-        const ChunkDesc* chunks = at<ChunkDesc>(ctx, L.chunks);
+        ChunkDesc* chunks = at<ChunkDesc>(ctx, L.chunks);
+        for (size_t f = 0; f < ctx->pending_chunks.size(); f += 128) {
+            ChunkBatch cb;
+            const uint32_t m = (uint32_t)(ctx->pending_chunks.size() - f < 128 ? ctx->pending_chunks.size() - f : 128);
+            memcpy(cb.d, ctx->pending_chunks.data() + f, m * sizeof(ChunkDesc));
+            k_set_chunks<<<1, 128, 0, ctx->stream>>>(chunks + ctx->chunks_uploaded, cb, m);
+            LAUNCHED();
+            ctx->chunks_uploaded += m;
+        }
+        ctx->pending_chunks.clear();
         SegStats* ss = at<SegStats>(ctx, L.sstats);
-        const uint32_t S = nt < ctx->S_otf ? nt : ctx->S_otf;  // one persistent CTA per segment, one wave
-        const Span span = {0u, nt, 0u, ctx->count_split};
-        const uint32_t n_cols = S * ctx->count_split;
         const bool pos = ctx->grid.has_pos != 0, edges = ctx->grid.ebin_mode != 0, proj = bm.has_map || bm.out_proj;
         const int bv = beam_variant(bm);
+        // 4096-record tiles pay when most records are written out (long runs per key); when jaws reject most of
+        // them the kernel is a read stream and two 1024-record-tile CTAs per SM overlap better
+        const bool big = ctx->big_tiles && bv == 0;
+        const uint32_t S_max = big ? ctx->S_otf : ctx->S_otf_small, split = big ? ctx->count_split : 1u;
+        const uint32_t S = nt < S_max ? nt : S_max;  // one persistent CTA per segment, one wave
+        const Span span = {0u, nt, 0u, split};
+        const uint32_t n_cols = S * split;
         {
             Prof prof(ctx, PSL_K_COUNT);
             count_otf_fn(pos, edges, bv)<<<n_cols, kThreads, ctx->sm_count_raw, ctx->stream>>>(chunks, ctx->n_chunks, span, ctx->grid, bm, d.K, 0,
                                                                                              table, d.cols_cap, ss, ctx->count_stages);
             LAUNCHED();
         }
-        psl_status s = run_scan(ctx, table, d.K, n_cols, d.cols_cap, scalar(ctx, SC_TOTAL));
-        if (s != PSL_OK) return s;
-        k_offsets_from_table<<<(d.K + 1 + 255) / 256, 256, 0, ctx->stream>>>(table, d.cols_cap, d.K, scalar(ctx, SC_TOTAL),
-                                                                           offsets, counts, d.n_pos, d.n_batches, batch_off);
-        LAUNCHED();
+        if ((uint64_t)d.K * n_cols <= kScanSmallMax) {  // the usual case: one small kernel for scan + offsets
+            Prof prof(ctx, PSL_K_SCAN);
+            k_scan_small<<<1, 1024, 0, ctx->stream>>>(table, n_cols, d.cols_cap, d.K, scalar(ctx, SC_TOTAL), d.K, offsets,
+                                                      counts, d.n_pos, d.n_batches, batch_off);
+            LAUNCHED();
+        } else {
+            psl_status s = run_scan(ctx, table, d.K, n_cols, d.cols_cap, scalar(ctx, SC_TOTAL));
+            if (s != PSL_OK) return s;
+            k_offsets_from_table<<<(d.K + 1 + 255) / 256, 256, 0, ctx->stream>>>(table, d.cols_cap, d.K, scalar(ctx, SC_TOTAL),
+                                                                               offsets, counts, d.n_pos, d.n_batches, batch_off);
+            LAUNCHED();
+        }
         {
             Prof prof(ctx, PSL_K_SCATTER);
-            if (ctx->big_tiles)
+            if (big)
                 scatter_big_fn(pos, edges, bv, proj)<<<S, kBigThreads, ctx->sm_scatter_otf, ctx->stream>>>(chunks, ctx->n_chunks, span, ctx->grid, bm,
                                                                                                           d.K, table, d.cols_cap, soa_out(ctx, L.out), ss);
             else
-                scatter_otf_fn(pos, edges, bv, proj)<<<S, kThreads, ctx->sm_scatter_otf, ctx->stream>>>(chunks, ctx->n_chunks, span, ctx->grid, bm,
+                scatter_otf_fn(pos, edges, bv, proj)<<<S, kThreads, ctx->sm_scatter_small, ctx->stream>>>(chunks, ctx->n_chunks, span, ctx->grid, bm,
                                                                                                        d.K, table, d.cols_cap, soa_out(ctx, L.out), ss);
             LAUNCHED();
         }
@@ -588,8 +612,15 @@ psl_status finalize_index(psl_ctx* ctx)
             k_count_keys<<<Sb, kThreads, ctx->sm_count_b, ctx->stream>>>(aos, scalar(ctx, SC_NIDX), d.B_hi, d.lo_bits, table_b, kMaxSegments);
             LAUNCHED();
         }
-        s = run_scan(ctx, table_b, d.B_hi, Sb, kMaxSegments, scalar(ctx, SC_TOTAL));
-        if (s != PSL_OK) return s;
+        if ((uint64_t)d.B_hi * Sb <= kScanSmallMax) {
+            Prof prof(ctx, PSL_K_SCAN);
+            k_scan_small<<<1, 1024, 0, ctx->stream>>>(table_b, Sb, kMaxSegments, d.B_hi, scalar(ctx, SC_TOTAL), 0, nullptr, nullptr, 1,
+                                                      0, nullptr);
+            LAUNCHED();
+        } else {
+            s = run_scan(ctx, table_b, d.B_hi, Sb, kMaxSegments, scalar(ctx, SC_TOTAL));
+            if (s != PSL_OK) return s;
+        }
         {
             Prof prof(ctx, PSL_K_INDEX_B);
             k_scatter_idx_b<<<Sb, kBigThreads, ctx->sm_idx_b, ctx->stream>>>(aos, scalar(ctx, SC_NIDX), d.B_hi, d.lo_bits, table_b,
@@ -850,17 +881,20 @@ psl_status psl_create(const psl_config* cfg, psl_ctx** out)
         ctx->big_tiles = round_up(d.K, 8) <= (uint32_t)kBigMaxKeys;
         ctx->sm_scatter_otf = ctx->big_tiles ? big_layout(d.K, ne).total : part_layout(kTile * kRecBytes, kStagesRaw, d.K, ne, true).total;
         const bool pos = d.n_pos > 1, edges = cfg->ebin_mode == PSL_EBIN_EDGES;
+        ctx->sm_scatter_small = part_layout(kTile * kRecBytes, kStagesRaw, d.K, ne, true).total;
         for (int bv = 0; bv < 3; ++bv) {
             CUC(allow_smem(count_otf_fn(pos, edges, bv), ctx->sm_count_raw));
-            for (int pj = 0; pj < 2; ++pj)
-                CUC(allow_smem(ctx->big_tiles ? scatter_big_fn(pos, edges, bv, pj != 0) : scatter_otf_fn(pos, edges, bv, pj != 0),
-                               ctx->sm_scatter_otf));
+            for (int pj = 0; pj < 2; ++pj) {
+                CUC(allow_smem(scatter_otf_fn(pos, edges, bv, pj != 0), ctx->sm_scatter_small));
+                if (ctx->big_tiles) CUC(allow_smem(scatter_big_fn(pos, edges, bv, pj != 0), ctx->sm_scatter_otf));
+            }
         }
-        if (ctx->big_tiles)
+        CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, scatter_otf_fn(pos, edges, 2, true), kThreads, ctx->sm_scatter_small));
+        ctx->S_otf_small = width(occ);
+        if (ctx->big_tiles) {
             CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, scatter_big_fn(pos, edges, 2, true), kBigThreads, ctx->sm_scatter_otf));
-        else
-            CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, scatter_otf_fn(pos, edges, 2, true), kThreads, ctx->sm_scatter_otf));
-        ctx->S_otf = width(occ);
+            ctx->S_otf = width(occ);
+        }
         ctx->count_split = ctx->big_tiles ? 2 : 1;  // one scatter CTA per SM, two histogram CTAs
     } else {
         ctx->count_stages = d.B_lo * 4 > 8192 ? 2 : kStagesCount;
@@ -895,6 +929,8 @@ psl_status psl_reset(psl_ctx* ctx)
     ctx->n_records = ctx->n_host_records = 0;
     ctx->n_tiles = ctx->n_chunks = ctx->n_cols = 0;
     ctx->idx_launches.clear();
+    ctx->pending_chunks.clear();
+    ctx->chunks_uploaded = 0;
     ctx->ragged = false;
     ctx->indexed = false;
     ctx->result = RES_NONE;
@@ -961,8 +997,12 @@ psl_status psl_load_chunk(psl_ctx* ctx, const void* records, uint64_t n, int32_t
     cd.tile0 = tile0;
     cd.pad = 0;
     ChunkDesc* chunks = at<ChunkDesc>(ctx, ctx->L.chunks);
-    k_set_chunk<<<1, 1, 0, ctx->stream>>>(chunks + ctx->n_chunks, cd);  // the descriptor travels as a kernel argument
-    LAUNCHED();
+    if (ctx->cfg.mode == PSL_MODE_INDEX) {
+        k_set_chunk<<<1, 1, 0, ctx->stream>>>(chunks + ctx->n_chunks, cd);  // the descriptor travels as a kernel argument
+        LAUNCHED();
+    } else {
+        ctx->pending_chunks.push_back(cd);  // ONTHEFLY reads the table only at build time: uploaded there, 128 at a time
+    }
     if (ctx->cfg.mode == PSL_MODE_INDEX) {
         // a8 for pass A, chunk by chunk: overlaps the transfer of the next chunk
         DevBeam none;

@@ -18,7 +18,7 @@ namespace psl {
 
 constexpr int kIdxMaxLo = 8192;   // most buckets of pass A
 constexpr int kIdxMaxHi = 256;    // most buckets of pass B
-constexpr int kStagesIdxA = 2;
+constexpr int kStagesIdxA = 1;
 
 struct IdxASmem {
     uint32_t ring, stage_bytes, run, skey, sdest, edges, desc, bars, total;
@@ -41,7 +41,7 @@ __host__ __device__ inline IdxASmem idx_a_layout(uint32_t B, uint32_t n_edges)
 }
 
 template <bool POS, bool EDGES>
-__global__ void __launch_bounds__(kThreads, 2) k_scatter_idx_a(const ChunkDesc* __restrict__ chunks, uint32_t n_chunks,
+__global__ void __launch_bounds__(kThreads, 3) k_scatter_idx_a(const ChunkDesc* __restrict__ chunks, uint32_t n_chunks,
                                                               Span sp, const __grid_constant__ DevGrid g,
                                                               const __grid_constant__ DevBeam bm, uint32_t B,
                                                               uint32_t lo_bits, const uint32_t* __restrict__ table,

@@ -110,6 +110,15 @@ __device__ __forceinline__ void stage_edges(const DevGrid& g, float* s_edges)
 // one entry of the chunk table (psl_load_chunk)
 __global__ void k_set_chunk(ChunkDesc* __restrict__ dst, ChunkDesc d) { *dst = d; }
 
+// up to 128 entries at once (the descriptors travel as a kernel argument)
+struct ChunkBatch {
+    ChunkDesc d[128];
+};
+__global__ void k_set_chunks(ChunkDesc* __restrict__ dst, const __grid_constant__ ChunkBatch b, uint32_t n)
+{
+    if (threadIdx.x < n) dst[threadIdx.x] = b.d[threadIdx.x];
+}
+
 // tile id -> descriptor.  Raw records: binary search over the chunk table (tiles never straddle chunks).
 __device__ __forceinline__ TileDesc raw_tile(const ChunkDesc* __restrict__ chunks, uint32_t n_chunks, uint32_t t)
 {
@@ -430,6 +439,63 @@ __global__ void __launch_bounds__(kScanThreads) k_scan_apply(uint32_t* __restric
         if (v < L) table[p] = carry + ex;
         carry += tot;
         __syncthreads();
+    }
+}
+
+// Small tables (a few keys x one wave of segments): the whole scan in ONE CTA -- a warp scans a row (bucket) at a
+// time with coalesced loads, the row totals are scanned by the CTA, the row bases are added back -- followed
+// (ONTHEFLY, offsets != nullptr) by what k_offsets_from_table computes.  B <= kMaxBuckets rows.
+__global__ void __launch_bounds__(1024) k_scan_small(uint32_t* __restrict__ table, uint32_t n_cols, uint32_t stride,
+                                                     uint32_t B, uint32_t* __restrict__ total_out, uint32_t K,
+                                                     uint32_t* __restrict__ offsets, uint32_t* __restrict__ counts,
+                                                     uint32_t n_pos, uint32_t n_batches,
+                                                     uint32_t* __restrict__ batch_offsets)
+{
+    __shared__ uint32_t s_misc[64];
+    __shared__ uint32_t s_row[kMaxBuckets];
+    const uint32_t w = warp_id();
+    for (uint32_t row = w; row < B; row += 32) {
+        uint32_t* r = table + (size_t)row * stride;
+        constexpr int kPieces = (kMaxSegments + 31) / 32;  // all loads of the row in flight before the first scan
+        uint32_t x[kPieces];
+#pragma unroll
+        for (int k = 0; k < kPieces; ++k) {
+            const uint32_t c = k * 32 + lane_id();
+            x[k] = c < n_cols ? r[c] : 0u;
+        }
+        uint32_t carry = 0;
+#pragma unroll
+        for (int k = 0; k < kPieces; ++k) {
+            const uint32_t c = k * 32 + lane_id();
+            if (k * 32 < (int)n_cols) {
+                const uint32_t inc = warp_incl_scan(x[k]);
+                if (c < n_cols) r[c] = carry + inc - x[k];
+                carry += __shfl_sync(0xFFFFFFFFu, inc, 31);
+            }
+        }
+        if (lane_id() == 0) s_row[row] = carry;
+    }
+    __syncthreads();
+    // exclusive scan of the row totals: thread t takes rows 2t, 2t+1
+    const uint32_t r0 = 2 * threadIdx.x;
+    const uint32_t a0 = r0 < B ? s_row[r0] : 0u, a1 = r0 + 1 < B ? s_row[r0 + 1] : 0u;
+    uint32_t total;
+    const uint32_t ex = block_excl_scan(a0 + a1, s_misc, &total);
+    if (r0 < B) s_row[r0] = ex;
+    if (r0 + 1 < B) s_row[r0 + 1] = ex + a0;
+    __syncthreads();
+    for (uint32_t row = w; row < B; row += 32) {
+        uint32_t* r = table + (size_t)row * stride;
+        const uint32_t base = s_row[row];
+        for (uint32_t c = lane_id(); c < n_cols; c += 32) r[c] += base;
+    }
+    if (threadIdx.x == 0) *total_out = total;
+    if (offsets == nullptr) return;
+    for (uint32_t k = threadIdx.x; k <= K; k += 1024) {  // offsets[k] = scanned table[k][0] = the row base
+        const uint32_t o = (k < K) ? s_row[k] : total;
+        offsets[k] = o;
+        if (k < K) counts[k] = ((k + 1 < K) ? s_row[k + 1] : total) - o;
+        if (k % n_pos == 0 && k / n_pos <= n_batches) batch_offsets[k / n_pos] = o;
     }
 }
 
