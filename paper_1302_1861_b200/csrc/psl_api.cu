@@ -35,7 +35,7 @@ struct Layout {
     // ONTHEFLY
     uint64_t table = 0, out[10] = {0}, offsets = 0, counts = 0;
     // INDEX
-    uint64_t table_a = 0, table_b = 0, aos = 0, idx[7] = {0}, keyfull = 0, idx_offsets = 0, idx_counts = 0,
+    uint64_t table_a = 0, table_b = 0, aos = 0, aos_index = 0, idx[7] = {0}, idx_offsets = 0, idx_counts = 0,
              idx_batch_off = 0;
     uint64_t seg = 0, beam_out[10] = {0}, beam_keys = 0, beam_offsets = 0, beam_counts = 0, lookback = 0, bstats = 0,
              beam_stats = 0;
@@ -121,8 +121,11 @@ psl_status derive(const psl_config* c, Derived* d, char* err)
         if (K > kMaxBuckets) { set_err(err, "ONTHEFLY mode handles at most %d keys (got %llu); use PSL_MODE_INDEX", kMaxBuckets, (unsigned long long)K); return PSL_ERR_ARG; }
     } else {
         if (K > (uint64_t)kIdxMaxHi * kIdxMaxLo) { set_err(err, "INDEX mode handles at most %d keys", kIdxMaxHi * kIdxMaxLo); return PSL_ERR_ARG; }
-        // key = hi * 2^lo_bits + lo: pass B wants few buckets (<= 256, long output runs), pass A takes the rest
-        uint32_t lo = 0;
+        // key = hi * 2^lo_bits + lo, two balanced digits: what matters is that (buckets x CTAs x 128 B), the lines
+        // being filled at any time, stays inside the 126 MB L2 in both passes
+        uint32_t bits = 0;
+        while ((1ull << bits) < K) ++bits;
+        uint32_t lo = bits / 2;
         while ((((K - 1) >> lo) + 1) > (uint64_t)kIdxMaxHi) ++lo;
         d->lo_bits = lo;
         d->B_lo = (uint32_t)((K < (1ull << lo)) ? K : (1ull << lo));
@@ -171,9 +174,13 @@ void plan(const psl_config* c, const Derived& d, Layout* L)
     } else {
         L->table_a = take(&cur, (uint64_t)d.B_lo * d.cols_cap * 4);
         L->table_b = take(&cur, (uint64_t)d.B_hi * kMaxSegments * 4);
-        L->aos = take(&cur, N * 32);
-        for (int i = 0; i < 7; ++i) L->idx[i] = take(&cur, N * 4);
-        L->keyfull = take(&cur, N * 4);
+        {   // pass A output; once the index is built the SoA view of the bare index (7 arrays) lives in the same bytes
+            const uint64_t view_bytes = 7 * ((N * 4 + kAlign - 1) / kAlign * kAlign);
+            L->aos = take(&cur, N * 32 > view_bytes ? N * 32 : view_bytes);
+            uint64_t view = L->aos;
+            for (int i = 0; i < 7; ++i) L->idx[i] = take(&view, N * 4);
+        }
+        L->aos_index = take(&cur, N * 32);  // the index: keyed records sorted by the full key
         L->idx_offsets = take(&cur, (uint64_t)(d.K + 1) * 4);
         L->idx_counts = take(&cur, (uint64_t)d.K * 4);
         L->idx_batch_off = take(&cur, (uint64_t)(d.n_batches + 1) * 4);
@@ -284,7 +291,7 @@ struct psl_ctx {
     uint64_t n_records = 0, n_host_records = 0;
     uint32_t n_tiles = 0, n_chunks = 0, n_cols = 0;
     bool ragged = false;  // a chunk with n % 4 != 0 was loaded: no more chunks may follow
-    bool indexed = false;
+    bool indexed = false, soa_view = false;
     int result = RES_NONE;
     DevStats idx_stats = {};
     uint64_t n_idx = 0, last_M = 0;
@@ -566,7 +573,7 @@ IdxOut idx_out(psl_ctx* ctx)
     o.E = at<float>(ctx, L.idx[0]); o.x = at<float>(ctx, L.idx[1]); o.y = at<float>(ctx, L.idx[2]);
     o.u = at<float>(ctx, L.idx[3]); o.v = at<float>(ctx, L.idx[4]); o.wt = at<float>(ctx, L.idx[5]);
     o.src = at<uint32_t>(ctx, L.idx[6]);
-    o.key = at<uint32_t>(ctx, L.keyfull);
+    o.key = nullptr;
     return o;
 }
 
@@ -623,11 +630,11 @@ psl_status finalize_index(psl_ctx* ctx)
         }
         {
             Prof prof(ctx, PSL_K_INDEX_B);
-            k_scatter_idx_b<<<Sb, kBigThreads, ctx->sm_idx_b, ctx->stream>>>(aos, scalar(ctx, SC_NIDX), d.B_hi, d.lo_bits, table_b,
-                                                                         kMaxSegments, idx_out(ctx));
+            k_scatter_idx_b<<<Sb, kThreads, ctx->sm_idx_b, ctx->stream>>>(aos, scalar(ctx, SC_NIDX), d.B_hi, d.lo_bits, table_b,
+                                                                         kMaxSegments, at<uint4>(ctx, L.aos_index));
             LAUNCHED();
         }
-        k_offsets_by_search<<<(d.K + 1 + 255) / 256, 256, 0, ctx->stream>>>(at<uint32_t>(ctx, L.keyfull), scalar(ctx, SC_NIDX), d.K, idx_offsets);
+        k_offsets_by_search_keyed<<<(d.K + 1 + 255) / 256, 256, 0, ctx->stream>>>(at<uint4>(ctx, L.aos_index), scalar(ctx, SC_NIDX), d.K, idx_offsets);
         LAUNCHED();
         k_counts_from_offsets<<<(d.K + 1 + 255) / 256, 256, 0, ctx->stream>>>(idx_offsets, d.K, idx_counts, d.n_pos, d.n_batches, idx_batch);
         LAUNCHED();
@@ -647,6 +654,11 @@ psl_status expose_index(psl_ctx* ctx)
 {
     const Derived& d = ctx->d;
     for (uint32_t b = 0; b <= d.n_batches; ++b) ctx->h_batch_off[b] = ctx->h_idx_offsets[(uint64_t)b * d.n_pos];
+    if (!ctx->soa_view && ctx->n_idx > 0) {  // the index is kept as keyed records; the SoA arrays are made on demand
+        k_index_to_soa<<<1184, 256, 0, ctx->stream>>>(at<uint4>(ctx, ctx->L.aos_index), scalar(ctx, SC_NIDX), idx_out(ctx));
+        LAUNCHED();
+        ctx->soa_view = true;
+    }
     CU(cudaEventRecord(ctx->ev_batch, ctx->stream));
     ctx->result = RES_INDEX;
     return PSL_OK;
@@ -712,9 +724,7 @@ psl_status build_beam_from_index(psl_ctx* ctx, const psl_beam* beam, const DevBe
         st.n_seg = n_seg;
         st.M = (uint32_t)M;
         IdxIn in;
-        in.E = at<float>(ctx, L.idx[0]); in.x = at<float>(ctx, L.idx[1]); in.y = at<float>(ctx, L.idx[2]);
-        in.u = at<float>(ctx, L.idx[3]); in.v = at<float>(ctx, L.idx[4]); in.wt = at<float>(ctx, L.idx[5]);
-        in.src = at<uint32_t>(ctx, L.idx[6]);
+        in.aos = at<uint4>(ctx, L.aos_index);
         {
             Prof prof(ctx, PSL_K_BEAM);
             k_beam_compact<<<nt, kThreads, 11 * kBeamTile * 4, ctx->stream>>>(st, in, ctx->grid, bm, soa_out(ctx, L.beam_out), beam_keys,
@@ -910,7 +920,7 @@ psl_status psl_create(const psl_config* cfg, psl_ctx** out)
         CUC(allow_smem(k_beam_compact, 11 * kBeamTile * 4));
         CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, scatter_idx_a_fn(pos, edges), kThreads, ctx->sm_idx_a));
         ctx->S_a = width(occ);
-        CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_scatter_idx_b, kBigThreads, ctx->sm_idx_b));
+        CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_scatter_idx_b, kThreads, ctx->sm_idx_b));
         ctx->S_b = width(occ);
     }
     CUC(cudaStreamSynchronize(ctx->stream));
@@ -933,6 +943,7 @@ psl_status psl_reset(psl_ctx* ctx)
     ctx->chunks_uploaded = 0;
     ctx->ragged = false;
     ctx->indexed = false;
+    ctx->soa_view = false;
     ctx->result = RES_NONE;
     ctx->n_idx = ctx->last_M = 0;
     return PSL_OK;

@@ -25,8 +25,7 @@ struct SegTable {
 };
 
 struct IdxIn {
-    const float *E, *x, *y, *u, *v, *wt;
-    const uint32_t* src;
+    const uint4* aos;  // the index: 32-byte keyed records {key, E, x, y, u, v, wt, src} sorted by key
 };
 
 struct BeamTileStats {  // 16 bytes
@@ -95,12 +94,12 @@ __global__ void __launch_bounds__(kThreads) k_beam_compact(SegTable seg, IdxIn i
             uint32_t vv = v0 + lv;
             uint32_t sg = seg_of(seg.vstart, s_first, s_last, vv);
             uint32_t p = __ldg(seg.src + sg) + (vv - __ldg(seg.vstart + sg));
-            E = in.E[p]; x = in.x[p]; y = in.y[p]; u = in.u[p]; v = in.v[p];
-            float wt0 = in.wt[p];
-            srci = in.src[p];
-            int ix = 0;
-            if (g.has_pos) axis_bin(x, g.inv_dx, g.ix0, g.n_xbins, ix);
-            key = __ldg(seg.keybase + sg) + (uint32_t)ix;
+            const uint4 ra = __ldg(in.aos + 2 * (size_t)p), rb = __ldg(in.aos + 2 * (size_t)p + 1);
+            E = __uint_as_float(ra.y); x = __uint_as_float(ra.z); y = __uint_as_float(ra.w);
+            u = __uint_as_float(rb.x); v = __uint_as_float(rb.y);
+            float wt0 = __uint_as_float(rb.z);
+            srci = rb.w;
+            key = ra.x;  // the full key travels with the record
             float q = q_of(u, v), tx, ty;
             slopes(u, v, q, wz, tx, ty);
             keep = !(bm.has_jaws) || jaw_pass(bm, x, y, tx, ty);

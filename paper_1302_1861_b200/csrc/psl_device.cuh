@@ -249,6 +249,19 @@ __device__ __forceinline__ void tma_load_1d(void* smem_dst, const void* gsrc, ui
                  : "memory");
 }
 
+// the same copy with an L2 evict-first policy: a read-once stream must not push half-filled output lines
+// out of L2 (the INDEX passes rely on L2 to merge their 32-byte sector writes into whole lines)
+__device__ __forceinline__ void tma_load_1d_stream(void* smem_dst, const void* gsrc, uint32_t bytes, uint64_t* bar)
+{
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
+            smem_u32(smem_dst)),
+        "l"(gsrc), "r"(bytes), "r"(smem_u32(bar)), "l"(pol)
+        : "memory");
+}
+
 // Bring `bytes` (a multiple of 4) from global into s_dst.  Must be called by all threads of the CTA; `bar`
 // must have been initialised (count 1) and made visible with a __syncthreads.  Ends with the data visible
 // to every thread.

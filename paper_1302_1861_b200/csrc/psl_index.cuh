@@ -16,12 +16,12 @@
 
 namespace psl {
 
-constexpr int kIdxMaxLo = 8192;   // most buckets of pass A
-constexpr int kIdxMaxHi = 256;    // most buckets of pass B
-constexpr int kStagesIdxA = 1;
+constexpr int kIdxMaxLo = 2048;   // most buckets of pass A
+constexpr int kIdxMaxHi = 2048;   // most buckets of pass B
+constexpr int kStagesIdxA = 2;
 
 struct IdxASmem {
-    uint32_t ring, stage_bytes, run, skey, sdest, edges, desc, bars, total;
+    uint32_t ring, stage_bytes, cnt, run, misc, skey, sdest, edges, desc, bars, total;
 };
 
 __host__ __device__ inline IdxASmem idx_a_layout(uint32_t B, uint32_t n_edges)
@@ -30,7 +30,9 @@ __host__ __device__ inline IdxASmem idx_a_layout(uint32_t B, uint32_t n_edges)
     uint32_t p = 0;
     L.stage_bytes = round_up(kTile * kRecBytes, 128);
     L.ring = p;  p += kStagesIdxA * L.stage_bytes;
-    L.run = p;   p += round_up(B * 4, 16);   // first free slot of every bucket, running over the segment
+    L.cnt = p;   p += round_up(kWarps * round_up(B, 8) * 2, 16);  // [kWarps][Bp] uint16 running counts
+    L.run = p;   p += round_up(B * 4, 16);   // first slot of every bucket for this tile
+    L.misc = p;  p += 64 * 4;
     L.skey = p;  p += kTile * 4;             // full key of every record of the tile, kNone = dropped
     L.sdest = p; p += kTile * 4;             // slot of every record
     L.edges = p; p += round_up(n_edges * 4, 16);
@@ -38,6 +40,14 @@ __host__ __device__ inline IdxASmem idx_a_layout(uint32_t B, uint32_t n_edges)
     L.bars = p;  p += kStagesIdxA * 8;
     L.total = p;
     return L;
+}
+
+__device__ __forceinline__ void ring_issue_stream(uint32_t* s_dst, uint64_t* bar, const void* src, uint32_t bytes)
+{
+    if (bulk_ok(src, bytes)) {
+        mbar_expect_tx(bar, bytes);
+        tma_load_1d_stream(s_dst, src, bytes, bar);
+    }
 }
 
 template <bool POS, bool EDGES>
@@ -68,10 +78,22 @@ __global__ void __launch_bounds__(kThreads, 3) k_scatter_idx_a(const ChunkDesc* 
         for (uint32_t k = 0; k < (uint32_t)kStagesIdxA && k < n; ++k) {
             TileDesc d = raw_tile(chunks, n_chunks, t0 + k);
             s_desc[k] = d;
-            ring_issue(reinterpret_cast<uint32_t*>(smem + L.ring + k * L.stage_bytes), &bars[k], d.ptr, d.count * kRecBytes);
+            ring_issue_stream(reinterpret_cast<uint32_t*>(smem + L.ring + k * L.stage_bytes), &bars[k], d.ptr, d.count * kRecBytes);
         }
     }
-    for (uint32_t b = threadIdx.x; b < B; b += kThreads) run[b] = table[(size_t)b * stride + col];
+    const uint32_t Bp = round_up(B, 8);
+    uint16_t* cnt = reinterpret_cast<uint16_t*>(smem + L.cnt);
+    uint32_t* misc = reinterpret_cast<uint32_t*>(smem + L.misc);
+    {
+        uint32_t* cz = reinterpret_cast<uint32_t*>(cnt);
+        for (uint32_t k = threadIdx.x; k < kWarps * Bp / 2; k += kThreads) cz[k] = 0;
+    }
+    uint32_t grun[8];  // thread t keeps the running first free slot of buckets 8t..8t+7
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        uint32_t b = threadIdx.x * 8 + k;
+        grun[k] = b < B ? table[(size_t)b * stride + col] : 0u;
+    }
     stage_edges(g, s_edges);
     __syncthreads();
 
@@ -82,41 +104,44 @@ __global__ void __launch_bounds__(kThreads, 3) k_scatter_idx_a(const ChunkDesc* 
         const TileDesc td = s_desc[stage];
         ring_acquire(raw, &bars[stage], phase_bits, stage, td.ptr, td.count * kRecBytes);
 
-        // keys of the tile (a1-a4); thread t takes records t, t + 256, ...
+        // keys (a1-a4) and stable ranks inside the warp's 128 consecutive records
+        uint32_t packed[kRounds];  // key << 9 | rank   (key < 2^22)
         {
             Rec rec[kRounds];
 #pragma unroll
             for (int r = 0; r < kRounds; ++r) {
-                int idx = r * kThreads + threadIdx.x;
+                int idx = w * kWarpSpan + r * 32 + lane_id();
                 rec[r] = rec_from_smem(raw, idx < (int)td.count ? idx : 0);
             }
 #pragma unroll
             for (int r = 0; r < kRounds; ++r) {
-                int idx = r * kThreads + threadIdx.x;
+                int idx = w * kWarpSpan + r * 32 + lane_id();
                 uint32_t key;
                 int cls = classify<POS, EDGES, 0>(g, bm, rec[r], s_edges, key);
-                skey[idx] = (idx < (int)td.count && cls == C_SURVIVOR) ? key : kNone;
+                packed[r] = (idx < (int)td.count && cls == C_SURVIVOR) ? key : kNone;
+            }
+#pragma unroll
+            for (int r = 0; r < kRounds; ++r) {
+                uint32_t key = packed[r];
+                uint32_t rank = warp_rank(key == kNone ? kNone : (key & lo_mask), cnt + w * Bp);
+                packed[r] = key == kNone ? kNone : ((key << 9) | rank);
             }
         }
         __syncthreads();
-        // slots, in input order: one warp walks the tile 32 keys at a time
-        if (w == 0) {
-#pragma unroll 4
-            for (int r = 0; r < kTile / 32; ++r) {
-                const uint32_t key = skey[r * 32 + lane_id()];
-                const uint32_t bucket = key == kNone ? kNone : (key & lo_mask);
-                const uint32_t peers = __match_any_sync(0xFFFFFFFFu, bucket);
-                const int leader = __ffs(peers) - 1;
-                uint32_t base = 0;
-                if ((int)lane_id() == leader && bucket != kNone) {
-                    base = run[bucket];
-                    run[bucket] = base + __popc(peers);
-                }
-                base = __shfl_sync(0xFFFFFFFFu, base, leader);
-                sdest[r * 32 + lane_id()] = bucket == kNone ? kNone : base + __popc(peers & lanemask_lt());
+        finish_ranks<false>(cnt, B, Bp, run, nullptr, misc, grun);
+#pragma unroll
+        for (int r = 0; r < kRounds; ++r) {
+            const uint32_t idx = w * kWarpSpan + r * 32 + lane_id();
+            uint32_t key = kNone, dest = kNone;
+            if (packed[r] != kNone) {
+                key = packed[r] >> 9;
+                const uint32_t bucket = key & lo_mask;
+                dest = run[bucket] + cnt[w * Bp + bucket] + (packed[r] & 511u);
             }
+            skey[idx] = key;
+            sdest[idx] = dest;
         }
-        __syncthreads();
+        __syncwarp();
         // one full 32-byte sector per record: lanes 2k and 2k+1 write its two halves in one instruction
         {
             const uint32_t half = lane_id() & 1u;
@@ -133,12 +158,15 @@ __global__ void __launch_bounds__(kThreads, 3) k_scatter_idx_a(const ChunkDesc* 
                 }
             }
         }
+        __syncwarp();
+        zero_row(cnt + w * Bp, Bp);
         __syncthreads();  // the stage, skey and sdest are free again
         if (threadIdx.x == 0 && i + kStagesIdxA < n) {
             TileDesc d = raw_tile(chunks, n_chunks, t0 + i + kStagesIdxA);
             s_desc[stage] = d;
-            ring_issue(raw, &bars[stage], d.ptr, d.count * kRecBytes);
+            ring_issue_stream(raw, &bars[stage], d.ptr, d.count * kRecBytes);
         }
+        if (kStagesIdxA == 1) __syncthreads();  // the descriptor just written is read at the top of the next tile
     }
 }
 
@@ -173,10 +201,8 @@ __global__ void __launch_bounds__(kThreads) k_count_keys(const uint4* __restrict
     }
 }
 
-constexpr int kIdxBStages = 5;  // 4 being worked on + 1 in flight (32 KB each)
-
 struct IdxBSmem {
-    uint32_t ring, stage_bytes, cnt, gcur, lstart, pdest, perm, misc, desc, bars, total;
+    uint32_t ring, stage_bytes, cnt, run, misc, sdest, desc, bar, total;
 };
 
 __host__ __device__ inline IdxBSmem idx_b_layout(uint32_t B)
@@ -184,37 +210,35 @@ __host__ __device__ inline IdxBSmem idx_b_layout(uint32_t B)
     IdxBSmem L;
     uint32_t p = 0;
     L.stage_bytes = kTile * 32;
-    L.ring = p;   p += kIdxBStages * L.stage_bytes;
-    L.cnt = p;    p += round_up(kBigWarps * round_up(B, 8) * 2, 16);
-    L.gcur = p;   p += round_up(B * 4, 16);
-    L.lstart = p; p += round_up(B * 4, 16);
-    L.pdest = p;  p += kBigTile * 4;
-    L.perm = p;   p += kBigTile * 2;
-    L.misc = p;   p += 64 * 4;
-    L.desc = p;   p += kIdxBStages * 16;
-    L.bars = p;   p += kIdxBStages * 8;
+    L.ring = p;  p += 2 * L.stage_bytes;     // two stages: the next tile loads while this one is ranked and written
+    L.cnt = p;   p += round_up(kWarps * round_up(B, 8) * 2, 16);
+    L.run = p;   p += round_up(B * 4, 16);
+    L.misc = p;  p += 64 * 4;
+    L.sdest = p; p += kTile * 4;
+    L.desc = p;  p += 16;
+    L.bar = p;   p += 16;
     L.total = p;
     return L;
 }
 
-// INDEX pass B scatter: keyed records (sorted by low digit) -> SoA index sorted by the full key, plus the
-// full key of every slot (used once, by binary search, to build offsets[K+1]).  4096-record tiles.
-__global__ void __launch_bounds__(kBigThreads, 1) k_scatter_idx_b(const uint4* __restrict__ aos,
-                                                                 const uint32_t* __restrict__ n_ptr, uint32_t B,
-                                                                 uint32_t lo_bits, const uint32_t* __restrict__ table,
-                                                                 uint32_t stride, IdxOut out)
+// INDEX pass B: keyed records (sorted by low digit) -> the index: keyed records sorted by the full key.  Same
+// shape as pass A: running slots per bucket in shared memory, one warp assigns slots in input order, one full
+// 32-byte sector per record.  With <= 2048 buckets the lines being filled (buckets x CTAs x 128 B) stay in L2
+// until they are complete, so DRAM sees whole lines.
+__global__ void __launch_bounds__(kThreads, 4) k_scatter_idx_b(const uint4* __restrict__ aos_in,
+                                                              const uint32_t* __restrict__ n_ptr, uint32_t B,
+                                                              uint32_t lo_bits, const uint32_t* __restrict__ table,
+                                                              uint32_t stride, uint4* __restrict__ aos_out)
 {
     extern __shared__ __align__(128) uint8_t smem[];
-    const uint32_t Bp = round_up(B, 8);
     const IdxBSmem L = idx_b_layout(B);
+    uint32_t* ring = reinterpret_cast<uint32_t*>(smem + L.ring);
+    uint32_t* run = reinterpret_cast<uint32_t*>(smem + L.run);
+    uint32_t* sdest = reinterpret_cast<uint32_t*>(smem + L.sdest);
+    uint64_t* bar = reinterpret_cast<uint64_t*>(smem + L.bar);
     uint16_t* cnt = reinterpret_cast<uint16_t*>(smem + L.cnt);
-    uint32_t* gcur = reinterpret_cast<uint32_t*>(smem + L.gcur);
-    uint32_t* lstart = reinterpret_cast<uint32_t*>(smem + L.lstart);
-    uint32_t* pdest = reinterpret_cast<uint32_t*>(smem + L.pdest);
-    uint16_t* perm = reinterpret_cast<uint16_t*>(smem + L.perm);
     uint32_t* misc = reinterpret_cast<uint32_t*>(smem + L.misc);
-    TileDesc* s_desc = reinterpret_cast<TileDesc*>(smem + L.desc);
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + L.bars);
+    const uint32_t Bp = round_up(B, 8);
     const uint32_t w = warp_id();
     const uint32_t n_rec = *n_ptr;
 
@@ -222,22 +246,21 @@ __global__ void __launch_bounds__(kBigThreads, 1) k_scatter_idx_b(const uint4* _
     uint32_t t0, t1;
     segment_of(sp, t0, t1);
     const uint32_t n = t1 - t0;
-
-    auto stage_ptr = [&](uint32_t i) { return reinterpret_cast<uint32_t*>(smem + L.ring + (i % kIdxBStages) * L.stage_bytes); };
     auto issue = [&](uint32_t i) {  // thread 0; 32-byte records from a 256-byte aligned array: always bulk-copyable
-        TileDesc d = keyed_tile(aos, n_rec, t0 + i);
-        s_desc[i % kIdxBStages] = d;
-        mbar_expect_tx(&bars[i % kIdxBStages], d.count * 32u);
-        tma_load_1d(stage_ptr(i), d.ptr, d.count * 32u, &bars[i % kIdxBStages]);
+        TileDesc d = keyed_tile(aos_in, n_rec, t0 + i);
+        mbar_expect_tx(&bar[i & 1u], d.count * 32u);
+        tma_load_1d_stream(ring + (i & 1u) * (kTile * 8), d.ptr, d.count * 32u, &bar[i & 1u]);
     };
     if (threadIdx.x == 0) {
-        for (int k = 0; k < kIdxBStages; ++k) mbar_init(&bars[k], 1);
+        mbar_init(&bar[0], 1);
+        mbar_init(&bar[1], 1);
         mbar_fence_init();
-        for (uint32_t k = 0; k < (uint32_t)kIdxBStages && k < n; ++k) issue(k);
+        if (n > 0) issue(0);
+        if (n > 1) issue(1);
     }
     {
         uint32_t* cz = reinterpret_cast<uint32_t*>(cnt);
-        for (uint32_t i = threadIdx.x; i < kBigWarps * Bp / 2; i += kBigThreads) cz[i] = 0;
+        for (uint32_t k = threadIdx.x; k < kWarps * Bp / 2; k += kThreads) cz[k] = 0;
     }
     uint32_t grun[8];
 #pragma unroll
@@ -247,67 +270,80 @@ __global__ void __launch_bounds__(kBigThreads, 1) k_scatter_idx_b(const uint4* _
     }
     __syncthreads();
 
-    for (uint32_t base = 0; base < n; base += kBigQ) {
-        const uint32_t nq = min((uint32_t)kBigQ, n - base);
-        uint32_t packed[kBigRounds];
+    for (uint32_t i = 0; i < n; ++i) {
+        const uint32_t count = keyed_tile(aos_in, n_rec, t0 + i).count;
+        const uint32_t* raw = ring + (i & 1u) * (kTile * 8);
+        const uint4* s_rec = reinterpret_cast<const uint4*>(raw);
+        mbar_wait(&bar[i & 1u], (i >> 1) & 1u);
+        uint32_t packed[kRounds];  // bucket << 9 | rank
 #pragma unroll
-        for (int r = 0; r < kBigRounds; ++r) packed[r] = kNone;
-        const uint32_t q = w / (kBigWarps / kBigQ);
-        if (q < nq) {
-            const uint32_t i = base + q;
-            const TileDesc td = s_desc[i % kIdxBStages];
-            mbar_wait(&bars[i % kIdxBStages], (i / kIdxBStages) & 1u);
-            const uint32_t* raw = stage_ptr(i);
-            const uint32_t first = (w % (kBigWarps / kBigQ)) * kBigSpan;
+        for (int r = 0; r < kRounds; ++r) {
+            const uint32_t idx = w * kWarpSpan + r * 32 + lane_id();
+            packed[r] = idx < count ? (raw[idx * 8] >> lo_bits) : kNone;
+        }
 #pragma unroll
-            for (int r = 0; r < kBigRounds; ++r) {
-                const uint32_t idx = first + r * 32 + lane_id();
-                packed[r] = idx < td.count ? (raw[idx * 8] >> lo_bits) : kNone;
-            }
-#pragma unroll
-            for (int r = 0; r < kBigRounds; ++r) {
-                uint32_t bucket = packed[r];
-                uint32_t rank = warp_rank(bucket, cnt + w * Bp);
-                packed[r] = bucket == kNone ? kNone : ((bucket << 9) | rank);
-            }
+        for (int r = 0; r < kRounds; ++r) {
+            uint32_t bucket = packed[r];
+            uint32_t rank = warp_rank(bucket, cnt + w * Bp);
+            packed[r] = bucket == kNone ? kNone : ((bucket << 9) | rank);
         }
         __syncthreads();
-        const uint32_t n_part = finish_ranks<true, kBigWarps>(cnt, B, Bp, gcur, lstart, misc, grun);
-
+        finish_ranks<false>(cnt, B, Bp, run, nullptr, misc, grun);
 #pragma unroll
-        for (int r = 0; r < kBigRounds; ++r) {
+        for (int r = 0; r < kRounds; ++r) {
+            uint32_t dest = kNone;
             if (packed[r] != kNone) {
-                uint32_t bucket = packed[r] >> 9, rank = packed[r] & 511u;
-                uint32_t rel = cnt[w * Bp + bucket] + rank;
-                uint32_t p = lstart[bucket] + rel;
-                perm[p] = (uint16_t)(w * kBigSpan + r * 32 + lane_id());
-                pdest[p] = gcur[bucket] + rel;
+                const uint32_t bucket = packed[r] >> 9;
+                dest = run[bucket] + cnt[w * Bp + bucket] + (packed[r] & 511u);
+            }
+            sdest[w * kWarpSpan + r * 32 + lane_id()] = dest;
+        }
+        __syncwarp();
+        {
+            const uint32_t half = lane_id() & 1u;
+#pragma unroll 4
+            for (int it = 0; it < kWarpSpan / 16; ++it) {
+                const uint32_t idx = w * kWarpSpan + it * 16 + (lane_id() >> 1);
+                const uint32_t dest = sdest[idx];
+                if (dest != kNone) aos_out[2 * (size_t)dest + half] = s_rec[2 * idx + half];
             }
         }
         __syncwarp();
         zero_row(cnt + w * Bp, Bp);
         __syncthreads();
-
-        for (uint32_t j = threadIdx.x; j < n_part; j += kBigThreads) {
-            const uint32_t irec = perm[j];
-            const uint32_t dest = pdest[j];
-            const uint4* s_rec = reinterpret_cast<const uint4*>(stage_ptr(base + irec / kTile)) + 2 * (irec % kTile);
-            const uint4 a = s_rec[0], b = s_rec[1];
-            out.key[dest] = a.x;
-            out.E[dest] = __uint_as_float(a.y);
-            out.x[dest] = __uint_as_float(a.z);
-            out.y[dest] = __uint_as_float(a.w);
-            out.u[dest] = __uint_as_float(b.x);
-            out.v[dest] = __uint_as_float(b.y);
-            out.wt[dest] = __uint_as_float(b.z);
-            out.src[dest] = b.w;
-        }
-        __syncthreads();
-        if (threadIdx.x == 0)
-            for (uint32_t k = 0; k < nq; ++k)
-                if (base + kIdxBStages + k < n) issue(base + kIdxBStages + k);
-        __syncthreads();  // the next tile reads descriptors just written
+        if (threadIdx.x == 0 && i + 2 < n) issue(i + 2);
     }
+}
+
+// The bare index as SoA arrays (psl_build_batches with beam == NULL): a streaming transpose of the keyed records.
+__global__ void __launch_bounds__(256) k_index_to_soa(const uint4* __restrict__ aos, const uint32_t* __restrict__ n_ptr, IdxOut out)
+{
+    const uint32_t n = *n_ptr;
+    for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const uint4 a = __ldg(aos + 2 * (size_t)i), b = __ldg(aos + 2 * (size_t)i + 1);
+        out.E[i] = __uint_as_float(a.y);
+        out.x[i] = __uint_as_float(a.z);
+        out.y[i] = __uint_as_float(a.w);
+        out.u[i] = __uint_as_float(b.x);
+        out.v[i] = __uint_as_float(b.y);
+        out.wt[i] = __uint_as_float(b.z);
+        out.src[i] = b.w;
+    }
+}
+
+// offsets[k] = number of index slots whose key is < k (binary search over the sorted keyed records; k = 0..K)
+__global__ void k_offsets_by_search_keyed(const uint4* __restrict__ aos, const uint32_t* __restrict__ n_ptr, uint32_t K,
+                                          uint32_t* __restrict__ offsets)
+{
+    uint32_t k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k > K) return;
+    const uint32_t* keys = reinterpret_cast<const uint32_t*>(aos);
+    uint32_t lo = 0, hi = *n_ptr;
+    while (lo < hi) {
+        uint32_t mid = lo + ((hi - lo) >> 1);
+        if (__ldg(keys + 8 * (size_t)mid) < k) lo = mid + 1; else hi = mid;
+    }
+    offsets[k] = lo;
 }
 
 }  // namespace psl
