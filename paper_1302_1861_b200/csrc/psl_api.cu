@@ -727,7 +727,7 @@ psl_status build_beam_from_index(psl_ctx* ctx, const psl_beam* beam, const DevBe
         in.aos = at<uint4>(ctx, L.aos_index);
         {
             Prof prof(ctx, PSL_K_BEAM);
-            k_beam_compact<<<nt, kThreads, 11 * kBeamTile * 4, ctx->stream>>>(st, in, ctx->grid, bm, soa_out(ctx, L.beam_out), beam_keys,
+            k_beam_compact<<<nt, kThreads, 0, ctx->stream>>>(st, in, ctx->grid, bm, soa_out(ctx, L.beam_out), beam_keys,
                                                                          at<unsigned long long>(ctx, L.lookback),
                                                                          scalar(ctx, SC_TILE_COUNTER), at<BeamTileStats>(ctx, L.bstats),
                                                                          scalar(ctx, SC_BEAM_NSURV));
@@ -917,7 +917,6 @@ psl_status psl_create(const psl_config* cfg, psl_ctx** out)
         CUC(allow_smem(scatter_idx_a_fn(pos, edges), ctx->sm_idx_a));
         CUC(allow_smem(k_count_keys, ctx->sm_count_b));
         CUC(allow_smem(k_scatter_idx_b, ctx->sm_idx_b));
-        CUC(allow_smem(k_beam_compact, 11 * kBeamTile * 4));
         CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, scatter_idx_a_fn(pos, edges), kThreads, ctx->sm_idx_a));
         ctx->S_a = width(occ);
         CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_scatter_idx_b, kThreads, ctx->sm_idx_b));

@@ -56,18 +56,20 @@ constexpr int kBeamTile = 2048;                       // index records one CTA o
 constexpr int kBeamRounds = kBeamTile / kThreads;      // 8
 constexpr int kBeamArrays = 12;  // E x y u v w wt xp yp src key + spare
 
-__global__ void __launch_bounds__(kThreads) k_beam_compact(SegTable seg, IdxIn in, const __grid_constant__ DevGrid g,
-                                                          const __grid_constant__ DevBeam bm, SoAOut out,
-                                                          uint32_t* __restrict__ out_key,
-                                                          unsigned long long* __restrict__ tile_state,
-                                                          uint32_t* __restrict__ tile_counter,
-                                                          BeamTileStats* __restrict__ bstats,
-                                                          uint32_t* __restrict__ n_surv_out)
+__global__ void __launch_bounds__(kThreads, 2) k_beam_compact(SegTable seg, IdxIn in, const __grid_constant__ DevGrid g,
+                                                             const __grid_constant__ DevBeam bm, SoAOut out,
+                                                             uint32_t* __restrict__ out_key,
+                                                             unsigned long long* __restrict__ tile_state,
+                                                             uint32_t* __restrict__ tile_counter,
+                                                             BeamTileStats* __restrict__ bstats,
+                                                             uint32_t* __restrict__ n_surv_out)
 {
-    extern __shared__ __align__(128) uint8_t smem[];
-    uint32_t* stage = reinterpret_cast<uint32_t*>(smem);  // [11][kBeamTile]
-    __shared__ uint32_t s_wc[2][kWarps];
-    __shared__ uint32_t s_ctl[4];  // tile, seg_first, seg_last, exclusive prefix
+    // Two phases, no shared-memory staging: (1) every thread loads its 8 records of the tile (16 independent
+    // 16-byte loads in flight), applies jaws / map / MU weight and keeps the results in registers;
+    // (2) after the tile's first output slot is known (look-back), survivors are stored straight from
+    // registers -- compaction is monotonic, so consecutive kept lanes write consecutive slots.
+    __shared__ uint32_t s_cnt[kBeamRounds * kWarps];  // survivors per (round, warp), then their exclusive prefix
+    __shared__ uint32_t s_ctl[5];                     // tile, seg_first, seg_last, first output slot, survivors
     __shared__ double s_d[kWarps];
     __shared__ uint32_t s_z[kWarps];
 
@@ -82,66 +84,58 @@ __global__ void __launch_bounds__(kThreads) k_beam_compact(SegTable seg, IdxIn i
     __syncthreads();
     const uint32_t s_first = s_ctl[1], s_last = s_ctl[2];
 
-    uint32_t run = 0, n_zero = 0;
-    double sum_out = 0.0;
-#pragma unroll 1
-    for (int r = 0; r < kBeamRounds; ++r) {
-        uint32_t lv = r * kThreads + threadIdx.x;
-        bool keep = false;
-        float E = 0, x = 0, y = 0, u = 0, v = 0, wz = 0, wt = 0, xm = 0, ym = 0;
-        uint32_t srci = 0, key = 0;
-        if (lv < cnt) {
-            uint32_t vv = v0 + lv;
-            uint32_t sg = seg_of(seg.vstart, s_first, s_last, vv);
-            uint32_t p = __ldg(seg.src + sg) + (vv - __ldg(seg.vstart + sg));
-            const uint4 ra = __ldg(in.aos + 2 * (size_t)p), rb = __ldg(in.aos + 2 * (size_t)p + 1);
-            E = __uint_as_float(ra.y); x = __uint_as_float(ra.z); y = __uint_as_float(ra.w);
-            u = __uint_as_float(rb.x); v = __uint_as_float(rb.y);
-            float wt0 = __uint_as_float(rb.z);
-            srci = rb.w;
-            key = ra.x;  // the full key travels with the record
-            float q = q_of(u, v), tx, ty;
-            slopes(u, v, q, wz, tx, ty);
-            keep = !(bm.has_jaws) || jaw_pass(bm, x, y, tx, ty);
-            xm = __fadd_rn(x, __fmul_rn(tx, bm.dzM));
-            ym = __fadd_rn(y, __fmul_rn(ty, bm.dzM));
-            wt = final_weight(bm, wt0, xm, ym);
-            if (keep && bm.drop_zero && wt == 0.0f) {
-                keep = false;
-                n_zero += 1;
-            }
-        }
-        uint32_t ballot = __ballot_sync(0xFFFFFFFFu, keep);
-        if (lane_id() == 0) s_wc[r & 1][w] = __popc(ballot);
-        __syncthreads();
-        uint32_t pre = 0, tot = 0;
+    uint4 ra[kBeamRounds], rb[kBeamRounds];
+    bool have[kBeamRounds];
 #pragma unroll
-        for (int k = 0; k < kWarps; ++k) {
-            uint32_t c = s_wc[r & 1][k];
-            pre += (k < (int)w) ? c : 0u;
-            tot += c;
+    for (int r = 0; r < kBeamRounds; ++r) {
+        const uint32_t lv = r * kThreads + threadIdx.x;
+        have[r] = lv < cnt;
+        ra[r] = make_uint4(0, 0, 0, 0);
+        rb[r] = make_uint4(0, 0, 0, 0);
+        if (have[r]) {
+            const uint32_t vv = v0 + lv;
+            const uint32_t sg = s_first == s_last ? s_first : seg_of(seg.vstart, s_first, s_last, vv);
+            const uint32_t p = __ldg(seg.src + sg) + (vv - __ldg(seg.vstart + sg));
+            ra[r] = __ldg(in.aos + 2 * (size_t)p);
+            rb[r] = __ldg(in.aos + 2 * (size_t)p + 1);
         }
-        if (keep) {
-            uint32_t pos = run + pre + __popc(ballot & lanemask_lt());
-            stage[0 * kBeamTile + pos] = __float_as_uint(E);
-            stage[1 * kBeamTile + pos] = __float_as_uint(x);
-            stage[2 * kBeamTile + pos] = __float_as_uint(y);
-            stage[3 * kBeamTile + pos] = __float_as_uint(u);
-            stage[4 * kBeamTile + pos] = __float_as_uint(v);
-            stage[5 * kBeamTile + pos] = __float_as_uint(wz);
-            stage[6 * kBeamTile + pos] = __float_as_uint(wt);
-            stage[7 * kBeamTile + pos] = __float_as_uint(xm);
-            stage[8 * kBeamTile + pos] = __float_as_uint(ym);
-            stage[9 * kBeamTile + pos] = srci;
-            stage[10 * kBeamTile + pos] = key;
-            sum_out += (double)wt;
-        }
-        run += tot;
     }
-    const uint32_t total = run;
+    float wz[kBeamRounds], wt[kBeamRounds], xm[kBeamRounds], ym[kBeamRounds];
+    uint32_t pre[kBeamRounds];
+    uint32_t keepbits = 0, n_zero = 0;
+    double sum_out = 0.0;
+#pragma unroll
+    for (int r = 0; r < kBeamRounds; ++r) {
+        const float x = __uint_as_float(ra[r].z), y = __uint_as_float(ra[r].w);
+        const float u = __uint_as_float(rb[r].x), v = __uint_as_float(rb[r].y);
+        const float q = q_of(u, v);
+        float tx, ty;
+        slopes(u, v, q, wz[r], tx, ty);
+        bool keep = have[r] && (!(bm.has_jaws) || jaw_pass(bm, x, y, tx, ty));
+        xm[r] = __fadd_rn(x, __fmul_rn(tx, bm.dzM));
+        ym[r] = __fadd_rn(y, __fmul_rn(ty, bm.dzM));
+        wt[r] = have[r] ? final_weight(bm, __uint_as_float(rb[r].z), xm[r], ym[r]) : 0.0f;
+        if (keep && bm.drop_zero && wt[r] == 0.0f) {
+            keep = false;
+            n_zero += 1;
+        }
+        const uint32_t ballot = __ballot_sync(0xFFFFFFFFu, keep);
+        if (lane_id() == 0) s_cnt[r * kWarps + w] = __popc(ballot);
+        pre[r] = __popc(ballot & lanemask_lt());
+        if (keep) {
+            keepbits |= 1u << r;
+            sum_out += (double)wt[r];
+        }
+    }
+    __syncthreads();
 
-    // decoupled look-back (warp 0): exclusive prefix of `total` over the tiles before this one
+    // warp 0: exclusive prefix of the 64 (round, warp) counts, then the decoupled look-back over tile aggregates
     if (w == 0) {
+        const uint32_t a = s_cnt[2 * lane_id()], b = s_cnt[2 * lane_id() + 1];
+        const uint32_t inc = warp_incl_scan(a + b);
+        s_cnt[2 * lane_id()] = inc - a - b;
+        s_cnt[2 * lane_id() + 1] = inc - b;
+        const uint32_t total = __shfl_sync(0xFFFFFFFFu, inc, 31);
         uint32_t excl = 0;
         if (tile == 0) {
             if (lane_id() == 0) atomicExch(&tile_state[0], kFlagInclusive | (unsigned long long)total);
@@ -169,6 +163,7 @@ __global__ void __launch_bounds__(kThreads) k_beam_compact(SegTable seg, IdxIn i
         }
         if (lane_id() == 0) {
             s_ctl[3] = excl;
+            s_ctl[4] = total;
             if (v0 + cnt == seg.M) *n_surv_out = excl + total;  // last tile
         }
     }
@@ -181,25 +176,27 @@ __global__ void __launch_bounds__(kThreads) k_beam_compact(SegTable seg, IdxIn i
     __syncthreads();
     const uint32_t gbase = s_ctl[3];
 
-    // coalesced copy-out of the tile's survivors
-    for (uint32_t j = threadIdx.x; j < total; j += kThreads) {
-        size_t d = (size_t)gbase + j;
-        out.E[d] = __uint_as_float(stage[0 * kBeamTile + j]);
-        out.x[d] = __uint_as_float(stage[1 * kBeamTile + j]);
-        out.y[d] = __uint_as_float(stage[2 * kBeamTile + j]);
-        out.u[d] = __uint_as_float(stage[3 * kBeamTile + j]);
-        out.v[d] = __uint_as_float(stage[4 * kBeamTile + j]);
-        out.w[d] = __uint_as_float(stage[5 * kBeamTile + j]);
-        out.wt[d] = __uint_as_float(stage[6 * kBeamTile + j]);
-        if (bm.out_proj) {
-            out.xp[d] = __uint_as_float(stage[7 * kBeamTile + j]);
-            out.yp[d] = __uint_as_float(stage[8 * kBeamTile + j]);
+#pragma unroll
+    for (int r = 0; r < kBeamRounds; ++r) {
+        if (keepbits & (1u << r)) {
+            const size_t d = (size_t)gbase + s_cnt[r * kWarps + w] + pre[r];
+            out.E[d] = __uint_as_float(ra[r].y);
+            out.x[d] = __uint_as_float(ra[r].z);
+            out.y[d] = __uint_as_float(ra[r].w);
+            out.u[d] = __uint_as_float(rb[r].x);
+            out.v[d] = __uint_as_float(rb[r].y);
+            out.w[d] = wz[r];
+            out.wt[d] = wt[r];
+            if (bm.out_proj) {
+                out.xp[d] = xm[r];
+                out.yp[d] = ym[r];
+            }
+            out.src[d] = rb[r].w;
+            out_key[d] = ra[r].x;
         }
-        out.src[d] = stage[9 * kBeamTile + j];
-        out_key[d] = stage[10 * kBeamTile + j];
     }
     if (threadIdx.x == 0) {
-        BeamTileStats bs = {0, total, 0.0};
+        BeamTileStats bs = {0, s_ctl[4], 0.0};
         for (int k = 0; k < kWarps; ++k) {
             bs.sum_out += s_d[k];
             bs.n_zero += s_z[k];
