@@ -1,15 +1,14 @@
 // psl_index.cuh -- the one-off sort behind the PSL index (paper method 3): two stable LSD
-// passes over the full key, split as key = hi * 2^s + lo with hi < 256 and lo < 8192.
+// passes over the full key, split into two balanced digits key = hi * 2^s + lo (each <= 2048 buckets).
 //
-// What shapes these kernels on B200 is the rate of distinct 128-byte lines the stores touch (about 35 G
-// line-writes/s chip-wide), not bytes:
-//   pass A (by lo, up to 8192 buckets = the position bins): a tile of 1024 records has about one record per
-//     bucket, so no staging can make runs; every record is written once as ONE full 32-byte sector
-//     {key, E, x, y, u, v, wt, src} by a pair of lanes (one request per record).  Ranks need no per-warp
-//     counter matrix: the CTA keeps the running first free slot of every bucket of its segment in shared
-//     memory and one warp walks the tile's keys in input order (__match_any_sync per 32 keys).
-//   pass B (by hi, <= 256 buckets = type x energy): the 4096-record-tile staged scatter of psl_bigtile.cuh
-//     on keyed input, SoA out -- runs of tens of records per key and tile.
+//   pass A: raw 28-byte records -> 32-byte keyed records {key, E, x, y, u, v, wt, src}, stably partitioned by lo
+//   pass B: keyed records -> the index: keyed records sorted by the full key (stable partition by hi)
+//
+// With ~1100 buckets and 1024-record tiles a tile holds about one record per bucket, so there are no runs to
+// stage: every record is written once as ONE full 32-byte sector by a pair of lanes (one request per sector;
+// measured on B200: 35 G sectors/s against 17.7 G/s when a thread writes the two halves itself, DESIGN.md
+// "Kernels").  Ranks: per-warp private uint16 counters + __match_any_sync, a 16-byte-vector scan over the 8
+// warps, the running first free slot of every bucket kept in registers (thread t owns buckets 8t..8t+7).
 #pragma once
 
 #include "psl_bigtile.cuh"

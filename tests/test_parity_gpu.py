@@ -310,3 +310,82 @@ def test_config2_full_size_element_by_element():
     w = W.config(2)
     r = w.records()
     check(w, r, None, chunk=w.chunk_records, mem="device")
+
+
+# ---------------------------------------------------------------------------------------------
+# kernel-structure cases: stage rings that wrap, tiles that straddle nothing but are ragged, sources TMA cannot
+# copy, both ONTHEFLY tile sizes, the INDEX digit split near its limits
+# ---------------------------------------------------------------------------------------------
+def test_big_tiles_ragged_chunks_and_ring_wraparound():
+    """config-2 keys (192 <= 256: the 4096-record-tile scatter); chunks of 3000 records leave a ragged 952-record
+    ring stage after every two full ones, and 2.4e6 records give every persistent CTA several big tiles, so ring
+    stages and their barriers are reused with both parities."""
+    w = W.config(2, 2_400_000)
+    r = dirty(w.records(), 7)
+    check(w, r, None, chunk=3000 * 40, mem="device")
+    w_small = W.config(2, 70_001)
+    check(w_small, dirty(w_small.records(), 8), None, chunk=3000, mem="device")
+
+
+def test_small_tiles_with_a_rejecting_beam_at_scale():
+    """a beam with jaws takes the 1024-record-tile scatter (two CTAs per SM); several tiles per CTA"""
+    w = W.config(3, 1_500_000)
+    check(w, w.records(), w.beams[0], chunk=500_000, mem="device", flags=P().OUT_PROJ, proj=True)
+
+
+def test_unaligned_device_source_takes_the_manual_stage_fill():
+    """a DEVICE chunk that is only 4-byte aligned cannot be bulk-copied: every stage is fetched by the threads"""
+    import torch
+
+    p = P()
+    w = W.config(2, 20_000)
+    r = w.records()
+    raw = np.ascontiguousarray(r).view(np.uint8).reshape(-1)
+    buf = torch.empty(len(raw) + 4, dtype=torch.uint8, device="cuda")
+    buf[4:].copy_(torch.from_numpy(raw.copy()))
+    for grid, beam in ((w.grid, None), (W.config(3, 1).grid, W.config(3, 1).beams[0])):
+        ctx = p.PslContext(grid, w.geometry, w.mode, max_records=len(r))
+        ctx.load_chunk(buf[4:], p.MEM_DEVICE)
+        ctx.build_batches(beam)
+        assert_matches_oracle(library_result(ctx), O.Oracle(grid, w.geometry).build(r, beam))
+        ctx.destroy()
+    w4 = W.config(4, 20_000)
+    ctx = p.PslContext(w4.grid, w4.geometry, w4.mode, max_records=len(r))
+    r4 = w4.records()
+    buf[4:].copy_(torch.from_numpy(np.ascontiguousarray(r4).view(np.uint8).reshape(-1).copy()))
+    ctx.load_chunk(buf[4:], p.MEM_DEVICE)
+    ctx.build_batches(w4.beams[0])
+    assert_matches_oracle(library_result(ctx), O.Oracle(w4.grid, w4.geometry).build(r4, w4.beams[0]))
+    ctx.destroy()
+
+
+def test_index_at_scale_many_segments_then_bare_index_and_beam():
+    """3e6 records: every persistent CTA of both INDEX passes owns several tiles; the bare index (SoA view made
+    on demand from the keyed records) and a beam build from the same index"""
+    w = W.config(4, 3_000_000)
+    r = dirty(w.records(), 11)
+    ctx = run_library(w, r, None, chunk=1_000_000, mem="device")
+    orc = O.Oracle(w.grid, w.geometry)
+    assert_matches_oracle(library_result(ctx), orc.build(r, None), index_only=True)
+    ctx.build_batches(w.beams[0])
+    assert_matches_oracle(library_result(ctx), orc.build(r, w.beams[0]))
+    ctx.build_batches(None)  # back to the bare index: the view is still valid
+    assert_matches_oracle(library_result(ctx), orc.build(r, None), index_only=True)
+    ctx.destroy()
+
+
+def test_index_digit_split_extremes():
+    """few keys (one digit does all the work) and close to the 2048 x 2048 limit"""
+    w = W.config(4, 40_000)
+    tiny = dict(w.grid, n_ebins=1, n_xbins=2, n_ybins=2, x_min=-20.0, dx=20.0, y_min=-20.0, dy=20.0)  # 12 keys
+    wt = W.Workload("idx_tiny", w.n_records, w.gen, w.mode, tiny)
+    r = wt.records()
+    ctx = run_library(wt, r, None)
+    assert_matches_oracle(library_result(ctx), O.Oracle(tiny, w.geometry).build(r, None), index_only=True)
+    ctx.destroy()
+    huge = dict(w.grid, n_ebins=100, n_xbins=100, n_ybins=100, x_min=-20.0, dx=0.4, y_min=-20.0, dy=0.4)  # 3e6 keys
+    wh = W.Workload("idx_huge", w.n_records, w.gen, w.mode, huge)
+    beam = W.make_beam(jaws=(-8, 8, -8, 8), roi=(-5, 5, -5, 5))
+    ctx = run_library(wh, r, beam)
+    assert_matches_oracle(library_result(ctx), O.Oracle(huge, w.geometry).build(r, beam))
+    ctx.destroy()
