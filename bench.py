@@ -381,6 +381,7 @@ def run_ours(args):
         pass
     roofline = {"bound": "hbm", "kernel": dom, "achieved": d["gbs"], "peak": peak, "unit": "GB/s",
                 "frac": d["gbs"] / peak, "peak_source": peak_src,
+                "frac_of_nominal_8000": d["gbs"] / 8000.0,  # also against the nominal ~8 TB/s
                 "bytes_per_launch": d["algorithmic_bytes_per_step"] / d["launches_per_step"],
                 "avg_launch_ms": d["avg_launch_ms"], "traffic": traffic,
                 "step_frac": sum(k["algorithmic_bytes_per_step"] for k in kernels.values() if "gbs" in k)

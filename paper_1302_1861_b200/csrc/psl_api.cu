@@ -573,7 +573,6 @@ IdxOut idx_out(psl_ctx* ctx)
     o.E = at<float>(ctx, L.idx[0]); o.x = at<float>(ctx, L.idx[1]); o.y = at<float>(ctx, L.idx[2]);
     o.u = at<float>(ctx, L.idx[3]); o.v = at<float>(ctx, L.idx[4]); o.wt = at<float>(ctx, L.idx[5]);
     o.src = at<uint32_t>(ctx, L.idx[6]);
-    o.key = nullptr;
     return o;
 }
 

@@ -15,9 +15,9 @@
 // the output is the unique stable order, bit-identical from run to run.
 //
 // ONTHEFLY (paper methods 1/2): one pass, bucket = the (type, energy) key, raw 28-byte
-// records in, transport-ready SoA out.  INDEX (method 3): two LSD passes over the full
-// (type, energy, y, x) key split as key = hi * 2^s + lo: pass A (raw -> 32-byte keyed records, by lo), pass
-// B (keyed records -> SoA index, by hi).
+// records in, transport-ready SoA out (this file: 1024-record tiles; psl_bigtile.cuh: 4096-record tiles).
+// INDEX (method 3): two LSD passes over the full (type, energy, y, x) key, psl_index.cuh;
+// they share the histogram, scan and ranking code below.
 #pragma once
 
 #include "psl_device.cuh"
@@ -37,10 +37,9 @@ struct SoAOut {
     uint32_t* src;
 };
 
-struct IdxOut {
+struct IdxOut {  // SoA view of the bare index
     float *E, *x, *y, *u, *v, *wt;
     uint32_t* src;
-    uint32_t* key;
 };
 
 // which tiles a launch covers and which table columns its CTAs own: CTA s of the launch (gridDim.x CTAs)
