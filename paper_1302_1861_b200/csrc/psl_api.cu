@@ -16,6 +16,7 @@
 #include "psl_beam.cuh"
 #include "psl_bigtile.cuh"
 #include "psl_index.cuh"
+#include "psl_index_big.cuh"
 #include "psl_device.cuh"
 #include "psl_partition.cuh"
 
@@ -26,6 +27,7 @@ namespace {
 thread_local char g_err[256] = "";
 
 constexpr uint64_t kAlign = 256;
+constexpr uint32_t kIdxSplit = 2;  // INDEX: one scatter CTA per SM, two histogram CTAs (= table columns) per segment
 constexpr uint64_t kScanSmallMax = 131072;  // table entries the single-CTA scan takes
 constexpr uint64_t kStageBytes = 32ull << 20;  // pinned staging buffers for pageable sources (two of them)
 
@@ -250,6 +252,15 @@ ScatterOtfFn scatter_big_fn(bool pos, bool edges, int beam, bool proj)
     return pos ? (edges ? scatter_big_pe<true, true>(beam, proj) : scatter_big_pe<true, false>(beam, proj))
                : (edges ? scatter_big_pe<false, true>(beam, proj) : scatter_big_pe<false, false>(beam, proj));
 }
+using ScatterIdxBigFn = void (*)(const ChunkDesc*, uint32_t, Span, const uint4*, const uint32_t*, DevGrid, DevBeam, uint32_t, uint32_t,
+                                 const uint32_t*, uint32_t, uint4*);
+// the 4096-record-tile INDEX passes: A (raw records in) per grid features, B (keyed records in)
+ScatterIdxBigFn scatter_idx_big_a_fn(bool pos, bool edges)
+{
+    return pos ? (edges ? k_scatter_idx_big<false, true, true> : k_scatter_idx_big<false, true, false>)
+               : (edges ? k_scatter_idx_big<false, false, true> : k_scatter_idx_big<false, false, false>);
+}
+ScatterIdxBigFn scatter_idx_big_b_fn() { return k_scatter_idx_big<true, false, false>; }
 ScatterIdxAFn scatter_idx_a_fn(bool pos, bool edges)
 {
     return pos ? (edges ? k_scatter_idx_a<true, true> : k_scatter_idx_a<true, false>)
@@ -605,8 +616,8 @@ psl_status finalize_index(psl_ctx* ctx)
         {
             Prof prof(ctx, PSL_K_INDEX_A);
             for (const psl_ctx::ChunkLaunch& cl : ctx->idx_launches) {  // the same segments the counts were taken on
-                scatter_idx_a_fn(ctx->grid.has_pos != 0, ctx->grid.ebin_mode != 0)<<<cl.n_seg, kThreads, ctx->sm_idx_a, ctx->stream>>>(
-                    chunks, ctx->n_chunks, cl.span, ctx->grid, none, d.B_lo, d.lo_bits, table_a, d.cols_cap, aos);
+                scatter_idx_big_a_fn(ctx->grid.has_pos != 0, ctx->grid.ebin_mode != 0)<<<cl.n_seg, kThreads, ctx->sm_idx_a, ctx->stream>>>(
+                    chunks, ctx->n_chunks, cl.span, nullptr, nullptr, ctx->grid, none, d.B_lo, d.lo_bits, table_a, d.cols_cap, aos);
                 LAUNCHED();
             }
         }
@@ -615,22 +626,24 @@ psl_status finalize_index(psl_ctx* ctx)
         const uint32_t Sb = ntb < ctx->S_b ? ntb : ctx->S_b;
         {
             Prof prof(ctx, PSL_K_COUNT);
-            k_count_keys<<<Sb, kThreads, ctx->sm_count_b, ctx->stream>>>(aos, scalar(ctx, SC_NIDX), d.B_hi, d.lo_bits, table_b, kMaxSegments);
+            k_count_keys<<<Sb * kIdxSplit, kThreads, ctx->sm_count_b, ctx->stream>>>(aos, scalar(ctx, SC_NIDX), d.B_hi, d.lo_bits, table_b,
+                                                                                     kMaxSegments, kIdxSplit);
             LAUNCHED();
         }
-        if ((uint64_t)d.B_hi * Sb <= kScanSmallMax) {
+        if ((uint64_t)d.B_hi * Sb * kIdxSplit <= kScanSmallMax) {
             Prof prof(ctx, PSL_K_SCAN);
-            k_scan_small<<<1, 1024, 0, ctx->stream>>>(table_b, Sb, kMaxSegments, d.B_hi, scalar(ctx, SC_TOTAL), 0, nullptr, nullptr, 1,
-                                                      0, nullptr);
+            k_scan_small<<<1, 1024, 0, ctx->stream>>>(table_b, Sb * kIdxSplit, kMaxSegments, d.B_hi, scalar(ctx, SC_TOTAL), 0, nullptr, nullptr,
+                                                      1, 0, nullptr);
             LAUNCHED();
         } else {
-            s = run_scan(ctx, table_b, d.B_hi, Sb, kMaxSegments, scalar(ctx, SC_TOTAL));
+            s = run_scan(ctx, table_b, d.B_hi, Sb * kIdxSplit, kMaxSegments, scalar(ctx, SC_TOTAL));
             if (s != PSL_OK) return s;
         }
         {
             Prof prof(ctx, PSL_K_INDEX_B);
-            k_scatter_idx_b<<<Sb, kThreads, ctx->sm_idx_b, ctx->stream>>>(aos, scalar(ctx, SC_NIDX), d.B_hi, d.lo_bits, table_b,
-                                                                         kMaxSegments, at<uint4>(ctx, L.aos_index));
+            const Span spb = {0u, 0u, 0u, kIdxSplit};
+            scatter_idx_big_b_fn()<<<Sb, kThreads, ctx->sm_idx_b, ctx->stream>>>(nullptr, 0, spb, aos, scalar(ctx, SC_NIDX), ctx->grid, none, d.B_hi,
+                                                                                d.lo_bits, table_b, kMaxSegments, at<uint4>(ctx, L.aos_index));
             LAUNCHED();
         }
         k_offsets_by_search_keyed<<<(d.K + 1 + 255) / 256, 256, 0, ctx->stream>>>(at<uint4>(ctx, L.aos_index), scalar(ctx, SC_NIDX), d.K, idx_offsets);
@@ -908,17 +921,17 @@ psl_status psl_create(const psl_config* cfg, psl_ctx** out)
     } else {
         ctx->count_stages = d.B_lo * 4 > 8192 ? 2 : kStagesCount;
         ctx->sm_count_raw = count_layout(kTile * kRecBytes, ctx->count_stages, d.B_lo, ne).total;
-        ctx->sm_idx_a = idx_a_layout(d.B_lo, ne).total;
+        ctx->sm_idx_a = idx_big_layout(false, d.B_lo, ne).total;
         ctx->sm_count_b = count_layout(0, 0, d.B_hi, 0).total;
-        ctx->sm_idx_b = idx_b_layout(d.B_hi).total;
+        ctx->sm_idx_b = idx_big_layout(true, d.B_hi, ne).total;  // same layout call as in the kernel
         const bool pos = d.n_pos > 1, edges = cfg->ebin_mode == PSL_EBIN_EDGES;
         CUC(allow_smem(count_idx_fn(pos, edges), ctx->sm_count_raw));
-        CUC(allow_smem(scatter_idx_a_fn(pos, edges), ctx->sm_idx_a));
+        CUC(allow_smem(scatter_idx_big_a_fn(pos, edges), ctx->sm_idx_a));
         CUC(allow_smem(k_count_keys, ctx->sm_count_b));
-        CUC(allow_smem(k_scatter_idx_b, ctx->sm_idx_b));
-        CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, scatter_idx_a_fn(pos, edges), kThreads, ctx->sm_idx_a));
+        CUC(allow_smem(scatter_idx_big_b_fn(), ctx->sm_idx_b));
+        CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, scatter_idx_big_a_fn(pos, edges), kThreads, ctx->sm_idx_a));
         ctx->S_a = width(occ);
-        CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_scatter_idx_b, kThreads, ctx->sm_idx_b));
+        CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, scatter_idx_big_b_fn(), kThreads, ctx->sm_idx_b));
         ctx->S_b = width(occ);
     }
     CUC(cudaStreamSynchronize(ctx->stream));
@@ -1017,16 +1030,16 @@ psl_status psl_load_chunk(psl_ctx* ctx, const void* records, uint64_t n, int32_t
         DevBeam none;
         memset(&none, 0, sizeof none);
         psl_ctx::ChunkLaunch cl;
-        cl.span = {tile0, nt, ctx->n_cols, 1u};
+        cl.span = {tile0, nt, ctx->n_cols, kIdxSplit};
         cl.n_seg = nt < ctx->S_a ? nt : ctx->S_a;
-        if (ctx->n_cols + cl.n_seg > ctx->d.cols_cap) { set_err(ctx->err, "load_chunk: out of table columns"); return PSL_ERR_CAPACITY; }
+        if (ctx->n_cols + cl.n_seg * kIdxSplit > ctx->d.cols_cap) { set_err(ctx->err, "load_chunk: out of table columns"); return PSL_ERR_CAPACITY; }
         Prof prof(ctx, PSL_K_COUNT);
-        count_idx_fn(ctx->grid.has_pos != 0, ctx->grid.ebin_mode != 0)<<<cl.n_seg, kThreads, ctx->sm_count_raw, ctx->stream>>>(
+        count_idx_fn(ctx->grid.has_pos != 0, ctx->grid.ebin_mode != 0)<<<cl.n_seg * kIdxSplit, kThreads, ctx->sm_count_raw, ctx->stream>>>(
             chunks, ctx->n_chunks + 1, cl.span, ctx->grid, none, ctx->d.B_lo, (1u << ctx->d.lo_bits) - 1u,
             at<uint32_t>(ctx, ctx->L.table_a), ctx->d.cols_cap, at<SegStats>(ctx, ctx->L.sstats), ctx->count_stages);
         LAUNCHED();
         ctx->idx_launches.push_back(cl);
-        ctx->n_cols += cl.n_seg;
+        ctx->n_cols += cl.n_seg * kIdxSplit;
     }
     ctx->n_records += n;
     if (host) ctx->n_host_records += n;

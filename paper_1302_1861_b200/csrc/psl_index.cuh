@@ -173,16 +173,16 @@ __global__ void __launch_bounds__(kThreads, 3) k_scatter_idx_a(const ChunkDesc* 
 // records.  Reads the key word of every 32-byte record.
 __global__ void __launch_bounds__(kThreads) k_count_keys(const uint4* __restrict__ aos, const uint32_t* __restrict__ n_ptr,
                                                         uint32_t B, uint32_t lo_bits, uint32_t* __restrict__ table,
-                                                        uint32_t stride)
+                                                        uint32_t stride, uint32_t split)
 {
     extern __shared__ __align__(128) uint8_t smem[];
     uint32_t* hist = reinterpret_cast<uint32_t*>(smem);
     const CountSmem L = count_layout(0, 0, B, 0);
     const uint32_t rmask = (1u << L.rlog) - 1u;
     const uint32_t n = *n_ptr;
-    Span sp = {0u, (n + kTile - 1) / kTile, 0u, 1u};
+    Span sp = {0u, (n + kTile - 1) / kTile, 0u, split};
     uint32_t t0, t1;
-    segment_of(sp, t0, t1);
+    split_segment_of(sp, t0, t1);
     for (uint32_t i = threadIdx.x; i < (B << L.rlog); i += kThreads) hist[i] = 0;
     __syncthreads();
     const uint32_t first = t0 * kTile, last = min(n, t1 * (uint32_t)kTile);

@@ -1,0 +1,219 @@
+// psl_index_big.cuh -- INDEX passes A and B with 4096-record tiles and tile-sorted staging.
+//
+// Why: a 32-byte sector that is written by a store request of its own costs the same ~40 G requests/s on
+// B200 whether or not its line is completed later; only a store instruction that covers
+// several consecutive sectors is cheap.  With ~1100 buckets per pass a 4096-record tile holds ~4 records per
+// bucket: ordered by (bucket, input order) inside the tile they form ~128-byte runs, and the lanes of a warp
+// write consecutive 16-byte halves of consecutive slots, so one request covers a whole run.
+//
+// One 256-thread CTA per SM: the tile is 4 ring stages of 1024 records that stay where TMA put them, a fifth
+// stage prefetches.  Warp w owns records [512 w, 512 w + 512) of the tile (half a stage): per-warp private
+// uint16 counters + __match_any_sync give stable ranks, finish_ranks the prefix over the 8 warps.
+#pragma once
+
+#include "psl_index.cuh"
+
+namespace psl {
+
+constexpr int kIdxBigQ = 4;                               // ring stages per tile
+constexpr int kIdxBigTile = kIdxBigQ * kTile;             // 4096 records
+constexpr int kIdxBigStages = 5;
+constexpr int kIdxBigSpan = kIdxBigTile / kWarps;         // 512 records per warp
+constexpr int kIdxBigRounds = kIdxBigSpan / 32;           // 16
+
+struct IdxBigSmem {
+    uint32_t ring, stage_bytes, cnt, gcur, lstart, perm, pbkt, skey, edges, misc, desc, bars, total;
+};
+
+__host__ __device__ inline IdxBigSmem idx_big_layout(bool keyed, uint32_t B, uint32_t n_edges)
+{
+    IdxBigSmem L;
+    uint32_t p = 0;
+    L.stage_bytes = round_up(kTile * (keyed ? 32 : kRecBytes), 128);
+    L.ring = p;   p += kIdxBigStages * L.stage_bytes;
+    L.cnt = p;    p += round_up(kWarps * round_up(B, 8) * 2, 16);
+    L.gcur = p;   p += round_up(B * 4, 16);
+    L.lstart = p; p += round_up(B * 4, 16);
+    L.perm = p;   p += kIdxBigTile * 2;                   // tile-sorted slot -> record in tile
+    L.pbkt = p;   p += kIdxBigTile * 2;                   // tile-sorted slot -> bucket
+    L.skey = p;   if (!keyed) p += kIdxBigTile * 4;       // pass A: the full key of every record
+    L.edges = p;  p += round_up(n_edges * 4, 16);
+    L.misc = p;   p += 64 * 4;
+    L.desc = p;   p += kIdxBigStages * 16;
+    L.bars = p;   p += kIdxBigStages * 8;
+    L.total = p;
+    return L;
+}
+
+template <bool KEYED, bool POS, bool EDGES>
+__global__ void __launch_bounds__(kThreads, 1) k_scatter_idx_big(const ChunkDesc* __restrict__ chunks, uint32_t n_chunks, Span sp,
+                                                                const uint4* __restrict__ aos_in,
+                                                                const uint32_t* __restrict__ n_ptr,
+                                                                const __grid_constant__ DevGrid g,
+                                                                const __grid_constant__ DevBeam bm, uint32_t B,
+                                                                uint32_t lo_bits, const uint32_t* __restrict__ table,
+                                                                uint32_t stride, uint4* __restrict__ aos_out)
+{
+    extern __shared__ __align__(128) uint8_t smem[];
+    constexpr uint32_t kRecB = KEYED ? 32u : (uint32_t)kRecBytes;
+    const uint32_t Bp = round_up(B, 8);
+    const IdxBigSmem L = idx_big_layout(KEYED, B, g.n_ebins + 1);
+    uint16_t* cnt = reinterpret_cast<uint16_t*>(smem + L.cnt);
+    uint32_t* gcur = reinterpret_cast<uint32_t*>(smem + L.gcur);
+    uint32_t* lstart = reinterpret_cast<uint32_t*>(smem + L.lstart);
+    uint16_t* perm = reinterpret_cast<uint16_t*>(smem + L.perm);
+    uint16_t* pbkt = reinterpret_cast<uint16_t*>(smem + L.pbkt);
+    uint32_t* skey = reinterpret_cast<uint32_t*>(smem + L.skey);
+    float* s_edges = reinterpret_cast<float*>(smem + L.edges);
+    uint32_t* misc = reinterpret_cast<uint32_t*>(smem + L.misc);
+    TileDesc* s_desc = reinterpret_cast<TileDesc*>(smem + L.desc);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + L.bars);
+    const uint32_t w = warp_id();
+    const uint32_t lo_mask = (1u << lo_bits) - 1u;
+    const uint32_t n_rec = KEYED ? *n_ptr : 0u;
+    if (KEYED) {
+        sp.tile_begin = 0;
+        sp.n_tiles = (n_rec + kTile - 1) / kTile;
+        sp.col0 = 0;
+    }
+    const uint32_t col = sp.col0 + blockIdx.x * sp.split;
+
+    uint32_t t0, t1;
+    segment_of(sp, t0, t1);
+    const uint32_t n = t1 - t0;  // ring stages (1024-record tiles) in this segment
+
+    auto stage_ptr = [&](uint32_t i) { return reinterpret_cast<uint32_t*>(smem + L.ring + (i % kIdxBigStages) * L.stage_bytes); };
+    auto issue = [&](uint32_t i) {  // thread 0
+        TileDesc d = KEYED ? keyed_tile(aos_in, n_rec, t0 + i) : raw_tile(chunks, n_chunks, t0 + i);
+        s_desc[i % kIdxBigStages] = d;
+        ring_issue_stream(stage_ptr(i), &bars[i % kIdxBigStages], d.ptr, d.count * kRecB);
+    };
+    if (threadIdx.x == 0) {
+        for (int k = 0; k < kIdxBigStages; ++k) mbar_init(&bars[k], 1);
+        mbar_fence_init();
+        for (uint32_t k = 0; k < (uint32_t)kIdxBigStages && k < n; ++k) issue(k);
+    }
+    {
+        uint32_t* cz = reinterpret_cast<uint32_t*>(cnt);
+        for (uint32_t i = threadIdx.x; i < kWarps * Bp / 2; i += kThreads) cz[i] = 0;
+    }
+    uint32_t grun[8];  // thread t keeps the running first free slot of buckets 8t..8t+7
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        uint32_t b = threadIdx.x * 8 + k;
+        grun[k] = b < B ? table[(size_t)b * stride + col] : 0u;
+    }
+    if (!KEYED) stage_edges(g, s_edges);
+    __syncthreads();
+
+    for (uint32_t base = 0; base < n; base += kIdxBigQ) {
+        const uint32_t nq = min((uint32_t)kIdxBigQ, n - base);
+        // stages TMA could not fill (unaligned source, ragged last tile): fetched by all threads, then the
+        // stage's barrier is completed by hand so that every stage flips its phase once per use
+        bool manual = false;
+        for (uint32_t q = 0; q < nq; ++q) {
+            const TileDesc d = s_desc[(base + q) % kIdxBigStages];
+            if (!bulk_ok(d.ptr, d.count * kRecB)) {
+                const uint32_t* src = reinterpret_cast<const uint32_t*>(d.ptr);
+                uint32_t* dst = stage_ptr(base + q);
+                for (uint32_t k = threadIdx.x; k < d.count * (kRecB / 4); k += kThreads) dst[k] = __ldg(src + k);
+                manual = true;
+            }
+        }
+        if (manual) {
+            __syncthreads();
+            if (threadIdx.x == 0)
+                for (uint32_t q = 0; q < nq; ++q) {
+                    const TileDesc d = s_desc[(base + q) % kIdxBigStages];
+                    if (!bulk_ok(d.ptr, d.count * kRecB)) mbar_arrive(&bars[(base + q) % kIdxBigStages]);
+                }
+        }
+
+        // buckets and stable ranks inside the warp's 512 records (half of ring stage base + w / 2)
+        uint32_t packed[kIdxBigRounds];
+#pragma unroll
+        for (int r = 0; r < kIdxBigRounds; ++r) packed[r] = kNone;
+        const uint32_t q = w / (kWarps / kIdxBigQ);
+        if (q < nq) {
+            const uint32_t i = base + q;
+            const TileDesc td = s_desc[i % kIdxBigStages];
+            mbar_wait(&bars[i % kIdxBigStages], (i / kIdxBigStages) & 1u);
+            const uint32_t* raw = stage_ptr(i);
+            const uint32_t first = (w % (kWarps / kIdxBigQ)) * kIdxBigSpan;
+            if (KEYED) {
+#pragma unroll
+                for (int r = 0; r < kIdxBigRounds; ++r) {
+                    const uint32_t idx = first + r * 32 + lane_id();
+                    packed[r] = idx < td.count ? (raw[idx * 8] >> lo_bits) : kNone;
+                }
+            } else {
+#pragma unroll
+                for (int h = 0; h < kIdxBigRounds; h += 4) {
+                    Rec rec[4];
+#pragma unroll
+                    for (int r = 0; r < 4; ++r) {
+                        const uint32_t idx = first + (h + r) * 32 + lane_id();
+                        rec[r] = rec_from_smem(raw, idx < td.count ? (int)idx : 0);
+                    }
+#pragma unroll
+                    for (int r = 0; r < 4; ++r) {
+                        const uint32_t idx = first + (h + r) * 32 + lane_id();
+                        uint32_t key;
+                        const int cls = classify<POS, EDGES, 0>(g, bm, rec[r], s_edges, key);
+                        const bool keep = idx < td.count && cls == C_SURVIVOR;
+                        skey[q * kTile + idx] = keep ? key : kNone;
+                        packed[h + r] = keep ? (key & lo_mask) : kNone;
+                    }
+                }
+            }
+#pragma unroll
+            for (int r = 0; r < kIdxBigRounds; ++r) {
+                const uint32_t bucket = packed[r];
+                const uint32_t rank = warp_rank(bucket, cnt + w * Bp);
+                packed[r] = bucket == kNone ? kNone : ((bucket << 10) | rank);  // rank < 512
+            }
+        }
+        __syncthreads();
+        const uint32_t n_part = finish_ranks<true>(cnt, B, Bp, gcur, lstart, misc, grun);
+
+        // tile-sorted order
+#pragma unroll
+        for (int r = 0; r < kIdxBigRounds; ++r) {
+            if (packed[r] != kNone) {
+                const uint32_t bucket = packed[r] >> 10, rank = packed[r] & 1023u;
+                const uint32_t p = lstart[bucket] + cnt[w * Bp + bucket] + rank;
+                perm[p] = (uint16_t)(w * kIdxBigSpan + r * 32 + lane_id());
+                pbkt[p] = (uint16_t)bucket;
+            }
+        }
+        __syncwarp();
+        zero_row(cnt + w * Bp, Bp);
+        __syncthreads();
+
+        // write-out: consecutive threads write consecutive 16-byte halves of consecutive tile-sorted slots, so a
+        // run of records of one bucket leaves as one request per 128-byte line
+        for (uint32_t m = threadIdx.x; m < 2 * n_part; m += kThreads) {
+            const uint32_t j = m >> 1, half = m & 1u;
+            const uint32_t bucket = pbkt[j];
+            const uint32_t dest = gcur[bucket] + (j - lstart[bucket]);
+            const uint32_t irec = perm[j];
+            const uint32_t i = base + irec / kTile, ir = irec % kTile;
+            uint4 v;
+            if (KEYED) {
+                v = reinterpret_cast<const uint4*>(stage_ptr(i))[2 * ir + half];
+            } else {
+                const uint32_t* p = stage_ptr(i) + ir * kRecWords;
+                if (half == 0) v = make_uint4(skey[irec], p[1], p[2], p[3]);
+                else v = make_uint4(p[4], p[5], p[6], s_desc[i % kIdxBigStages].first_index + ir);
+            }
+            aos_out[2 * (size_t)dest + half] = v;
+        }
+        __syncthreads();  // the tile's stages, perm, pbkt and skey are free again
+        if (threadIdx.x == 0)
+            for (uint32_t k = 0; k < nq; ++k)
+                if (base + kIdxBigStages + k < n) issue(base + kIdxBigStages + k);
+        __syncthreads();  // the next tile reads descriptors just written
+    }
+}
+
+}  // namespace psl
