@@ -294,6 +294,9 @@ struct psl_ctx {
     bool big_tiles = false;  // ONTHEFLY with few keys: the 4096-record-tile scatter
     uint32_t count_stages = kStagesCount, count_split = 1;
     uint32_t sm_count_raw = 0, sm_scatter_otf = 0, sm_idx_a = 0, sm_count_b = 0, sm_idx_b = 0;  // dynamic smem bytes
+    // INDEX passes: 4096-record tiles when the counters of the pass fit shared memory beside the ring, else 1024
+    bool idx_big_a = false, idx_big_b = false;
+    uint32_t split_a = 1, split_b = 1;  // histogram CTAs (= table columns) per scatter segment
     struct ChunkLaunch { Span span; uint32_t n_seg; };
     std::vector<ChunkDesc> pending_chunks;  // ONTHEFLY: chunk descriptors not yet on the device
     uint32_t chunks_uploaded = 0;
@@ -616,8 +619,12 @@ psl_status finalize_index(psl_ctx* ctx)
         {
             Prof prof(ctx, PSL_K_INDEX_A);
             for (const psl_ctx::ChunkLaunch& cl : ctx->idx_launches) {  // the same segments the counts were taken on
-                scatter_idx_big_a_fn(ctx->grid.has_pos != 0, ctx->grid.ebin_mode != 0)<<<cl.n_seg, kThreads, ctx->sm_idx_a, ctx->stream>>>(
-                    chunks, ctx->n_chunks, cl.span, nullptr, nullptr, ctx->grid, none, d.B_lo, d.lo_bits, table_a, d.cols_cap, aos);
+                if (ctx->idx_big_a)
+                    scatter_idx_big_a_fn(ctx->grid.has_pos != 0, ctx->grid.ebin_mode != 0)<<<cl.n_seg, kIdxBigThreads, ctx->sm_idx_a, ctx->stream>>>(
+                        chunks, ctx->n_chunks, cl.span, nullptr, nullptr, ctx->grid, none, d.B_lo, d.lo_bits, table_a, d.cols_cap, aos);
+                else
+                    scatter_idx_a_fn(ctx->grid.has_pos != 0, ctx->grid.ebin_mode != 0)<<<cl.n_seg, kThreads, ctx->sm_idx_a, ctx->stream>>>(
+                        chunks, ctx->n_chunks, cl.span, ctx->grid, none, d.B_lo, d.lo_bits, table_a, d.cols_cap, aos);
                 LAUNCHED();
             }
         }
@@ -626,24 +633,29 @@ psl_status finalize_index(psl_ctx* ctx)
         const uint32_t Sb = ntb < ctx->S_b ? ntb : ctx->S_b;
         {
             Prof prof(ctx, PSL_K_COUNT);
-            k_count_keys<<<Sb * kIdxSplit, kThreads, ctx->sm_count_b, ctx->stream>>>(aos, scalar(ctx, SC_NIDX), d.B_hi, d.lo_bits, table_b,
-                                                                                     kMaxSegments, kIdxSplit);
+            k_count_keys<<<Sb * ctx->split_b, kThreads, ctx->sm_count_b, ctx->stream>>>(aos, scalar(ctx, SC_NIDX), d.B_hi, d.lo_bits, table_b,
+                                                                                     kMaxSegments, ctx->split_b);
             LAUNCHED();
         }
-        if ((uint64_t)d.B_hi * Sb * kIdxSplit <= kScanSmallMax) {
+        if ((uint64_t)d.B_hi * Sb * ctx->split_b <= kScanSmallMax) {
             Prof prof(ctx, PSL_K_SCAN);
-            k_scan_small<<<1, 1024, 0, ctx->stream>>>(table_b, Sb * kIdxSplit, kMaxSegments, d.B_hi, scalar(ctx, SC_TOTAL), 0, nullptr, nullptr,
+            k_scan_small<<<1, 1024, 0, ctx->stream>>>(table_b, Sb * ctx->split_b, kMaxSegments, d.B_hi, scalar(ctx, SC_TOTAL), 0, nullptr, nullptr,
                                                       1, 0, nullptr);
             LAUNCHED();
         } else {
-            s = run_scan(ctx, table_b, d.B_hi, Sb * kIdxSplit, kMaxSegments, scalar(ctx, SC_TOTAL));
+            s = run_scan(ctx, table_b, d.B_hi, Sb * ctx->split_b, kMaxSegments, scalar(ctx, SC_TOTAL));
             if (s != PSL_OK) return s;
         }
         {
             Prof prof(ctx, PSL_K_INDEX_B);
-            const Span spb = {0u, 0u, 0u, kIdxSplit};
-            scatter_idx_big_b_fn()<<<Sb, kThreads, ctx->sm_idx_b, ctx->stream>>>(nullptr, 0, spb, aos, scalar(ctx, SC_NIDX), ctx->grid, none, d.B_hi,
-                                                                                d.lo_bits, table_b, kMaxSegments, at<uint4>(ctx, L.aos_index));
+            const Span spb = {0u, 0u, 0u, ctx->split_b};
+            if (ctx->idx_big_b)
+                scatter_idx_big_b_fn()<<<Sb, kIdxBigThreads, ctx->sm_idx_b, ctx->stream>>>(nullptr, 0, spb, aos, scalar(ctx, SC_NIDX), ctx->grid, none,
+                                                                                    d.B_hi, d.lo_bits, table_b, kMaxSegments,
+                                                                                    at<uint4>(ctx, L.aos_index));
+            else
+                k_scatter_idx_b<<<Sb, kThreads, ctx->sm_idx_b, ctx->stream>>>(aos, scalar(ctx, SC_NIDX), d.B_hi, d.lo_bits, table_b, kMaxSegments,
+                                                                             at<uint4>(ctx, L.aos_index));
             LAUNCHED();
         }
         k_offsets_by_search_keyed<<<(d.K + 1 + 255) / 256, 256, 0, ctx->stream>>>(at<uint4>(ctx, L.aos_index), scalar(ctx, SC_NIDX), d.K, idx_offsets);
@@ -921,17 +933,27 @@ psl_status psl_create(const psl_config* cfg, psl_ctx** out)
     } else {
         ctx->count_stages = d.B_lo * 4 > 8192 ? 2 : kStagesCount;
         ctx->sm_count_raw = count_layout(kTile * kRecBytes, ctx->count_stages, d.B_lo, ne).total;
-        ctx->sm_idx_a = idx_big_layout(false, d.B_lo, ne).total;
+        int max_smem = 0;
+        CUC(cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, cfg->device));
+        ctx->idx_big_a = idx_big_layout(false, d.B_lo, ne).total + 1024 <= (uint32_t)max_smem;
+        ctx->idx_big_b = idx_big_layout(true, d.B_hi, ne).total + 1024 <= (uint32_t)max_smem;
+        ctx->split_a = ctx->idx_big_a ? kIdxSplit : 1;
+        ctx->split_b = ctx->idx_big_b ? kIdxSplit : 1;
+        ctx->sm_idx_a = ctx->idx_big_a ? idx_big_layout(false, d.B_lo, ne).total : idx_a_layout(d.B_lo, ne).total;
         ctx->sm_count_b = count_layout(0, 0, d.B_hi, 0).total;
-        ctx->sm_idx_b = idx_big_layout(true, d.B_hi, ne).total;  // same layout call as in the kernel
+        ctx->sm_idx_b = ctx->idx_big_b ? idx_big_layout(true, d.B_hi, ne).total : idx_b_layout(d.B_hi).total;
         const bool pos = d.n_pos > 1, edges = cfg->ebin_mode == PSL_EBIN_EDGES;
         CUC(allow_smem(count_idx_fn(pos, edges), ctx->sm_count_raw));
-        CUC(allow_smem(scatter_idx_big_a_fn(pos, edges), ctx->sm_idx_a));
+        if (ctx->idx_big_a) CUC(allow_smem(scatter_idx_big_a_fn(pos, edges), ctx->sm_idx_a));
+        else CUC(allow_smem(scatter_idx_a_fn(pos, edges), ctx->sm_idx_a));
         CUC(allow_smem(k_count_keys, ctx->sm_count_b));
-        CUC(allow_smem(scatter_idx_big_b_fn(), ctx->sm_idx_b));
-        CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, scatter_idx_big_a_fn(pos, edges), kThreads, ctx->sm_idx_a));
+        if (ctx->idx_big_b) CUC(allow_smem(scatter_idx_big_b_fn(), ctx->sm_idx_b));
+        else CUC(allow_smem(k_scatter_idx_b, ctx->sm_idx_b));
+        if (ctx->idx_big_a) CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, scatter_idx_big_a_fn(pos, edges), kIdxBigThreads, ctx->sm_idx_a));
+        else CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, scatter_idx_a_fn(pos, edges), kThreads, ctx->sm_idx_a));
         ctx->S_a = width(occ);
-        CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, scatter_idx_big_b_fn(), kThreads, ctx->sm_idx_b));
+        if (ctx->idx_big_b) CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, scatter_idx_big_b_fn(), kIdxBigThreads, ctx->sm_idx_b));
+        else CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_scatter_idx_b, kThreads, ctx->sm_idx_b));
         ctx->S_b = width(occ);
     }
     CUC(cudaStreamSynchronize(ctx->stream));
@@ -1030,16 +1052,16 @@ psl_status psl_load_chunk(psl_ctx* ctx, const void* records, uint64_t n, int32_t
         DevBeam none;
         memset(&none, 0, sizeof none);
         psl_ctx::ChunkLaunch cl;
-        cl.span = {tile0, nt, ctx->n_cols, kIdxSplit};
+        cl.span = {tile0, nt, ctx->n_cols, ctx->split_a};
         cl.n_seg = nt < ctx->S_a ? nt : ctx->S_a;
-        if (ctx->n_cols + cl.n_seg * kIdxSplit > ctx->d.cols_cap) { set_err(ctx->err, "load_chunk: out of table columns"); return PSL_ERR_CAPACITY; }
+        if (ctx->n_cols + cl.n_seg * ctx->split_a > ctx->d.cols_cap) { set_err(ctx->err, "load_chunk: out of table columns"); return PSL_ERR_CAPACITY; }
         Prof prof(ctx, PSL_K_COUNT);
-        count_idx_fn(ctx->grid.has_pos != 0, ctx->grid.ebin_mode != 0)<<<cl.n_seg * kIdxSplit, kThreads, ctx->sm_count_raw, ctx->stream>>>(
+        count_idx_fn(ctx->grid.has_pos != 0, ctx->grid.ebin_mode != 0)<<<cl.n_seg * ctx->split_a, kThreads, ctx->sm_count_raw, ctx->stream>>>(
             chunks, ctx->n_chunks + 1, cl.span, ctx->grid, none, ctx->d.B_lo, (1u << ctx->d.lo_bits) - 1u,
             at<uint32_t>(ctx, ctx->L.table_a), ctx->d.cols_cap, at<SegStats>(ctx, ctx->L.sstats), ctx->count_stages);
         LAUNCHED();
         ctx->idx_launches.push_back(cl);
-        ctx->n_cols += cl.n_seg * kIdxSplit;
+        ctx->n_cols += cl.n_seg * ctx->split_a;
     }
     ctx->n_records += n;
     if (host) ctx->n_host_records += n;

@@ -6,9 +6,9 @@
 // bucket: ordered by (bucket, input order) inside the tile they form ~128-byte runs, and the lanes of a warp
 // write consecutive 16-byte halves of consecutive slots, so one request covers a whole run.
 //
-// One 256-thread CTA per SM: the tile is 4 ring stages of 1024 records that stay where TMA put them, a fifth
-// stage prefetches.  Warp w owns records [512 w, 512 w + 512) of the tile (half a stage): per-warp private
-// uint16 counters + __match_any_sync give stable ranks, finish_ranks the prefix over the 8 warps.
+// One 512-thread CTA per SM: the tile is 4 ring stages of 1024 records that stay where TMA put them, a fifth
+// stage prefetches.  Warp w owns records [256 w, 256 w + 256) of the tile (a quarter of a stage): per-warp private
+// uint16 counters + __match_any_sync give stable ranks, finish_ranks the prefix over the 16 warps.
 #pragma once
 
 #include "psl_index.cuh"
@@ -18,8 +18,10 @@ namespace psl {
 constexpr int kIdxBigQ = 4;                               // ring stages per tile
 constexpr int kIdxBigTile = kIdxBigQ * kTile;             // 4096 records
 constexpr int kIdxBigStages = 5;
-constexpr int kIdxBigSpan = kIdxBigTile / kWarps;         // 512 records per warp
-constexpr int kIdxBigRounds = kIdxBigSpan / 32;           // 16
+constexpr int kIdxBigThreads = 512;
+constexpr int kIdxBigWarps = kIdxBigThreads / 32;         // 16
+constexpr int kIdxBigSpan = kIdxBigTile / kIdxBigWarps;   // 256 records per warp
+constexpr int kIdxBigRounds = kIdxBigSpan / 32;           // 8
 
 struct IdxBigSmem {
     uint32_t ring, stage_bytes, cnt, gcur, lstart, perm, pbkt, skey, edges, misc, desc, bars, total;
@@ -31,7 +33,7 @@ __host__ __device__ inline IdxBigSmem idx_big_layout(bool keyed, uint32_t B, uin
     uint32_t p = 0;
     L.stage_bytes = round_up(kTile * (keyed ? 32 : kRecBytes), 128);
     L.ring = p;   p += kIdxBigStages * L.stage_bytes;
-    L.cnt = p;    p += round_up(kWarps * round_up(B, 8) * 2, 16);
+    L.cnt = p;    p += round_up(kIdxBigWarps * round_up(B, 8) * 2, 16);
     L.gcur = p;   p += round_up(B * 4, 16);
     L.lstart = p; p += round_up(B * 4, 16);
     L.perm = p;   p += kIdxBigTile * 2;                   // tile-sorted slot -> record in tile
@@ -46,7 +48,7 @@ __host__ __device__ inline IdxBigSmem idx_big_layout(bool keyed, uint32_t B, uin
 }
 
 template <bool KEYED, bool POS, bool EDGES>
-__global__ void __launch_bounds__(kThreads, 1) k_scatter_idx_big(const ChunkDesc* __restrict__ chunks, uint32_t n_chunks, Span sp,
+__global__ void __launch_bounds__(kIdxBigThreads, 1) k_scatter_idx_big(const ChunkDesc* __restrict__ chunks, uint32_t n_chunks, Span sp,
                                                                 const uint4* __restrict__ aos_in,
                                                                 const uint32_t* __restrict__ n_ptr,
                                                                 const __grid_constant__ DevGrid g,
@@ -95,7 +97,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_scatter_idx_big(const ChunkDesc
     }
     {
         uint32_t* cz = reinterpret_cast<uint32_t*>(cnt);
-        for (uint32_t i = threadIdx.x; i < kWarps * Bp / 2; i += kThreads) cz[i] = 0;
+        for (uint32_t i = threadIdx.x; i < kIdxBigWarps * Bp / 2; i += kIdxBigThreads) cz[i] = 0;
     }
     uint32_t grun[8];  // thread t keeps the running first free slot of buckets 8t..8t+7
 #pragma unroll
@@ -116,7 +118,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_scatter_idx_big(const ChunkDesc
             if (!bulk_ok(d.ptr, d.count * kRecB)) {
                 const uint32_t* src = reinterpret_cast<const uint32_t*>(d.ptr);
                 uint32_t* dst = stage_ptr(base + q);
-                for (uint32_t k = threadIdx.x; k < d.count * (kRecB / 4); k += kThreads) dst[k] = __ldg(src + k);
+                for (uint32_t k = threadIdx.x; k < d.count * (kRecB / 4); k += kIdxBigThreads) dst[k] = __ldg(src + k);
                 manual = true;
             }
         }
@@ -133,13 +135,13 @@ __global__ void __launch_bounds__(kThreads, 1) k_scatter_idx_big(const ChunkDesc
         uint32_t packed[kIdxBigRounds];
 #pragma unroll
         for (int r = 0; r < kIdxBigRounds; ++r) packed[r] = kNone;
-        const uint32_t q = w / (kWarps / kIdxBigQ);
+        const uint32_t q = w / (kIdxBigWarps / kIdxBigQ);
         if (q < nq) {
             const uint32_t i = base + q;
             const TileDesc td = s_desc[i % kIdxBigStages];
             mbar_wait(&bars[i % kIdxBigStages], (i / kIdxBigStages) & 1u);
             const uint32_t* raw = stage_ptr(i);
-            const uint32_t first = (w % (kWarps / kIdxBigQ)) * kIdxBigSpan;
+            const uint32_t first = (w % (kIdxBigWarps / kIdxBigQ)) * kIdxBigSpan;
             if (KEYED) {
 #pragma unroll
                 for (int r = 0; r < kIdxBigRounds; ++r) {
@@ -170,11 +172,11 @@ __global__ void __launch_bounds__(kThreads, 1) k_scatter_idx_big(const ChunkDesc
             for (int r = 0; r < kIdxBigRounds; ++r) {
                 const uint32_t bucket = packed[r];
                 const uint32_t rank = warp_rank(bucket, cnt + w * Bp);
-                packed[r] = bucket == kNone ? kNone : ((bucket << 10) | rank);  // rank < 512
+                packed[r] = bucket == kNone ? kNone : ((bucket << 10) | rank);  // rank < 256
             }
         }
         __syncthreads();
-        const uint32_t n_part = finish_ranks<true>(cnt, B, Bp, gcur, lstart, misc, grun);
+        const uint32_t n_part = finish_ranks<true, kIdxBigWarps>(cnt, B, Bp, gcur, lstart, misc, grun);
 
         // tile-sorted order
 #pragma unroll
@@ -192,7 +194,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_scatter_idx_big(const ChunkDesc
 
         // write-out: consecutive threads write consecutive 16-byte halves of consecutive tile-sorted slots, so a
         // run of records of one bucket leaves as one request per 128-byte line
-        for (uint32_t m = threadIdx.x; m < 2 * n_part; m += kThreads) {
+        for (uint32_t m = threadIdx.x; m < 2 * n_part; m += kIdxBigThreads) {
             const uint32_t j = m >> 1, half = m & 1u;
             const uint32_t bucket = pbkt[j];
             const uint32_t dest = gcur[bucket] + (j - lstart[bucket]);
