@@ -33,7 +33,7 @@ constexpr uint64_t kStageBytes = 32ull << 20;  // pinned staging buffers for pag
 
 struct Layout {
     uint64_t total = 0;
-    uint64_t raw = 0, chunks = 0, sstats = 0, scan_sums = 0, scalars = 0, edges = 0, stats = 0, batch_off = 0;
+    uint64_t raw = 0, chunks = 0, spans = 0, sstats = 0, scan_sums = 0, scalars = 0, edges = 0, stats = 0, batch_off = 0;
     // ONTHEFLY
     uint64_t table = 0, out[10] = {0}, offsets = 0, counts = 0;
     // INDEX
@@ -162,6 +162,7 @@ void plan(const psl_config* c, const Derived& d, Layout* L)
     const bool proj = (c->flags & PSL_OUT_PROJ) != 0;
     L->raw = take(&cur, c->max_host_records * kRecBytes);
     L->chunks = take(&cur, (uint64_t)d.max_chunks * sizeof(ChunkDesc));
+    L->spans = take(&cur, (uint64_t)d.max_chunks * sizeof(SpanSeg));
     L->sstats = take(&cur, (uint64_t)d.cols_cap * sizeof(SegStats));
     L->scan_sums = take(&cur, (uint64_t)(d.scan_blocks_cap + 1) * 4);
     L->scalars = take(&cur, 64);
@@ -252,8 +253,8 @@ ScatterOtfFn scatter_big_fn(bool pos, bool edges, int beam, bool proj)
     return pos ? (edges ? scatter_big_pe<true, true>(beam, proj) : scatter_big_pe<true, false>(beam, proj))
                : (edges ? scatter_big_pe<false, true>(beam, proj) : scatter_big_pe<false, false>(beam, proj));
 }
-using ScatterIdxBigFn = void (*)(const ChunkDesc*, uint32_t, Span, const uint4*, const uint32_t*, DevGrid, DevBeam, uint32_t, uint32_t,
-                                 const uint32_t*, uint32_t, uint4*);
+using ScatterIdxBigFn = void (*)(const ChunkDesc*, uint32_t, const SpanSeg*, uint32_t, Span, const uint4*, const uint32_t*, DevGrid, DevBeam,
+                                 uint32_t, uint32_t, const uint32_t*, uint32_t, uint4*);
 // the 4096-record-tile INDEX passes: A (raw records in) per grid features, B (keyed records in)
 ScatterIdxBigFn scatter_idx_big_a_fn(bool pos, bool edges)
 {
@@ -300,7 +301,8 @@ struct psl_ctx {
     struct ChunkLaunch { Span span; uint32_t n_seg; };
     std::vector<ChunkDesc> pending_chunks;  // ONTHEFLY: chunk descriptors not yet on the device
     uint32_t chunks_uploaded = 0;
-    std::vector<ChunkLaunch> idx_launches;  // INDEX: the per-chunk count launches, replayed by pass A's scatter
+    std::vector<ChunkLaunch> idx_launches;
+    std::vector<SpanSeg> h_spans;  // INDEX: the per-chunk count launches, replayed by pass A's scatter
     // state
     uint64_t n_records = 0, n_host_records = 0;
     uint32_t n_tiles = 0, n_chunks = 0, n_cols = 0;
@@ -618,14 +620,28 @@ psl_status finalize_index(psl_ctx* ctx)
         if (s != PSL_OK) return s;
         {
             Prof prof(ctx, PSL_K_INDEX_A);
-            for (const psl_ctx::ChunkLaunch& cl : ctx->idx_launches) {  // the same segments the counts were taken on
-                if (ctx->idx_big_a)
-                    scatter_idx_big_a_fn(ctx->grid.has_pos != 0, ctx->grid.ebin_mode != 0)<<<cl.n_seg, kIdxBigThreads, ctx->sm_idx_a, ctx->stream>>>(
-                        chunks, ctx->n_chunks, cl.span, nullptr, nullptr, ctx->grid, none, d.B_lo, d.lo_bits, table_a, d.cols_cap, aos);
-                else
+            if (ctx->idx_big_a) {
+                // ONE launch walks every chunk's span with the segments the counts were taken on
+                std::vector<SpanSeg>& hs = ctx->h_spans;  // lives as long as the context: the copy below is asynchronous
+                hs.clear();
+                uint32_t grid = 1;
+                for (const psl_ctx::ChunkLaunch& cl : ctx->idx_launches) {
+                    hs.push_back({cl.span, cl.n_seg});
+                    if (cl.n_seg > grid) grid = cl.n_seg;
+                }
+                SpanSeg* d_spans = at<SpanSeg>(ctx, L.spans);
+                CU(cudaMemcpyAsync(d_spans, hs.data(), hs.size() * sizeof(SpanSeg), cudaMemcpyHostToDevice, ctx->stream));
+                const Span unused = {0u, 0u, 0u, 1u};
+                scatter_idx_big_a_fn(ctx->grid.has_pos != 0, ctx->grid.ebin_mode != 0)<<<grid, kIdxBigThreads, ctx->sm_idx_a, ctx->stream>>>(
+                    chunks, ctx->n_chunks, d_spans, (uint32_t)hs.size(), unused, nullptr, nullptr, ctx->grid, none, d.B_lo, d.lo_bits, table_a,
+                    d.cols_cap, aos);
+                LAUNCHED();
+            } else {
+                for (const psl_ctx::ChunkLaunch& cl : ctx->idx_launches) {  // the same segments the counts were taken on
                     scatter_idx_a_fn(ctx->grid.has_pos != 0, ctx->grid.ebin_mode != 0)<<<cl.n_seg, kThreads, ctx->sm_idx_a, ctx->stream>>>(
                         chunks, ctx->n_chunks, cl.span, ctx->grid, none, d.B_lo, d.lo_bits, table_a, d.cols_cap, aos);
-                LAUNCHED();
+                    LAUNCHED();
+                }
             }
         }
         // pass B runs over the n_idx <= n_records keyed records; the device knows n_idx, the host only the bound
@@ -650,7 +666,7 @@ psl_status finalize_index(psl_ctx* ctx)
             Prof prof(ctx, PSL_K_INDEX_B);
             const Span spb = {0u, 0u, 0u, ctx->split_b};
             if (ctx->idx_big_b)
-                scatter_idx_big_b_fn()<<<Sb, kIdxBigThreads, ctx->sm_idx_b, ctx->stream>>>(nullptr, 0, spb, aos, scalar(ctx, SC_NIDX), ctx->grid, none,
+                scatter_idx_big_b_fn()<<<Sb, kIdxBigThreads, ctx->sm_idx_b, ctx->stream>>>(nullptr, 0, nullptr, 0, spb, aos, scalar(ctx, SC_NIDX), ctx->grid, none,
                                                                                     d.B_hi, d.lo_bits, table_b, kMaxSegments,
                                                                                     at<uint4>(ctx, L.aos_index));
             else

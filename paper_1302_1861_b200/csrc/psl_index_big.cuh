@@ -47,8 +47,18 @@ __host__ __device__ inline IdxBigSmem idx_big_layout(bool keyed, uint32_t B, uin
     return L;
 }
 
+// one per-chunk histogram launch of pass A: its span and how many segments (scatter CTAs) it was cut into
+struct SpanSeg {
+    Span sp;
+    uint32_t n_seg;
+};
+
+// Pass A (KEYED = false) walks ALL chunk launches in one kernel: CTA s takes segment s of every span that has one,
+// with the running slots re-read from that span's table columns.  Pass B (KEYED = true) has one span, computed
+// from *n_ptr.
 template <bool KEYED, bool POS, bool EDGES>
-__global__ void __launch_bounds__(kIdxBigThreads, 1) k_scatter_idx_big(const ChunkDesc* __restrict__ chunks, uint32_t n_chunks, Span sp,
+__global__ void __launch_bounds__(kIdxBigThreads, 1) k_scatter_idx_big(const ChunkDesc* __restrict__ chunks, uint32_t n_chunks,
+                                                                const SpanSeg* __restrict__ spans, uint32_t n_spans, Span sp,
                                                                 const uint4* __restrict__ aos_in,
                                                                 const uint32_t* __restrict__ n_ptr,
                                                                 const __grid_constant__ DevGrid g,
@@ -73,39 +83,51 @@ __global__ void __launch_bounds__(kIdxBigThreads, 1) k_scatter_idx_big(const Chu
     const uint32_t w = warp_id();
     const uint32_t lo_mask = (1u << lo_bits) - 1u;
     const uint32_t n_rec = KEYED ? *n_ptr : 0u;
-    if (KEYED) {
-        sp.tile_begin = 0;
-        sp.n_tiles = (n_rec + kTile - 1) / kTile;
-        sp.col0 = 0;
-    }
-    const uint32_t col = sp.col0 + blockIdx.x * sp.split;
-
-    uint32_t t0, t1;
-    segment_of(sp, t0, t1);
-    const uint32_t n = t1 - t0;  // ring stages (1024-record tiles) in this segment
-
-    auto stage_ptr = [&](uint32_t i) { return reinterpret_cast<uint32_t*>(smem + L.ring + (i % kIdxBigStages) * L.stage_bytes); };
+    uint32_t goff = 0;  // ring stages this CTA has consumed in earlier spans (stage and parity bookkeeping runs on)
+    uint32_t t0 = 0, n = 0;
+    auto stage_ptr = [&](uint32_t i) { return reinterpret_cast<uint32_t*>(smem + L.ring + ((goff + i) % kIdxBigStages) * L.stage_bytes); };
     auto issue = [&](uint32_t i) {  // thread 0
         TileDesc d = KEYED ? keyed_tile(aos_in, n_rec, t0 + i) : raw_tile(chunks, n_chunks, t0 + i);
-        s_desc[i % kIdxBigStages] = d;
-        ring_issue_stream(stage_ptr(i), &bars[i % kIdxBigStages], d.ptr, d.count * kRecB);
+        s_desc[(goff + i) % kIdxBigStages] = d;
+        ring_issue_stream(stage_ptr(i), &bars[(goff + i) % kIdxBigStages], d.ptr, d.count * kRecB);
     };
     if (threadIdx.x == 0) {
         for (int k = 0; k < kIdxBigStages; ++k) mbar_init(&bars[k], 1);
         mbar_fence_init();
-        for (uint32_t k = 0; k < (uint32_t)kIdxBigStages && k < n; ++k) issue(k);
     }
     {
         uint32_t* cz = reinterpret_cast<uint32_t*>(cnt);
         for (uint32_t i = threadIdx.x; i < kIdxBigWarps * Bp / 2; i += kIdxBigThreads) cz[i] = 0;
     }
+    if (!KEYED) stage_edges(g, s_edges);
+    __syncthreads();
+
+    const uint32_t n_iter = KEYED ? 1u : n_spans;
+    for (uint32_t si = 0; si < n_iter; ++si) {
+    uint32_t S = gridDim.x;
+    if (KEYED) {
+        sp.tile_begin = 0;
+        sp.n_tiles = (n_rec + kTile - 1) / kTile;
+        sp.col0 = 0;
+    } else {
+        sp = spans[si].sp;
+        S = spans[si].n_seg;
+        if (blockIdx.x >= S) continue;  // this span was cut into fewer segments than there are CTAs
+    }
+    const uint32_t col = sp.col0 + blockIdx.x * sp.split;
+    {
+        const unsigned long long nt = sp.n_tiles, s_ = blockIdx.x;
+        t0 = sp.tile_begin + (uint32_t)(nt * s_ / S);
+        n = sp.tile_begin + (uint32_t)(nt * (s_ + 1) / S) - t0;  // ring stages (1024-record tiles) in this segment
+    }
+    if (threadIdx.x == 0)
+        for (uint32_t k = 0; k < (uint32_t)kIdxBigStages && k < n; ++k) issue(k);
     uint32_t grun[8];  // thread t keeps the running first free slot of buckets 8t..8t+7
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
         uint32_t b = threadIdx.x * 8 + k;
         grun[k] = b < B ? table[(size_t)b * stride + col] : 0u;
     }
-    if (!KEYED) stage_edges(g, s_edges);
     __syncthreads();
 
     for (uint32_t base = 0; base < n; base += kIdxBigQ) {
@@ -114,7 +136,7 @@ __global__ void __launch_bounds__(kIdxBigThreads, 1) k_scatter_idx_big(const Chu
         // stage's barrier is completed by hand so that every stage flips its phase once per use
         bool manual = false;
         for (uint32_t q = 0; q < nq; ++q) {
-            const TileDesc d = s_desc[(base + q) % kIdxBigStages];
+            const TileDesc d = s_desc[(goff + base + q) % kIdxBigStages];
             if (!bulk_ok(d.ptr, d.count * kRecB)) {
                 const uint32_t* src = reinterpret_cast<const uint32_t*>(d.ptr);
                 uint32_t* dst = stage_ptr(base + q);
@@ -126,8 +148,8 @@ __global__ void __launch_bounds__(kIdxBigThreads, 1) k_scatter_idx_big(const Chu
             __syncthreads();
             if (threadIdx.x == 0)
                 for (uint32_t q = 0; q < nq; ++q) {
-                    const TileDesc d = s_desc[(base + q) % kIdxBigStages];
-                    if (!bulk_ok(d.ptr, d.count * kRecB)) mbar_arrive(&bars[(base + q) % kIdxBigStages]);
+                    const TileDesc d = s_desc[(goff + base + q) % kIdxBigStages];
+                    if (!bulk_ok(d.ptr, d.count * kRecB)) mbar_arrive(&bars[(goff + base + q) % kIdxBigStages]);
                 }
         }
 
@@ -138,8 +160,8 @@ __global__ void __launch_bounds__(kIdxBigThreads, 1) k_scatter_idx_big(const Chu
         const uint32_t q = w / (kIdxBigWarps / kIdxBigQ);
         if (q < nq) {
             const uint32_t i = base + q;
-            const TileDesc td = s_desc[i % kIdxBigStages];
-            mbar_wait(&bars[i % kIdxBigStages], (i / kIdxBigStages) & 1u);
+            const TileDesc td = s_desc[(goff + i) % kIdxBigStages];
+            mbar_wait(&bars[(goff + i) % kIdxBigStages], ((goff + i) / kIdxBigStages) & 1u);
             const uint32_t* raw = stage_ptr(i);
             const uint32_t first = (w % (kIdxBigWarps / kIdxBigQ)) * kIdxBigSpan;
             if (KEYED) {
@@ -206,7 +228,7 @@ __global__ void __launch_bounds__(kIdxBigThreads, 1) k_scatter_idx_big(const Chu
             } else {
                 const uint32_t* p = stage_ptr(i) + ir * kRecWords;
                 if (half == 0) v = make_uint4(skey[irec], p[1], p[2], p[3]);
-                else v = make_uint4(p[4], p[5], p[6], s_desc[i % kIdxBigStages].first_index + ir);
+                else v = make_uint4(p[4], p[5], p[6], s_desc[(goff + i) % kIdxBigStages].first_index + ir);
             }
             aos_out[2 * (size_t)dest + half] = v;
         }
@@ -216,6 +238,8 @@ __global__ void __launch_bounds__(kIdxBigThreads, 1) k_scatter_idx_big(const Chu
                 if (base + kIdxBigStages + k < n) issue(base + kIdxBigStages + k);
         __syncthreads();  // the next tile reads descriptors just written
     }
+    goff += n;
+    }  // spans
 }
 
 }  // namespace psl
