@@ -128,6 +128,11 @@ typedef struct {
     uint32_t n_bins;                /* n_xbins * n_ybins */
 } psl_batch;
 
+/* Limits.  K = n_types * n_ebins * n_xbins * n_ybins keys.  PSL_MODE_ONTHEFLY: K <= 2048 (one partition pass;
+ * K <= 256 takes the 4096-record-tile scatter).  PSL_MODE_INDEX: K <= 2048 * 2048 (two passes over two balanced
+ * digits of the key).  n_ebins <= 1024, n_xbins, n_ybins <= 4096, fewer than 2^32 records per context.  Anything
+ * beyond is PSL_ERR_ARG from psl_workspace_bytes (0) / psl_create. */
+
 /* Bytes of device workspace a configuration needs (cfg->workspace* ignored).  0 on a bad configuration. */
 uint64_t psl_workspace_bytes(const psl_config* cfg);
 

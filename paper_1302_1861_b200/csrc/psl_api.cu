@@ -35,7 +35,7 @@ struct Layout {
     uint64_t total = 0;
     uint64_t raw = 0, chunks = 0, spans = 0, sstats = 0, scan_sums = 0, scalars = 0, edges = 0, stats = 0, batch_off = 0;
     // ONTHEFLY
-    uint64_t table = 0, out[10] = {0}, offsets = 0, counts = 0;
+    uint64_t table = 0, out[10] = {0}, offsets = 0, counts = 0, codes = 0;
     // INDEX
     uint64_t table_a = 0, table_b = 0, aos = 0, aos_index = 0, idx[7] = {0}, idx_offsets = 0, idx_counts = 0,
              idx_batch_off = 0;
@@ -174,6 +174,7 @@ void plan(const psl_config* c, const Derived& d, Layout* L)
         for (int i = 0; i < 10; ++i) L->out[i] = ((i == 7 || i == 8) && !proj) ? 0 : take(&cur, N * 4);
         L->offsets = take(&cur, (uint64_t)(d.K + 1) * 4);
         L->counts = take(&cur, (uint64_t)d.K * 4);
+        L->codes = take(&cur, N);  // one byte per record: the histogram kernel's verdict for the scatter of a rejecting beam
     } else {
         L->table_a = take(&cur, (uint64_t)d.B_lo * d.cols_cap * 4);
         L->table_b = take(&cur, (uint64_t)d.B_hi * kMaxSegments * 4);
@@ -203,8 +204,10 @@ void plan(const psl_config* c, const Derived& d, Layout* L)
 enum ResultKind { RES_NONE = 0, RES_OTF = 1, RES_INDEX = 2, RES_BEAM = 3 };
 
 // ---- kernel variants: the features a configuration / beam does not use are compiled out ------------------
-using CountFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, uint32_t, uint32_t*, uint32_t, SegStats*, uint32_t);
-using ScatterOtfFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, const uint32_t*, uint32_t, SoAOut, SegStats*);
+using CountFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, uint32_t, uint32_t*, uint32_t, SegStats*, uint32_t, uint8_t*);
+using ScatterOtfFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, const uint32_t*, uint32_t, SoAOut, SegStats*,
+                              const uint8_t*);
+using ScatterBigFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, const uint32_t*, uint32_t, SoAOut, SegStats*);
 using ScatterIdxAFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, uint32_t, const uint32_t*, uint32_t, uint4*);
 
 template <bool POS, bool EDGES>
@@ -238,17 +241,17 @@ ScatterOtfFn scatter_otf_fn(bool pos, bool edges, int beam, bool proj)
                : (edges ? scatter_otf_pe<false, true>(beam, proj) : scatter_otf_pe<false, false>(beam, proj));
 }
 template <bool POS, bool EDGES, bool PROJ>
-ScatterOtfFn scatter_big_pep(int beam)
+ScatterBigFn scatter_big_pep(int beam)
 {
     return beam == 0 ? k_scatter_otf_big<POS, EDGES, 0, PROJ> : (beam == 1 ? k_scatter_otf_big<POS, EDGES, 1, PROJ> : k_scatter_otf_big<POS, EDGES, 2, PROJ>);
 }
 template <bool POS, bool EDGES>
-ScatterOtfFn scatter_big_pe(int beam, bool proj)
+ScatterBigFn scatter_big_pe(int beam, bool proj)
 {
     return proj ? scatter_big_pep<POS, EDGES, true>(beam) : scatter_big_pep<POS, EDGES, false>(beam);
 }
 // the 4096-record-tile scatter (keys <= kBigMaxKeys)
-ScatterOtfFn scatter_big_fn(bool pos, bool edges, int beam, bool proj)
+ScatterBigFn scatter_big_fn(bool pos, bool edges, int beam, bool proj)
 {
     return pos ? (edges ? scatter_big_pe<true, true>(beam, proj) : scatter_big_pe<true, false>(beam, proj))
                : (edges ? scatter_big_pe<false, true>(beam, proj) : scatter_big_pe<false, false>(beam, proj));
@@ -544,10 +547,13 @@ psl_status build_onthefly(psl_ctx* ctx, const DevBeam& bm)
         const uint32_t S = nt < S_max ? nt : S_max;  // one persistent CTA per segment, one wave
         const Span span = {0u, nt, 0u, split};
         const uint32_t n_cols = S * split;
+        // a beam that rejects (jaws, zero-weight policy): the histogram kernel leaves one byte per record (key or
+        // 255 = dropped) and the scatter ranks from those instead of repeating the projection arithmetic
+        uint8_t* codes = (!big && bv != 0 && d.K <= 254) ? at<uint8_t>(ctx, L.codes) : nullptr;
         {
             Prof prof(ctx, PSL_K_COUNT);
             count_otf_fn(pos, edges, bv)<<<n_cols, kThreads, ctx->sm_count_raw, ctx->stream>>>(chunks, ctx->n_chunks, span, ctx->grid, bm, d.K, 0,
-                                                                                             table, d.cols_cap, ss, ctx->count_stages);
+                                                                                             table, d.cols_cap, ss, ctx->count_stages, codes);
             LAUNCHED();
         }
         if ((uint64_t)d.K * n_cols <= kScanSmallMax) {  // the usual case: one small kernel for scan + offsets
@@ -569,7 +575,8 @@ psl_status build_onthefly(psl_ctx* ctx, const DevBeam& bm)
                                                                                                           d.K, table, d.cols_cap, soa_out(ctx, L.out), ss);
             else
                 scatter_otf_fn(pos, edges, bv, proj)<<<S, kThreads, ctx->sm_scatter_small, ctx->stream>>>(chunks, ctx->n_chunks, span, ctx->grid, bm,
-                                                                                                       d.K, table, d.cols_cap, soa_out(ctx, L.out), ss);
+                                                                                                       d.K, table, d.cols_cap, soa_out(ctx, L.out), ss,
+                                                                                                       codes);
             LAUNCHED();
         }
         k_reduce_stats<<<1, 1024, 0, ctx->stream>>>(ss, n_cols, stats);
@@ -1074,7 +1081,7 @@ psl_status psl_load_chunk(psl_ctx* ctx, const void* records, uint64_t n, int32_t
         Prof prof(ctx, PSL_K_COUNT);
         count_idx_fn(ctx->grid.has_pos != 0, ctx->grid.ebin_mode != 0)<<<cl.n_seg * ctx->split_a, kThreads, ctx->sm_count_raw, ctx->stream>>>(
             chunks, ctx->n_chunks + 1, cl.span, ctx->grid, none, ctx->d.B_lo, (1u << ctx->d.lo_bits) - 1u,
-            at<uint32_t>(ctx, ctx->L.table_a), ctx->d.cols_cap, at<SegStats>(ctx, ctx->L.sstats), ctx->count_stages);
+            at<uint32_t>(ctx, ctx->L.table_a), ctx->d.cols_cap, at<SegStats>(ctx, ctx->L.sstats), ctx->count_stages, nullptr);
         LAUNCHED();
         ctx->idx_launches.push_back(cl);
         ctx->n_cols += cl.n_seg * ctx->split_a;

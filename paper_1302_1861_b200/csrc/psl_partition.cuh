@@ -290,7 +290,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_count_raw(const ChunkDesc* __re
                                                           const __grid_constant__ DevBeam bm, uint32_t B,
                                                           uint32_t lo_mask, uint32_t* __restrict__ table,
                                                           uint32_t stride, SegStats* __restrict__ sstats,
-                                                          uint32_t n_stages)
+                                                          uint32_t n_stages, uint8_t* __restrict__ codes)
 {
     extern __shared__ __align__(128) uint8_t smem[];
     const CountSmem L = count_layout(kTile * kRecBytes, n_stages, B, g.n_ebins + 1);
@@ -349,6 +349,10 @@ __global__ void __launch_bounds__(kThreads, 2) k_count_raw(const ChunkDesc* __re
                 const uint32_t bucket = IDX ? (key & lo_mask) : key;
                 atomicAdd(&hist[(bucket << L.rlog) + (lane_id() & rmask)], 1u);
             }
+            // one byte per record for the scatter of a rejecting beam: its key (< 255) or 255 = dropped, so that the
+            // jaw / zero-weight arithmetic is not repeated there
+            if (!IDX && codes != nullptr && have[r])
+                codes[td.first_index + r * kThreads + threadIdx.x] = (uint8_t)(cls == C_SURVIVOR ? key : 255u);
         }
         __syncthreads();  // every thread is done with the stage
         if (threadIdx.x == 0 && i + n_stages < n) {
@@ -550,7 +554,8 @@ __global__ void __launch_bounds__(kThreads, 2) k_scatter_otf(const ChunkDesc* __
                                                             Span sp, const __grid_constant__ DevGrid g,
                                                             const __grid_constant__ DevBeam bm, uint32_t B,
                                                             const uint32_t* __restrict__ table, uint32_t stride,
-                                                            SoAOut out, SegStats* __restrict__ sstats)
+                                                            SoAOut out, SegStats* __restrict__ sstats,
+                                                            const uint8_t* __restrict__ codes)
 {
     extern __shared__ __align__(128) uint8_t smem[];
     const uint32_t Bp = round_up(B, 8);
@@ -578,6 +583,15 @@ __global__ void __launch_bounds__(kThreads, 2) k_scatter_otf(const ChunkDesc* __
 
     double sum_out = 0.0;
     uint32_t phase_bits = 0;
+    uint32_t code_next[kRounds] = {255u, 255u, 255u, 255u};  // the histogram kernel's bytes for the NEXT tile
+    if (codes != nullptr && n > 0) {
+        const TileDesc nd = s_desc[0];
+#pragma unroll
+        for (int r = 0; r < kRounds; ++r) {
+            const uint32_t idx = w * kWarpSpan + r * 32 + lane_id();
+            code_next[r] = idx < nd.count ? (uint32_t)__ldg(codes + nd.first_index + idx) : 255u;
+        }
+    }
     for (uint32_t i = 0; i < n; ++i) {
         const uint32_t stage = i % kStagesRaw;
         uint32_t* raw = reinterpret_cast<uint32_t*>(smem + L.ring + stage * L.stage_bytes);
@@ -586,7 +600,20 @@ __global__ void __launch_bounds__(kThreads, 2) k_scatter_otf(const ChunkDesc* __
 
         // bucket and stable rank inside the warp's slice of the tile
         uint32_t packed[kRounds];  // bucket << 9 | rank   (bucket < 2^11, rank < 2^7)
-        {
+        if (codes != nullptr) {
+            // the histogram kernel left the key of every record (255 = dropped): nothing to decode or test here; the
+            // bytes of the next tile are fetched now and used one iteration later
+#pragma unroll
+            for (int r = 0; r < kRounds; ++r) packed[r] = code_next[r] == 255u ? kNone : code_next[r];
+            if (i + 1 < n) {
+                const TileDesc nd = s_desc[(i + 1) % kStagesRaw];
+#pragma unroll
+                for (int r = 0; r < kRounds; ++r) {
+                    const uint32_t idx = w * kWarpSpan + r * 32 + lane_id();
+                    code_next[r] = idx < nd.count ? (uint32_t)__ldg(codes + nd.first_index + idx) : 255u;
+                }
+            }
+        } else {
             Rec rec[kRounds];
 #pragma unroll
             for (int r = 0; r < kRounds; ++r) {
@@ -600,12 +627,12 @@ __global__ void __launch_bounds__(kThreads, 2) k_scatter_otf(const ChunkDesc* __
                 int cls = classify<POS, EDGES, BEAM>(g, bm, rec[r], s_edges, key);
                 packed[r] = (idx < (int)td.count && cls == C_SURVIVOR) ? key : kNone;
             }
+        }
 #pragma unroll
-            for (int r = 0; r < kRounds; ++r) {  // ranks: round r before round r + 1
-                uint32_t bucket = packed[r];
-                uint32_t rank = warp_rank(bucket, cnt + w * Bp);
-                packed[r] = bucket == kNone ? kNone : ((bucket << 9) | rank);
-            }
+        for (int r = 0; r < kRounds; ++r) {  // ranks: round r before round r + 1
+            uint32_t bucket = packed[r];
+            uint32_t rank = warp_rank(bucket, cnt + w * Bp);
+            packed[r] = bucket == kNone ? kNone : ((bucket << 9) | rank);
         }
         __syncthreads();
         const uint32_t n_part = finish_ranks<true>(cnt, B, Bp, gcur, lstart, misc, grun);
