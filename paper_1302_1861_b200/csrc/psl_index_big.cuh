@@ -7,7 +7,7 @@
 // write consecutive 16-byte halves of consecutive slots, so one request covers a whole run.
 //
 // One 512-thread CTA per SM: the tile is 4 ring stages of 1024 records that stay where TMA put them, a fifth
-// stage prefetches.  Warp w owns records [256 w, 256 w + 256) of the tile (a quarter of a stage): per-warp private
+// (pass B) or fifth and sixth (pass A) stage prefetch.  Warp w owns records [256 w, 256 w + 256) of the tile (a quarter of a stage): per-warp private
 // uint16 counters + __match_any_sync give stable ranks, finish_ranks the prefix over the 16 warps.
 #pragma once
 
@@ -17,14 +17,15 @@ namespace psl {
 
 constexpr int kIdxBigQ = 4;                               // ring stages per tile
 constexpr int kIdxBigTile = kIdxBigQ * kTile;             // 4096 records
-constexpr int kIdxBigStages = 5;
+constexpr int kIdxBigStagesRaw = 6;    // pass A: 4 being worked on + 2 in flight (28 KB each)
+constexpr int kIdxBigStagesKeyed = 5;  // pass B: 4 + 1 (32 KB each)
 constexpr int kIdxBigThreads = 512;
 constexpr int kIdxBigWarps = kIdxBigThreads / 32;         // 16
 constexpr int kIdxBigSpan = kIdxBigTile / kIdxBigWarps;   // 256 records per warp
 constexpr int kIdxBigRounds = kIdxBigSpan / 32;           // 8
 
 struct IdxBigSmem {
-    uint32_t ring, stage_bytes, cnt, gcur, lstart, perm, pbkt, skey, edges, misc, desc, bars, total;
+    uint32_t ring, stage_bytes, cnt, gcur, lstart, perm, pbkt, edges, misc, desc, bars, total;
 };
 
 __host__ __device__ inline IdxBigSmem idx_big_layout(bool keyed, uint32_t B, uint32_t n_edges)
@@ -32,17 +33,17 @@ __host__ __device__ inline IdxBigSmem idx_big_layout(bool keyed, uint32_t B, uin
     IdxBigSmem L;
     uint32_t p = 0;
     L.stage_bytes = round_up(kTile * (keyed ? 32 : kRecBytes), 128);
-    L.ring = p;   p += kIdxBigStages * L.stage_bytes;
+    const uint32_t stages = keyed ? kIdxBigStagesKeyed : kIdxBigStagesRaw;
+    L.ring = p;   p += stages * L.stage_bytes;
     L.cnt = p;    p += round_up(kIdxBigWarps * round_up(B, 8) * 2, 16);
     L.gcur = p;   p += round_up(B * 4, 16);
     L.lstart = p; p += round_up(B * 4, 16);
     L.perm = p;   p += kIdxBigTile * 2;                   // tile-sorted slot -> record in tile
     L.pbkt = p;   p += kIdxBigTile * 2;                   // tile-sorted slot -> bucket
-    L.skey = p;   if (!keyed) p += kIdxBigTile * 4;       // pass A: the full key of every record
     L.edges = p;  p += round_up(n_edges * 4, 16);
     L.misc = p;   p += 64 * 4;
-    L.desc = p;   p += kIdxBigStages * 16;
-    L.bars = p;   p += kIdxBigStages * 8;
+    L.desc = p;   p += stages * 16;
+    L.bars = p;   p += stages * 8;
     L.total = p;
     return L;
 }
@@ -68,6 +69,7 @@ __global__ void __launch_bounds__(kIdxBigThreads, 1) k_scatter_idx_big(const Chu
 {
     extern __shared__ __align__(128) uint8_t smem[];
     constexpr uint32_t kRecB = KEYED ? 32u : (uint32_t)kRecBytes;
+    constexpr uint32_t kIdxBigStages = KEYED ? kIdxBigStagesKeyed : kIdxBigStagesRaw;
     const uint32_t Bp = round_up(B, 8);
     const IdxBigSmem L = idx_big_layout(KEYED, B, g.n_ebins + 1);
     uint16_t* cnt = reinterpret_cast<uint16_t*>(smem + L.cnt);
@@ -75,7 +77,6 @@ __global__ void __launch_bounds__(kIdxBigThreads, 1) k_scatter_idx_big(const Chu
     uint32_t* lstart = reinterpret_cast<uint32_t*>(smem + L.lstart);
     uint16_t* perm = reinterpret_cast<uint16_t*>(smem + L.perm);
     uint16_t* pbkt = reinterpret_cast<uint16_t*>(smem + L.pbkt);
-    uint32_t* skey = reinterpret_cast<uint32_t*>(smem + L.skey);
     float* s_edges = reinterpret_cast<float*>(smem + L.edges);
     uint32_t* misc = reinterpret_cast<uint32_t*>(smem + L.misc);
     TileDesc* s_desc = reinterpret_cast<TileDesc*>(smem + L.desc);
@@ -162,7 +163,7 @@ __global__ void __launch_bounds__(kIdxBigThreads, 1) k_scatter_idx_big(const Chu
             const uint32_t i = base + q;
             const TileDesc td = s_desc[(goff + i) % kIdxBigStages];
             mbar_wait(&bars[(goff + i) % kIdxBigStages], ((goff + i) / kIdxBigStages) & 1u);
-            const uint32_t* raw = stage_ptr(i);
+            uint32_t* raw = stage_ptr(i);
             const uint32_t first = (w % (kIdxBigWarps / kIdxBigQ)) * kIdxBigSpan;
             if (KEYED) {
 #pragma unroll
@@ -185,7 +186,8 @@ __global__ void __launch_bounds__(kIdxBigThreads, 1) k_scatter_idx_big(const Chu
                         uint32_t key;
                         const int cls = classify<POS, EDGES, 0>(g, bm, rec[r], s_edges, key);
                         const bool keep = idx < td.count && cls == C_SURVIVOR;
-                        skey[q * kTile + idx] = keep ? key : kNone;
+                        // the key takes the place of the type word of the staged record (the type is part of the key)
+                        if (idx < td.count) raw[idx * kRecWords] = keep ? key : kNone;
                         packed[h + r] = keep ? (key & lo_mask) : kNone;
                     }
                 }
@@ -227,12 +229,12 @@ __global__ void __launch_bounds__(kIdxBigThreads, 1) k_scatter_idx_big(const Chu
                 v = reinterpret_cast<const uint4*>(stage_ptr(i))[2 * ir + half];
             } else {
                 const uint32_t* p = stage_ptr(i) + ir * kRecWords;
-                if (half == 0) v = make_uint4(skey[irec], p[1], p[2], p[3]);
+                if (half == 0) v = make_uint4(p[0], p[1], p[2], p[3]);
                 else v = make_uint4(p[4], p[5], p[6], s_desc[(goff + i) % kIdxBigStages].first_index + ir);
             }
             aos_out[2 * (size_t)dest + half] = v;
         }
-        __syncthreads();  // the tile's stages, perm, pbkt and skey are free again
+        __syncthreads();  // the tile's stages, perm and pbkt are free again
         if (threadIdx.x == 0)
             for (uint32_t k = 0; k < nq; ++k)
                 if (base + kIdxBigStages + k < n) issue(base + kIdxBigStages + k);
