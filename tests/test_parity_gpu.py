@@ -389,3 +389,23 @@ def test_index_digit_split_extremes():
     ctx = run_library(wh, r, beam)
     assert_matches_oracle(library_result(ctx), O.Oracle(huge, w.geometry).build(r, beam))
     ctx.destroy()
+
+
+def test_config3_full_size_element_by_element():
+    """config 3 as bench.py times it: 5e7 records, jaws 30x30 at isocentre, 160x160 fluence map, one device chunk"""
+    w = W.config(3)
+    r = w.records()
+    check(w, r, w.beams[0], mem="device")
+
+
+def test_config4_full_size_index_and_beam():
+    """config 4 as bench.py times it: 2e8 records -> PSL index over 1 228 800 keys -> the 10x10 beam with its ROI.
+    The whole index (counts, offsets, permutation, copied fields) and the beam's batches against the oracle."""
+    w = W.config(4)
+    r = w.records()
+    orc = O.Oracle(w.grid, w.geometry)
+    ctx = run_library(w, r, None, mem="device")
+    assert_matches_oracle(library_result(ctx), orc.build(r, None), index_only=True)
+    ctx.build_batches(w.beams[0])
+    assert_matches_oracle(library_result(ctx), orc.build(r, w.beams[0]))
+    ctx.destroy()
