@@ -409,3 +409,31 @@ def test_config4_full_size_index_and_beam():
     ctx.build_batches(w.beams[0])
     assert_matches_oracle(library_result(ctx), orc.build(r, w.beams[0]))
     ctx.destroy()
+
+
+def test_hundreds_of_small_chunks_and_index_determinism():
+    """295 chunks of 68 records and 13 chunks of ~5000: INDEX pass A walks one span per chunk inside ONE launch (ring
+    stage and barrier-parity bookkeeping runs on across spans); ONTHEFLY gets tiles of 68 records.  Then the INDEX
+    build twice: bit-identical outputs and statistics from run to run."""
+    w4 = W.config(4, 20_060)
+    r4 = dirty(w4.records(), 21)
+    orc = O.Oracle(w4.grid, w4.geometry)
+    want_idx, want_beam = orc.build(r4, None), orc.build(r4, w4.beams[0])
+    outs = []
+    for chunk in (68, 5000, 68):
+        ctx = run_library(w4, r4, None, chunk=chunk, mem="device")
+        a = library_result(ctx)
+        assert_matches_oracle(a, want_idx, index_only=True)
+        ctx.build_batches(w4.beams[0])
+        b = library_result(ctx)
+        assert_matches_oracle(b, want_beam)
+        outs.append((a, b))
+        ctx.destroy()
+    for k in ("E", "wt", "src_index", "counts", "offsets"):
+        assert np.array_equal(outs[0][0][k].view(np.uint32), outs[2][0][k].view(np.uint32))
+        assert np.array_equal(outs[0][1][k].view(np.uint32), outs[2][1][k].view(np.uint32))
+    assert outs[0][1]["stats"] == outs[2][1]["stats"]  # including the double sums: fixed reduction order
+    w2 = W.config(2, 20_060)
+    check(w2, dirty(w2.records(), 22), None, chunk=68, mem="device")
+    w3 = W.config(3, 20_060)
+    check(w3, w3.records(), w3.beams[0], chunk=68, mem="pinned")
