@@ -437,3 +437,33 @@ def test_hundreds_of_small_chunks_and_index_determinism():
     check(w2, dirty(w2.records(), 22), None, chunk=68, mem="device")
     w3 = W.config(3, 20_060)
     check(w3, w3.records(), w3.beams[0], chunk=68, mem="pinned")
+
+
+def test_config5_streamed_at_1e8_records_nine_beams():
+    """config 5 at a tenth of its size, in the launch configuration bench.py times: 1e8 records in pinned host
+    memory, streamed in 268 435 440-byte chunks (9 586 980 records) through the copy stream while the histogram of
+    the previous chunk runs, one index, nine IMRT beams -- every beam's batches against the oracle."""
+    import torch
+
+    p = P()
+    w = W.config(5, 100_000_000)
+    chunk = W.config(5).chunk_records
+    n = w.n_records
+    host = torch.empty(n * 28, dtype=torch.uint8).pin_memory()
+    W.generate_into(w.gen, 0, n, host.data_ptr(), threads=8)
+    r = host.numpy().view(W.RECORD_DTYPE)
+    ctx = p.PslContext(w.grid, w.geometry, w.mode, max_records=n, max_chunks=n // chunk + 2)
+    for f in range(0, n, chunk):
+        ctx.load_chunk(host[f * 28:min(n, f + chunk) * 28], p.MEM_PINNED)
+    orc = O.Oracle(w.grid, w.geometry)
+    for k, beam in enumerate(w.beams):
+        ctx.build_batches(beam)
+        if k in (0, 4, 8):  # three of the nine against the oracle element by element, the rest by their statistics
+            assert_matches_oracle(library_result(ctx), orc.build(r, beam))
+        else:
+            st = ctx.get_stats()
+            c, o = ctx.get_tables()
+            assert int(c.sum().item()) == st["n_survivors"] == int(o[-1].item())
+            assert st["n_in"] == n and st["n_survivors"] + st["n_jaw_rejected"] + st["n_roi_skipped"] + st["n_invalid"] + \
+                st["n_outside_grid"] + st["n_zero_weight"] == n
+    ctx.destroy()
