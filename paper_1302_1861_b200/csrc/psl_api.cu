@@ -207,7 +207,7 @@ enum ResultKind { RES_NONE = 0, RES_OTF = 1, RES_INDEX = 2, RES_BEAM = 3 };
 using CountFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, uint32_t, uint32_t*, uint32_t, SegStats*, uint32_t, uint8_t*);
 using ScatterOtfFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, const uint32_t*, uint32_t, SoAOut, SegStats*,
                               const uint8_t*);
-using ScatterBigFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, const uint32_t*, uint32_t, SoAOut, SegStats*);
+using ScatterBigFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, const uint32_t*, uint32_t, SoAOut, SegStats*, FusedScan);
 using ScatterIdxAFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, uint32_t, const uint32_t*, uint32_t, uint4*);
 
 template <bool POS, bool EDGES>
@@ -556,7 +556,13 @@ psl_status build_onthefly(psl_ctx* ctx, const DevBeam& bm)
                                                                                              table, d.cols_cap, ss, ctx->count_stages, codes);
             LAUNCHED();
         }
-        if ((uint64_t)d.K * n_cols <= kScanSmallMax) {  // the usual case: one small kernel for scan + offsets
+        // 4096-record tiles: the table is small and stays raw -- the scatter CTAs scan it themselves (fused_first_slots)
+        FusedScan fs;
+        memset(&fs, 0, sizeof fs);
+        if (big) {
+            fs.n_cols = n_cols; fs.n_pos = d.n_pos; fs.n_batches = d.n_batches;
+            fs.total_out = scalar(ctx, SC_TOTAL); fs.offsets = offsets; fs.counts = counts; fs.batch_offsets = batch_off;
+        } else if ((uint64_t)d.K * n_cols <= kScanSmallMax) {  // one small kernel for scan + offsets
             Prof prof(ctx, PSL_K_SCAN);
             k_scan_small<<<1, 1024, 0, ctx->stream>>>(table, n_cols, d.cols_cap, d.K, scalar(ctx, SC_TOTAL), d.K, offsets,
                                                       counts, d.n_pos, d.n_batches, batch_off);
@@ -572,7 +578,7 @@ psl_status build_onthefly(psl_ctx* ctx, const DevBeam& bm)
             Prof prof(ctx, PSL_K_SCATTER);
             if (big)
                 scatter_big_fn(pos, edges, bv, proj)<<<S, kBigThreads, ctx->sm_scatter_otf, ctx->stream>>>(chunks, ctx->n_chunks, span, ctx->grid, bm,
-                                                                                                          d.K, table, d.cols_cap, soa_out(ctx, L.out), ss);
+                                                                                                          d.K, table, d.cols_cap, soa_out(ctx, L.out), ss, fs);
             else
                 scatter_otf_fn(pos, edges, bv, proj)<<<S, kThreads, ctx->sm_scatter_small, ctx->stream>>>(chunks, ctx->n_chunks, span, ctx->grid, bm,
                                                                                                        d.K, table, d.cols_cap, soa_out(ctx, L.out), ss,

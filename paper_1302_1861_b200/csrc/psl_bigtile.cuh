@@ -58,7 +58,7 @@ __global__ void __launch_bounds__(kBigThreads, 1) k_scatter_otf_big(const ChunkD
                                                                    Span sp, const __grid_constant__ DevGrid g,
                                                                    const __grid_constant__ DevBeam bm, uint32_t B,
                                                                    const uint32_t* __restrict__ table, uint32_t stride,
-                                                                   SoAOut out, SegStats* __restrict__ sstats)
+                                                                   SoAOut out, SegStats* __restrict__ sstats, const FusedScan fs)
 {
     extern __shared__ __align__(128) uint8_t smem[];
     const uint32_t Bp = round_up(B, 8);
@@ -95,10 +95,14 @@ __global__ void __launch_bounds__(kBigThreads, 1) k_scatter_otf_big(const ChunkD
         for (uint32_t i = threadIdx.x; i < kBigWarps * Bp / 2; i += kBigThreads) cz[i] = 0;
     }
     uint32_t grun[8];
+    if (fs.n_cols != 0) {
+        fused_first_slots<kBigWarps>(fs, table, stride, B, col, gcur, lstart, misc, grun);
+    } else {
 #pragma unroll
-    for (int k = 0; k < 8; ++k) {
-        uint32_t b = threadIdx.x * 8 + k;
-        grun[k] = b < B ? table[(size_t)b * stride + col] : 0u;
+        for (int k = 0; k < 8; ++k) {
+            uint32_t b = threadIdx.x * 8 + k;
+            grun[k] = b < B ? table[(size_t)b * stride + col] : 0u;
+        }
     }
     stage_edges(g, s_edges);
     __syncthreads();

@@ -502,6 +502,104 @@ __global__ void __launch_bounds__(1024) k_scan_small(uint32_t* __restrict__ tabl
     }
 }
 
+// The same scan folded into the scatter kernel's prologue (small tables only): the table keeps the RAW counts
+// and every scatter CTA derives its own first slots -- row totals (-> key offsets, scanned by warp 0) plus the
+// sum of the row's columns before its own.  The table sits in L2 (the histogram kernel has just written it), the
+// reads overlap the first record copies, and one kernel launch plus its serial 25 us leave the step.
+// CTA 0 also writes what k_scan_small writes for the host (offsets, counts, batch offsets, total).
+struct FusedScan {
+    uint32_t n_cols;  // 0: the table is already scanned
+    uint32_t n_pos, n_batches;
+    uint32_t *total_out, *offsets, *counts, *batch_offsets;
+};
+
+// On return (after a __syncthreads() by the caller before s_off / s_part are reused) grun[k] holds the first slot
+// of bucket 8 * threadIdx.x + k for this CTA's column.  B <= 256; s_off, s_part: B words each; NW warps.
+template <int NW>
+__device__ __forceinline__ void fused_first_slots(const FusedScan& fs, const uint32_t* __restrict__ table, uint32_t stride,
+                                                  uint32_t B, uint32_t col, uint32_t* s_off, uint32_t* s_part,
+                                                  uint32_t* s_total, uint32_t (&grun)[8])
+{
+    const uint32_t w = warp_id(), lane = lane_id();
+    // Four rows x 320 columns of loads in flight per warp (the loop is L2 round trips, not bytes); CTAs start at
+    // different rows so that they do not all ask the same L2 slice for the same line at once.
+    constexpr int kRowsInFlight = 4, kPieces = 10;
+    const uint32_t rot = (blockIdx.x * 13u) % B;
+    for (uint32_t j0 = w; j0 < B; j0 += kRowsInFlight * NW) {
+        uint32_t tot[kRowsInFlight], part[kRowsInFlight];
+#pragma unroll
+        for (int a = 0; a < kRowsInFlight; ++a) tot[a] = part[a] = 0u;
+        for (uint32_t c0 = 0; c0 < fs.n_cols; c0 += 32 * kPieces) {
+            uint32_t v[kRowsInFlight][kPieces];
+#pragma unroll
+            for (int a = 0; a < kRowsInFlight; ++a) {
+                const uint32_t j = j0 + a * NW;
+                const uint32_t row = j + rot < B ? j + rot : j + rot - B;
+                const uint32_t* r = table + (size_t)(j < B ? row : 0u) * stride;
+#pragma unroll
+                for (int k = 0; k < kPieces; ++k) {
+                    const uint32_t c = c0 + k * 32 + lane;
+                    v[a][k] = (j < B && c < fs.n_cols) ? r[c] : 0u;
+                }
+            }
+#pragma unroll
+            for (int a = 0; a < kRowsInFlight; ++a)
+#pragma unroll
+                for (int k = 0; k < kPieces; ++k) {
+                    const uint32_t c = c0 + k * 32 + lane;
+                    tot[a] += v[a][k];
+                    part[a] += c < col ? v[a][k] : 0u;
+                }
+        }
+#pragma unroll
+        for (int a = 0; a < kRowsInFlight; ++a) {
+            const uint32_t j = j0 + a * NW;
+            const uint32_t row = j + rot < B ? j + rot : j + rot - B;
+            const uint32_t t = __reduce_add_sync(0xFFFFFFFFu, tot[a]);
+            const uint32_t q = __reduce_add_sync(0xFFFFFFFFu, part[a]);
+            if (lane == 0 && j < B) {
+                s_off[row] = t;
+                s_part[row] = q;
+            }
+        }
+    }
+    __syncthreads();
+    if (w == 0) {  // exclusive scan of the row totals: lane takes rows 8 * lane .. 8 * lane + 7
+        uint32_t v[8], s = 0;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            const uint32_t b = lane * 8 + k;
+            v[k] = b < B ? s_off[b] : 0u;
+            s += v[k];
+        }
+        const uint32_t inc = warp_incl_scan(s);
+        uint32_t ex = inc - s;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            const uint32_t b = lane * 8 + k;
+            if (b < B) s_off[b] = ex;
+            ex += v[k];
+        }
+        if (lane == 31) *s_total = inc;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        const uint32_t b = threadIdx.x * 8 + k;
+        grun[k] = b < B ? s_off[b] + s_part[b] : 0u;
+    }
+    if (blockIdx.x == 0) {
+        const uint32_t total = *s_total;
+        if (threadIdx.x == 0) *fs.total_out = total;
+        for (uint32_t k = threadIdx.x; k <= B; k += blockDim.x) {
+            const uint32_t o = (k < B) ? s_off[k] : total;
+            fs.offsets[k] = o;
+            if (k < B) fs.counts[k] = ((k + 1 < B) ? s_off[k + 1] : total) - o;
+            if (k % fs.n_pos == 0 && k / fs.n_pos <= fs.n_batches) fs.batch_offsets[k / fs.n_pos] = o;
+        }
+    }
+}
+
 // ONTHEFLY: offsets[k] = first slot of key k = scanned table[k][0]; counts; per-(type,energy) batch offsets.
 __global__ void k_offsets_from_table(const uint32_t* __restrict__ table, uint32_t stride, uint32_t K,
                                      const uint32_t* __restrict__ total, uint32_t* __restrict__ offsets,
