@@ -207,7 +207,7 @@ enum ResultKind { RES_NONE = 0, RES_OTF = 1, RES_INDEX = 2, RES_BEAM = 3 };
 using CountFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, uint32_t, uint32_t*, uint32_t, SegStats*, uint32_t, uint8_t*);
 using ScatterOtfFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, const uint32_t*, uint32_t, SoAOut, SegStats*,
                               const uint8_t*);
-using ScatterBigFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, const uint32_t*, uint32_t, SoAOut, SegStats*, FusedScan);
+using ScatterBigFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, const uint32_t*, uint32_t, SoAOut, SegStats*, FusedScan, StatsTail);
 using ScatterIdxAFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, uint32_t, const uint32_t*, uint32_t, uint4*);
 
 template <bool POS, bool EDGES>
@@ -289,6 +289,8 @@ struct psl_ctx {
     uint32_t* h_idx_offsets = nullptr; // K+1 (INDEX)
     uint32_t* h_seg = nullptr;         // 3*max_seg+1
     DevStats* h_stats = nullptr;
+    DevStats* d_h_stats = nullptr;      // device views of the pinned copies (null: not mapped, copies are used)
+    uint32_t* d_h_batch_off = nullptr;
     DevBeamStats* h_beam_stats = nullptr;
     uint32_t* h_scalars = nullptr;
     bool seg_pending = false;
@@ -381,7 +383,7 @@ template <typename T>
 T* at(psl_ctx* ctx, uint64_t off) { return reinterpret_cast<T*>(ctx->ws + off); }
 
 uint32_t* scalar(psl_ctx* ctx, int i) { return at<uint32_t>(ctx, ctx->L.scalars) + i; }
-enum { SC_TOTAL = 0, SC_NIDX = 1, SC_TILE_COUNTER = 2, SC_BEAM_NSURV = 3 };
+enum { SC_TOTAL = 0, SC_NIDX = 1, SC_TILE_COUNTER = 2, SC_BEAM_NSURV = 3, SC_TICKET = 4 };
 
 DevGrid make_grid(const psl_config& c, const Derived& d, const float* dev_edges)
 {
@@ -521,6 +523,8 @@ psl_status build_onthefly(psl_ctx* ctx, const DevBeam& bm)
     uint32_t* batch_off = at<uint32_t>(ctx, L.batch_off);
     DevStats* stats = at<DevStats>(ctx, L.stats);
     const uint32_t nt = ctx->n_tiles;
+    StatsTail tail;
+    bool to_host = false;
     if (nt == 0) {
         CU(cudaMemsetAsync(offsets, 0, (uint64_t)(d.K + 1) * 4, ctx->stream));
         CU(cudaMemsetAsync(counts, 0, (uint64_t)d.K * 4, ctx->stream));
@@ -559,7 +563,13 @@ psl_status build_onthefly(psl_ctx* ctx, const DevBeam& bm)
         // 4096-record tiles: the table is small and stays raw -- the scatter CTAs scan it themselves (fused_first_slots)
         FusedScan fs;
         memset(&fs, 0, sizeof fs);
+        memset(&tail, 0, sizeof tail);
         if (big) {
+            // ... and the last of them to finish reduces the statistics; both results go straight to the mapped
+            // pinned copies the host reads (no reduce launch, no device-to-host copies behind the scatter)
+            tail.n_cols = n_cols; tail.ticket = scalar(ctx, SC_TICKET); tail.out = stats; tail.out_host = ctx->d_h_stats;
+            fs.batch_offsets_host = ctx->d_h_batch_off;
+            to_host = ctx->d_h_stats != nullptr && ctx->d_h_batch_off != nullptr;
             fs.n_cols = n_cols; fs.n_pos = d.n_pos; fs.n_batches = d.n_batches;
             fs.total_out = scalar(ctx, SC_TOTAL); fs.offsets = offsets; fs.counts = counts; fs.batch_offsets = batch_off;
         } else if ((uint64_t)d.K * n_cols <= kScanSmallMax) {  // one small kernel for scan + offsets
@@ -578,18 +588,22 @@ psl_status build_onthefly(psl_ctx* ctx, const DevBeam& bm)
             Prof prof(ctx, PSL_K_SCATTER);
             if (big)
                 scatter_big_fn(pos, edges, bv, proj)<<<S, kBigThreads, ctx->sm_scatter_otf, ctx->stream>>>(chunks, ctx->n_chunks, span, ctx->grid, bm,
-                                                                                                          d.K, table, d.cols_cap, soa_out(ctx, L.out), ss, fs);
+                                                                                                          d.K, table, d.cols_cap, soa_out(ctx, L.out), ss, fs, tail);
             else
                 scatter_otf_fn(pos, edges, bv, proj)<<<S, kThreads, ctx->sm_scatter_small, ctx->stream>>>(chunks, ctx->n_chunks, span, ctx->grid, bm,
                                                                                                        d.K, table, d.cols_cap, soa_out(ctx, L.out), ss,
                                                                                                        codes);
             LAUNCHED();
         }
-        k_reduce_stats<<<1, 1024, 0, ctx->stream>>>(ss, n_cols, stats);
-        LAUNCHED();
+        if (tail.n_cols == 0) {
+            k_reduce_stats<<<1, 1024, 0, ctx->stream>>>(ss, n_cols, stats);
+            LAUNCHED();
+        }
     }
-    CU(cudaMemcpyAsync(ctx->h_batch_off, batch_off, (uint64_t)(d.n_batches + 1) * 4, cudaMemcpyDeviceToHost, ctx->stream));
-    CU(cudaMemcpyAsync(ctx->h_stats, stats, sizeof(DevStats), cudaMemcpyDeviceToHost, ctx->stream));
+    if (!to_host) {
+        CU(cudaMemcpyAsync(ctx->h_batch_off, batch_off, (uint64_t)(d.n_batches + 1) * 4, cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaMemcpyAsync(ctx->h_stats, stats, sizeof(DevStats), cudaMemcpyDeviceToHost, ctx->stream));
+    }
     CU(cudaEventRecord(ctx->ev_batch, ctx->stream));
     ctx->result = RES_OTF;
     return PSL_OK;
@@ -916,8 +930,15 @@ psl_status psl_create(const psl_config* cfg, psl_ctx** out)
     CUC(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
     cudaEvent_t* evs[] = {&ctx->ev_chunk, &ctx->ev_main, &ctx->ev_batch, &ctx->ev_seg, &ctx->ev_stage[0], &ctx->ev_stage[1]};
     for (cudaEvent_t* e : evs) CUC(cudaEventCreateWithFlags(e, cudaEventDisableTiming));
-    CUC(cudaHostAlloc(&ctx->h_batch_off, (uint64_t)(d.n_batches + 1) * 4, cudaHostAllocDefault));
-    CUC(cudaHostAlloc(&ctx->h_stats, sizeof(DevStats), cudaHostAllocDefault));
+    CUC(cudaHostAlloc(&ctx->h_batch_off, (uint64_t)(d.n_batches + 1) * 4, cudaHostAllocMapped));
+    CUC(cudaHostAlloc(&ctx->h_stats, sizeof(DevStats), cudaHostAllocMapped));
+    if (cudaHostGetDevicePointer(&ctx->d_h_stats, ctx->h_stats, 0) != cudaSuccess ||
+        cudaHostGetDevicePointer(&ctx->d_h_batch_off, ctx->h_batch_off, 0) != cudaSuccess) {
+        (void)cudaGetLastError();
+        ctx->d_h_stats = nullptr;
+        ctx->d_h_batch_off = nullptr;
+    }
+    CUC(cudaMemsetAsync(at<uint8_t>(ctx, L.scalars), 0, 64, ctx->stream));
     CUC(cudaHostAlloc(&ctx->h_beam_stats, sizeof(DevBeamStats), cudaHostAllocDefault));
     CUC(cudaHostAlloc(&ctx->h_scalars, 64, cudaHostAllocDefault));
     if (cfg->mode == PSL_MODE_INDEX) {

@@ -58,7 +58,8 @@ __global__ void __launch_bounds__(kBigThreads, 1) k_scatter_otf_big(const ChunkD
                                                                    Span sp, const __grid_constant__ DevGrid g,
                                                                    const __grid_constant__ DevBeam bm, uint32_t B,
                                                                    const uint32_t* __restrict__ table, uint32_t stride,
-                                                                   SoAOut out, SegStats* __restrict__ sstats, const FusedScan fs)
+                                                                   SoAOut out, SegStats* sstats, const FusedScan fs,
+                                                                   const StatsTail st)
 {
     extern __shared__ __align__(128) uint8_t smem[];
     const uint32_t Bp = round_up(B, 8);
@@ -229,6 +230,7 @@ __global__ void __launch_bounds__(kBigThreads, 1) k_scatter_otf_big(const ChunkD
         for (int k = 0; k < kBigWarps; ++k) t += s_d[k];
         sstats[col].sum_out = t;
     }
+    stats_tail(st, sstats);
 }
 
 }  // namespace psl

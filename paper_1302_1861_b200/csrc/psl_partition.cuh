@@ -511,6 +511,7 @@ struct FusedScan {
     uint32_t n_cols;  // 0: the table is already scanned
     uint32_t n_pos, n_batches;
     uint32_t *total_out, *offsets, *counts, *batch_offsets;
+    uint32_t* batch_offsets_host;  // mapped pinned copy of batch_offsets (may be null)
 };
 
 // On return (after a __syncthreads() by the caller before s_off / s_part are reused) grun[k] holds the first slot
@@ -595,7 +596,10 @@ __device__ __forceinline__ void fused_first_slots(const FusedScan& fs, const uin
             const uint32_t o = (k < B) ? s_off[k] : total;
             fs.offsets[k] = o;
             if (k < B) fs.counts[k] = ((k + 1 < B) ? s_off[k + 1] : total) - o;
-            if (k % fs.n_pos == 0 && k / fs.n_pos <= fs.n_batches) fs.batch_offsets[k / fs.n_pos] = o;
+            if (k % fs.n_pos == 0 && k / fs.n_pos <= fs.n_batches) {
+                fs.batch_offsets[k / fs.n_pos] = o;
+                if (fs.batch_offsets_host != nullptr) fs.batch_offsets_host[k / fs.n_pos] = o;
+            }
         }
     }
 }
@@ -838,17 +842,21 @@ struct DevStats {
     double sum_in, sum_idx, sum_out;
 };
 
-__global__ void __launch_bounds__(1024) k_reduce_stats(const SegStats* __restrict__ ts, uint32_t n_cols,
-                                                       DevStats* __restrict__ out)
+// the reduction proper, by one CTA of any size; out_host (may be null) is the mapped pinned copy the host reads
+__device__ __forceinline__ void reduce_stats_cta(const SegStats* ts, uint32_t n_cols, DevStats* out, DevStats* out_host)
 {
     __shared__ unsigned long long s_n[32][5];
     __shared__ double s_d[32][3];
     unsigned long long n[5] = {0, 0, 0, 0, 0};
     double d[3] = {0.0, 0.0, 0.0};
-    for (uint32_t t = threadIdx.x; t < n_cols; t += 1024) {
-        SegStats x = ts[t];
-        n[0] += x.n_invalid; n[1] += x.n_outside; n[2] += x.n_jaw; n[3] += x.n_zero; n[4] += x.n_surv;
-        d[0] += x.sum_in; d[1] += x.sum_idx; d[2] += x.sum_out;
+    for (uint32_t t = threadIdx.x; t < n_cols; t += blockDim.x) {
+        // L2 loads: the records may have been written by other CTAs of the running kernel (stats_tail)
+        const uint4* p = reinterpret_cast<const uint4*>(ts + t);
+        const uint4 a = __ldcg(p), b = __ldcg(p + 1), c = __ldcg(p + 2);
+        n[0] += a.x; n[1] += a.y; n[2] += a.z; n[3] += a.w; n[4] += b.x;
+        d[0] += __hiloint2double((int)b.w, (int)b.z);
+        d[1] += __hiloint2double((int)c.y, (int)c.x);
+        d[2] += __hiloint2double((int)c.w, (int)c.z);
     }
     for (int k = 0; k < 5; ++k)
         for (int o = 16; o > 0; o >>= 1) n[k] += __shfl_xor_sync(0xFFFFFFFFu, n[k], o);
@@ -860,13 +868,43 @@ __global__ void __launch_bounds__(1024) k_reduce_stats(const SegStats* __restric
     __syncthreads();
     if (threadIdx.x == 0) {
         DevStats r = {0, 0, 0, 0, 0, 0.0, 0.0, 0.0};
-        for (int w = 0; w < 32; ++w) {
+        for (uint32_t w = 0; w < blockDim.x / 32; ++w) {
             r.n_invalid += s_n[w][0]; r.n_outside += s_n[w][1]; r.n_jaw += s_n[w][2]; r.n_zero += s_n[w][3];
             r.n_surv += s_n[w][4];
             r.sum_in += s_d[w][0]; r.sum_idx += s_d[w][1]; r.sum_out += s_d[w][2];
         }
         *out = r;
+        if (out_host != nullptr) *out_host = r;
     }
+}
+
+__global__ void __launch_bounds__(1024) k_reduce_stats(const SegStats* __restrict__ ts, uint32_t n_cols,
+                                                       DevStats* __restrict__ out)
+{
+    reduce_stats_cta(ts, n_cols, out, nullptr);
+}
+
+// The same reduction as the tail of a scatter kernel: each CTA, having written its SegStats, takes a ticket; the
+// last one reduces all n_cols records in the same fixed order and leaves the ticket at zero for the next launch.
+struct StatsTail {
+    uint32_t n_cols;  // 0: off (k_reduce_stats follows)
+    uint32_t* ticket;
+    DevStats *out, *out_host;
+};
+
+__device__ __forceinline__ void stats_tail(const StatsTail& st, const SegStats* sstats)
+{
+    if (st.n_cols == 0) return;
+    __shared__ uint32_t s_last;
+    if (threadIdx.x == 0) {
+        __threadfence();  // this CTA's SegStats before its ticket
+        s_last = atomicAdd(st.ticket, 1u) == gridDim.x - 1 ? 1u : 0u;
+    }
+    __syncthreads();
+    if (s_last == 0) return;
+    __threadfence();
+    reduce_stats_cta(sstats, st.n_cols, st.out, st.out_host);
+    if (threadIdx.x == 0) *st.ticket = 0u;
 }
 
 }  // namespace psl
