@@ -206,7 +206,7 @@ enum ResultKind { RES_NONE = 0, RES_OTF = 1, RES_INDEX = 2, RES_BEAM = 3 };
 // ---- kernel variants: the features a configuration / beam does not use are compiled out ------------------
 using CountFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, uint32_t, uint32_t*, uint32_t, SegStats*, uint32_t, uint8_t*);
 using ScatterOtfFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, const uint32_t*, uint32_t, SoAOut, SegStats*,
-                              const uint8_t*);
+                              const uint8_t*, FusedScan, StatsTail);
 using ScatterBigFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, const uint32_t*, uint32_t, SoAOut, SegStats*, FusedScan, StatsTail);
 using ScatterIdxAFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, uint32_t, const uint32_t*, uint32_t, uint4*);
 
@@ -560,11 +560,11 @@ psl_status build_onthefly(psl_ctx* ctx, const DevBeam& bm)
                                                                                              table, d.cols_cap, ss, ctx->count_stages, codes);
             LAUNCHED();
         }
-        // 4096-record tiles: the table is small and stays raw -- the scatter CTAs scan it themselves (fused_first_slots)
+        // few keys: the table is small and stays raw -- the scatter CTAs scan it themselves (fused_first_slots)
         FusedScan fs;
         memset(&fs, 0, sizeof fs);
         memset(&tail, 0, sizeof tail);
-        if (big) {
+        if (ctx->big_tiles) {  // K <= 256, either tile size
             // ... and the last of them to finish reduces the statistics; both results go straight to the mapped
             // pinned copies the host reads (no reduce launch, no device-to-host copies behind the scatter)
             tail.n_cols = n_cols; tail.ticket = scalar(ctx, SC_TICKET); tail.out = stats; tail.out_host = ctx->d_h_stats;
@@ -592,7 +592,7 @@ psl_status build_onthefly(psl_ctx* ctx, const DevBeam& bm)
             else
                 scatter_otf_fn(pos, edges, bv, proj)<<<S, kThreads, ctx->sm_scatter_small, ctx->stream>>>(chunks, ctx->n_chunks, span, ctx->grid, bm,
                                                                                                        d.K, table, d.cols_cap, soa_out(ctx, L.out), ss,
-                                                                                                       codes);
+                                                                                                       codes, fs, tail);
             LAUNCHED();
         }
         if (tail.n_cols == 0) {

@@ -618,6 +618,77 @@ __global__ void k_offsets_from_table(const uint32_t* __restrict__ table, uint32_
     if (k % n_pos == 0 && k / n_pos <= n_batches) batch_offsets[k / n_pos] = o;
 }
 
+// fixed-order reduction of the per-segment statistics into one record (single CTA)
+struct DevStats {
+    unsigned long long n_invalid, n_outside, n_jaw, n_zero, n_surv;
+    double sum_in, sum_idx, sum_out;
+};
+
+// the reduction proper, by one CTA of any size; out_host (may be null) is the mapped pinned copy the host reads
+__device__ __forceinline__ void reduce_stats_cta(const SegStats* ts, uint32_t n_cols, DevStats* out, DevStats* out_host)
+{
+    __shared__ unsigned long long s_n[32][5];
+    __shared__ double s_d[32][3];
+    unsigned long long n[5] = {0, 0, 0, 0, 0};
+    double d[3] = {0.0, 0.0, 0.0};
+    for (uint32_t t = threadIdx.x; t < n_cols; t += blockDim.x) {
+        // L2 loads: the records may have been written by other CTAs of the running kernel (stats_tail)
+        const uint4* p = reinterpret_cast<const uint4*>(ts + t);
+        const uint4 a = __ldcg(p), b = __ldcg(p + 1), c = __ldcg(p + 2);
+        n[0] += a.x; n[1] += a.y; n[2] += a.z; n[3] += a.w; n[4] += b.x;
+        d[0] += __hiloint2double((int)b.w, (int)b.z);
+        d[1] += __hiloint2double((int)c.y, (int)c.x);
+        d[2] += __hiloint2double((int)c.w, (int)c.z);
+    }
+    for (int k = 0; k < 5; ++k)
+        for (int o = 16; o > 0; o >>= 1) n[k] += __shfl_xor_sync(0xFFFFFFFFu, n[k], o);
+    for (int k = 0; k < 3; ++k) d[k] = warp_sum_double(d[k]);
+    if (lane_id() == 0) {
+        for (int k = 0; k < 5; ++k) s_n[warp_id()][k] = n[k];
+        for (int k = 0; k < 3; ++k) s_d[warp_id()][k] = d[k];
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        DevStats r = {0, 0, 0, 0, 0, 0.0, 0.0, 0.0};
+        for (uint32_t w = 0; w < blockDim.x / 32; ++w) {
+            r.n_invalid += s_n[w][0]; r.n_outside += s_n[w][1]; r.n_jaw += s_n[w][2]; r.n_zero += s_n[w][3];
+            r.n_surv += s_n[w][4];
+            r.sum_in += s_d[w][0]; r.sum_idx += s_d[w][1]; r.sum_out += s_d[w][2];
+        }
+        *out = r;
+        if (out_host != nullptr) *out_host = r;
+    }
+}
+
+__global__ void __launch_bounds__(1024) k_reduce_stats(const SegStats* __restrict__ ts, uint32_t n_cols,
+                                                       DevStats* __restrict__ out)
+{
+    reduce_stats_cta(ts, n_cols, out, nullptr);
+}
+
+// The same reduction as the tail of a scatter kernel: each CTA, having written its SegStats, takes a ticket; the
+// last one reduces all n_cols records in the same fixed order and leaves the ticket at zero for the next launch.
+struct StatsTail {
+    uint32_t n_cols;  // 0: off (k_reduce_stats follows)
+    uint32_t* ticket;
+    DevStats *out, *out_host;
+};
+
+__device__ __forceinline__ void stats_tail(const StatsTail& st, const SegStats* sstats)
+{
+    if (st.n_cols == 0) return;
+    __shared__ uint32_t s_last;
+    if (threadIdx.x == 0) {
+        __threadfence();  // this CTA's SegStats before its ticket
+        s_last = atomicAdd(st.ticket, 1u) == gridDim.x - 1 ? 1u : 0u;
+    }
+    __syncthreads();
+    if (s_last == 0) return;
+    __threadfence();
+    reduce_stats_cta(sstats, st.n_cols, st.out, st.out_host);
+    if (threadIdx.x == 0) *st.ticket = 0u;
+}
+
 // prologue shared by the scatter kernels: barriers, first STAGES copies, zeroed counters, running slots
 template <int STAGES, typename DescFn>
 __device__ __forceinline__ void scatter_prologue(uint8_t* smem, const PartSmem& L, uint32_t B, uint32_t Bp, uint32_t n,
@@ -656,8 +727,9 @@ __global__ void __launch_bounds__(kThreads, 2) k_scatter_otf(const ChunkDesc* __
                                                             Span sp, const __grid_constant__ DevGrid g,
                                                             const __grid_constant__ DevBeam bm, uint32_t B,
                                                             const uint32_t* __restrict__ table, uint32_t stride,
-                                                            SoAOut out, SegStats* __restrict__ sstats,
-                                                            const uint8_t* __restrict__ codes)
+                                                            SoAOut out, SegStats* sstats,
+                                                            const uint8_t* __restrict__ codes, const FusedScan fs,
+                                                            const StatsTail st)
 {
     extern __shared__ __align__(128) uint8_t smem[];
     const uint32_t Bp = round_up(B, 8);
@@ -680,6 +752,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_scatter_otf(const ChunkDesc* __
     uint32_t grun[8];
     auto desc_of = [&](uint32_t t) { return raw_tile(chunks, n_chunks, t); };
     scatter_prologue<kStagesRaw>(smem, L, B, Bp, n, t0, kRecBytes, desc_of, table, stride, col, grun);
+    if (fs.n_cols != 0) fused_first_slots<kWarps>(fs, table, stride, B, col, gcur, lstart, misc, grun);  // raw table
     stage_edges(g, s_edges);
     __syncthreads();
 
@@ -800,6 +873,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_scatter_otf(const ChunkDesc* __
         for (int k = 0; k < kWarps; ++k) t += s_d[k];
         sstats[col].sum_out = t;
     }
+    stats_tail(st, sstats);
 }
 
 // tiles of the pass-A output: n keyed records (32 bytes each), contiguous
@@ -834,77 +908,6 @@ __global__ void k_counts_from_offsets(const uint32_t* __restrict__ offsets, uint
     uint32_t o = offsets[k];
     if (k < K) counts[k] = offsets[k + 1] - o;
     if (k % n_pos == 0 && k / n_pos <= n_batches) batch_offsets[k / n_pos] = o;
-}
-
-// fixed-order reduction of the per-segment statistics into one record (single CTA)
-struct DevStats {
-    unsigned long long n_invalid, n_outside, n_jaw, n_zero, n_surv;
-    double sum_in, sum_idx, sum_out;
-};
-
-// the reduction proper, by one CTA of any size; out_host (may be null) is the mapped pinned copy the host reads
-__device__ __forceinline__ void reduce_stats_cta(const SegStats* ts, uint32_t n_cols, DevStats* out, DevStats* out_host)
-{
-    __shared__ unsigned long long s_n[32][5];
-    __shared__ double s_d[32][3];
-    unsigned long long n[5] = {0, 0, 0, 0, 0};
-    double d[3] = {0.0, 0.0, 0.0};
-    for (uint32_t t = threadIdx.x; t < n_cols; t += blockDim.x) {
-        // L2 loads: the records may have been written by other CTAs of the running kernel (stats_tail)
-        const uint4* p = reinterpret_cast<const uint4*>(ts + t);
-        const uint4 a = __ldcg(p), b = __ldcg(p + 1), c = __ldcg(p + 2);
-        n[0] += a.x; n[1] += a.y; n[2] += a.z; n[3] += a.w; n[4] += b.x;
-        d[0] += __hiloint2double((int)b.w, (int)b.z);
-        d[1] += __hiloint2double((int)c.y, (int)c.x);
-        d[2] += __hiloint2double((int)c.w, (int)c.z);
-    }
-    for (int k = 0; k < 5; ++k)
-        for (int o = 16; o > 0; o >>= 1) n[k] += __shfl_xor_sync(0xFFFFFFFFu, n[k], o);
-    for (int k = 0; k < 3; ++k) d[k] = warp_sum_double(d[k]);
-    if (lane_id() == 0) {
-        for (int k = 0; k < 5; ++k) s_n[warp_id()][k] = n[k];
-        for (int k = 0; k < 3; ++k) s_d[warp_id()][k] = d[k];
-    }
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        DevStats r = {0, 0, 0, 0, 0, 0.0, 0.0, 0.0};
-        for (uint32_t w = 0; w < blockDim.x / 32; ++w) {
-            r.n_invalid += s_n[w][0]; r.n_outside += s_n[w][1]; r.n_jaw += s_n[w][2]; r.n_zero += s_n[w][3];
-            r.n_surv += s_n[w][4];
-            r.sum_in += s_d[w][0]; r.sum_idx += s_d[w][1]; r.sum_out += s_d[w][2];
-        }
-        *out = r;
-        if (out_host != nullptr) *out_host = r;
-    }
-}
-
-__global__ void __launch_bounds__(1024) k_reduce_stats(const SegStats* __restrict__ ts, uint32_t n_cols,
-                                                       DevStats* __restrict__ out)
-{
-    reduce_stats_cta(ts, n_cols, out, nullptr);
-}
-
-// The same reduction as the tail of a scatter kernel: each CTA, having written its SegStats, takes a ticket; the
-// last one reduces all n_cols records in the same fixed order and leaves the ticket at zero for the next launch.
-struct StatsTail {
-    uint32_t n_cols;  // 0: off (k_reduce_stats follows)
-    uint32_t* ticket;
-    DevStats *out, *out_host;
-};
-
-__device__ __forceinline__ void stats_tail(const StatsTail& st, const SegStats* sstats)
-{
-    if (st.n_cols == 0) return;
-    __shared__ uint32_t s_last;
-    if (threadIdx.x == 0) {
-        __threadfence();  // this CTA's SegStats before its ticket
-        s_last = atomicAdd(st.ticket, 1u) == gridDim.x - 1 ? 1u : 0u;
-    }
-    __syncthreads();
-    if (s_last == 0) return;
-    __threadfence();
-    reduce_stats_cta(sstats, st.n_cols, st.out, st.out_host);
-    if (threadIdx.x == 0) *st.ticket = 0u;
 }
 
 }  // namespace psl
