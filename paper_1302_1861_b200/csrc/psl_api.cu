@@ -11,6 +11,7 @@
 #include <string.h>
 
 #include <new>
+#include <utility>
 #include <vector>
 
 #include "psl_beam.cuh"
@@ -379,6 +380,25 @@ struct Prof {
     }
 };
 
+// launch with programmatic stream serialisation (psl_device.cuh, griddep_wait): the kernel may start while its
+// predecessor in the stream drains.  Off while kernels are bracketed by events.
+template <typename... Params, typename... Args>
+cudaError_t launch_after(bool overlap, void (*fn)(Params...), uint32_t grid, uint32_t block, uint32_t smem, cudaStream_t st,
+                         Args&&... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(block);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = overlap ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, fn, std::forward<Args>(args)...);
+}
+
 template <typename T>
 T* at(psl_ctx* ctx, uint64_t off) { return reinterpret_cast<T*>(ctx->ws + off); }
 
@@ -586,13 +606,16 @@ psl_status build_onthefly(psl_ctx* ctx, const DevBeam& bm)
         }
         {
             Prof prof(ctx, PSL_K_SCATTER);
+            // directly behind the histogram kernel (fused scan, no event bracket): programmatic dependent launch
+            const bool overlap = fs.n_cols != 0 && !ctx->profiling;
+            const uint32_t* ctable = table;
+            const uint8_t* ccodes = codes;
             if (big)
-                scatter_big_fn(pos, edges, bv, proj)<<<S, kBigThreads, ctx->sm_scatter_otf, ctx->stream>>>(chunks, ctx->n_chunks, span, ctx->grid, bm,
-                                                                                                          d.K, table, d.cols_cap, soa_out(ctx, L.out), ss, fs, tail);
+                CU(launch_after(overlap, scatter_big_fn(pos, edges, bv, proj), S, kBigThreads, ctx->sm_scatter_otf, ctx->stream, (const ChunkDesc*)chunks,
+                                ctx->n_chunks, span, ctx->grid, bm, d.K, ctable, d.cols_cap, soa_out(ctx, L.out), ss, fs, tail));
             else
-                scatter_otf_fn(pos, edges, bv, proj)<<<S, kThreads, ctx->sm_scatter_small, ctx->stream>>>(chunks, ctx->n_chunks, span, ctx->grid, bm,
-                                                                                                       d.K, table, d.cols_cap, soa_out(ctx, L.out), ss,
-                                                                                                       codes, fs, tail);
+                CU(launch_after(overlap, scatter_otf_fn(pos, edges, bv, proj), S, kThreads, ctx->sm_scatter_small, ctx->stream, (const ChunkDesc*)chunks,
+                                ctx->n_chunks, span, ctx->grid, bm, d.K, ctable, d.cols_cap, soa_out(ctx, L.out), ss, ccodes, fs, tail));
             LAUNCHED();
         }
         if (tail.n_cols == 0) {

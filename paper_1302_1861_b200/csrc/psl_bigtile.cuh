@@ -96,6 +96,7 @@ __global__ void __launch_bounds__(kBigThreads, 1) k_scatter_otf_big(const ChunkD
         for (uint32_t i = threadIdx.x; i < kBigWarps * Bp / 2; i += kBigThreads) cz[i] = 0;
     }
     uint32_t grun[8];
+    griddep_wait();  // the histogram kernel's table and statistics from here on
     if (fs.n_cols != 0) {
         fused_first_slots<kBigWarps>(fs, table, stride, B, col, gcur, lstart, misc, grun);
     } else {

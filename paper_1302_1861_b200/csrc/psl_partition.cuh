@@ -304,6 +304,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_count_raw(const ChunkDesc* __re
     split_segment_of(sp, t0, t1);
     const uint32_t n = t1 - t0;
 
+    griddep_launch();  // the scatter behind this kernel may set up and prefetch on SMs this grid has left
     if (threadIdx.x == 0) {
         for (uint32_t k = 0; k < n_stages; ++k) mbar_init(&bars[k], 1);
         mbar_fence_init();
@@ -709,6 +710,7 @@ __device__ __forceinline__ void scatter_prologue(uint8_t* smem, const PartSmem& 
     }
     uint32_t* cz = reinterpret_cast<uint32_t*>(smem + L.cnt);
     for (uint32_t i = threadIdx.x; i < kWarps * Bp / 2; i += kThreads) cz[i] = 0;
+    griddep_wait();  // the histogram kernel's table (and code bytes, statistics) from here on
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
         uint32_t b = threadIdx.x * 8 + k;
