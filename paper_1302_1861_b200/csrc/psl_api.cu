@@ -576,8 +576,8 @@ psl_status build_onthefly(psl_ctx* ctx, const DevBeam& bm)
         uint8_t* codes = (!big && bv != 0 && d.K <= 254) ? at<uint8_t>(ctx, L.codes) : nullptr;
         {
             Prof prof(ctx, PSL_K_COUNT);
-            count_otf_fn(pos, edges, bv)<<<n_cols, kThreads, ctx->sm_count_raw, ctx->stream>>>(chunks, ctx->n_chunks, span, ctx->grid, bm, d.K, 0,
-                                                                                             table, d.cols_cap, ss, ctx->count_stages, codes);
+            CU(launch_after(!ctx->profiling, count_otf_fn(pos, edges, bv), n_cols, kThreads, ctx->sm_count_raw, ctx->stream, (const ChunkDesc*)chunks,
+                            ctx->n_chunks, span, ctx->grid, bm, d.K, 0u, table, d.cols_cap, ss, ctx->count_stages, codes));
             LAUNCHED();
         }
         // few keys: the table is small and stays raw -- the scatter CTAs scan it themselves (fused_first_slots)

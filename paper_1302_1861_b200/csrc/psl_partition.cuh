@@ -115,6 +115,7 @@ struct ChunkBatch {
 };
 __global__ void k_set_chunks(ChunkDesc* __restrict__ dst, const __grid_constant__ ChunkBatch b, uint32_t n)
 {
+    griddep_launch();
     if (threadIdx.x < n) dst[threadIdx.x] = b.d[threadIdx.x];
 }
 
@@ -305,6 +306,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_count_raw(const ChunkDesc* __re
     const uint32_t n = t1 - t0;
 
     griddep_launch();  // the scatter behind this kernel may set up and prefetch on SMs this grid has left
+    griddep_wait();    // the chunk table (k_set_chunks) when this kernel was itself launched as a dependent
     if (threadIdx.x == 0) {
         for (uint32_t k = 0; k < n_stages; ++k) mbar_init(&bars[k], 1);
         mbar_fence_init();
