@@ -7,6 +7,7 @@
 
 #include <math.h>
 #include <stdarg.h>
+#include <stdlib.h>
 #include <stdio.h>
 #include <string.h>
 
@@ -15,6 +16,7 @@
 #include <vector>
 
 #include "psl_beam.cuh"
+#include "psl_compact.cuh"
 #include "psl_bigtile.cuh"
 #include "psl_index.cuh"
 #include "psl_index_big.cuh"
@@ -36,7 +38,7 @@ struct Layout {
     uint64_t total = 0;
     uint64_t raw = 0, chunks = 0, spans = 0, sstats = 0, scan_sums = 0, scalars = 0, edges = 0, stats = 0, batch_off = 0;
     // ONTHEFLY
-    uint64_t table = 0, out[10] = {0}, offsets = 0, counts = 0, codes = 0;
+    uint64_t table = 0, out[10] = {0}, offsets = 0, counts = 0, codes = 0, comp = 0;
     // INDEX
     uint64_t table_a = 0, table_b = 0, aos = 0, aos_index = 0, idx[7] = {0}, idx_offsets = 0, idx_counts = 0,
              idx_batch_off = 0;
@@ -176,6 +178,9 @@ void plan(const psl_config* c, const Derived& d, Layout* L)
         L->offsets = take(&cur, (uint64_t)(d.K + 1) * 4);
         L->counts = take(&cur, (uint64_t)d.K * 4);
         L->codes = take(&cur, N);  // one byte per record: the histogram kernel's verdict for the scatter of a rejecting beam
+        // few keys: the survivors of a rejecting beam, compacted per histogram segment (32 B each, a segment's region
+        // starts at its first record, so only the survivors' share of it is ever touched)
+        if (round_up(d.K, 8) <= (uint32_t)kBigMaxKeys) L->comp = take(&cur, (uint64_t)d.tiles_cap * kTile * kCompBytes);
     } else {
         L->table_a = take(&cur, (uint64_t)d.B_lo * d.cols_cap * 4);
         L->table_b = take(&cur, (uint64_t)d.B_hi * kMaxSegments * 4);
@@ -205,7 +210,8 @@ void plan(const psl_config* c, const Derived& d, Layout* L)
 enum ResultKind { RES_NONE = 0, RES_OTF = 1, RES_INDEX = 2, RES_BEAM = 3 };
 
 // ---- kernel variants: the features a configuration / beam does not use are compiled out ------------------
-using CountFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, uint32_t, uint32_t*, uint32_t, SegStats*, uint32_t, uint8_t*);
+using CountFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, uint32_t, uint32_t*, uint32_t, SegStats*, uint32_t, uint8_t*, uint4*);
+using ScatterCompFn = void (*)(const uint4*, Span, DevBeam, uint32_t, const uint32_t*, uint32_t, SoAOut, SegStats*, FusedScan, StatsTail);
 using ScatterOtfFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, const uint32_t*, uint32_t, SoAOut, SegStats*,
                               const uint8_t*, FusedScan, StatsTail);
 using ScatterBigFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, const uint32_t*, uint32_t, SoAOut, SegStats*, FusedScan, StatsTail);
@@ -296,8 +302,9 @@ struct psl_ctx {
     uint32_t* h_scalars = nullptr;
     bool seg_pending = false;
     // launch shapes: persistent CTAs per launch (= SMs x resident CTAs of the scatter kernel, one wave)
-    uint32_t S_otf = 0, S_otf_small = 0, S_a = 0, S_b = 0;
-    uint32_t sm_scatter_small = 0;
+    uint32_t S_otf = 0, S_otf_small = 0, S_a = 0, S_b = 0, S_comp = 0;
+    uint32_t sm_scatter_small = 0, sm_scatter_comp = 0;
+    bool compact = false;  // ONTHEFLY with few keys, rejecting beam: the histogram kernel compacts the survivors
     bool big_tiles = false;  // ONTHEFLY with few keys: the 4096-record-tile scatter
     uint32_t count_stages = kStagesCount, count_split = 1;
     uint32_t sm_count_raw = 0, sm_scatter_otf = 0, sm_idx_a = 0, sm_count_b = 0, sm_idx_b = 0;  // dynamic smem bytes
@@ -567,17 +574,20 @@ psl_status build_onthefly(psl_ctx* ctx, const DevBeam& bm)
         // 4096-record tiles pay when most records are written out (long runs per key); when jaws reject most of
         // them the kernel is a read stream and two 1024-record-tile CTAs per SM overlap better
         const bool big = ctx->big_tiles && bv == 0;
-        const uint32_t S_max = big ? ctx->S_otf : ctx->S_otf_small, split = big ? ctx->count_split : 1u;
+        // ... unless the histogram kernel compacts the survivors: then the scatter reads only those, in 4096-survivor tiles
+        const bool compact = ctx->compact && bv != 0;
+        const uint32_t S_max = big ? ctx->S_otf : (compact ? ctx->S_comp : ctx->S_otf_small), split = (big || compact) ? ctx->count_split : 1u;
         const uint32_t S = nt < S_max ? nt : S_max;  // one persistent CTA per segment, one wave
         const Span span = {0u, nt, 0u, split};
         const uint32_t n_cols = S * split;
         // a beam that rejects (jaws, zero-weight policy): the histogram kernel leaves one byte per record (key or
         // 255 = dropped) and the scatter ranks from those instead of repeating the projection arithmetic
-        uint8_t* codes = (!big && bv != 0 && d.K <= 254) ? at<uint8_t>(ctx, L.codes) : nullptr;
+        uint8_t* codes = (!big && !compact && bv != 0 && d.K <= 254) ? at<uint8_t>(ctx, L.codes) : nullptr;
+        uint4* comp = compact ? at<uint4>(ctx, L.comp) : nullptr;
         {
             Prof prof(ctx, PSL_K_COUNT);
             CU(launch_after(!ctx->profiling, count_otf_fn(pos, edges, bv), n_cols, kThreads, ctx->sm_count_raw, ctx->stream, (const ChunkDesc*)chunks,
-                            ctx->n_chunks, span, ctx->grid, bm, d.K, 0u, table, d.cols_cap, ss, ctx->count_stages, codes));
+                            ctx->n_chunks, span, ctx->grid, bm, d.K, 0u, table, d.cols_cap, ss, ctx->count_stages, codes, comp));
             LAUNCHED();
         }
         // few keys: the table is small and stays raw -- the scatter CTAs scan it themselves (fused_first_slots)
@@ -610,7 +620,10 @@ psl_status build_onthefly(psl_ctx* ctx, const DevBeam& bm)
             const bool overlap = fs.n_cols != 0 && !ctx->profiling;
             const uint32_t* ctable = table;
             const uint8_t* ccodes = codes;
-            if (big)
+            if (compact)
+                CU(launch_after(overlap, proj ? (ScatterCompFn)k_scatter_comp_big<true> : (ScatterCompFn)k_scatter_comp_big<false>, S, kBigThreads,
+                                ctx->sm_scatter_comp, ctx->stream, (const uint4*)comp, span, bm, d.K, ctable, d.cols_cap, soa_out(ctx, L.out), ss, fs, tail));
+            else if (big)
                 CU(launch_after(overlap, scatter_big_fn(pos, edges, bv, proj), S, kBigThreads, ctx->sm_scatter_otf, ctx->stream, (const ChunkDesc*)chunks,
                                 ctx->n_chunks, span, ctx->grid, bm, d.K, ctable, d.cols_cap, soa_out(ctx, L.out), ss, fs, tail));
             else
@@ -1003,6 +1016,17 @@ psl_status psl_create(const psl_config* cfg, psl_ctx** out)
             ctx->S_otf = width(occ);
         }
         ctx->count_split = ctx->big_tiles ? 2 : 1;  // one scatter CTA per SM, two histogram CTAs
+        if (ctx->big_tiles && ctx->L.comp != 0 && getenv("PSL_NO_COMPACT") == nullptr) {
+            int max_smem = 0;
+            CUC(cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, cfg->device));
+            ctx->sm_scatter_comp = comp_layout(d.K).total;
+            if (ctx->sm_scatter_comp + 3072 <= (uint32_t)max_smem) {  // + the kernel's static shared memory
+                CUC(allow_smem(k_scatter_comp_big<true>, ctx->sm_scatter_comp));
+                CUC(allow_smem(k_scatter_comp_big<false>, ctx->sm_scatter_comp));
+                ctx->S_comp = width(1);
+                ctx->compact = true;
+            }
+        }
     } else {
         ctx->count_stages = d.B_lo * 4 > 8192 ? 2 : kStagesCount;
         ctx->sm_count_raw = count_layout(kTile * kRecBytes, ctx->count_stages, d.B_lo, ne).total;
@@ -1131,7 +1155,7 @@ psl_status psl_load_chunk(psl_ctx* ctx, const void* records, uint64_t n, int32_t
         Prof prof(ctx, PSL_K_COUNT);
         count_idx_fn(ctx->grid.has_pos != 0, ctx->grid.ebin_mode != 0)<<<cl.n_seg * ctx->split_a, kThreads, ctx->sm_count_raw, ctx->stream>>>(
             chunks, ctx->n_chunks + 1, cl.span, ctx->grid, none, ctx->d.B_lo, (1u << ctx->d.lo_bits) - 1u,
-            at<uint32_t>(ctx, ctx->L.table_a), ctx->d.cols_cap, at<SegStats>(ctx, ctx->L.sstats), ctx->count_stages, nullptr);
+            at<uint32_t>(ctx, ctx->L.table_a), ctx->d.cols_cap, at<SegStats>(ctx, ctx->L.sstats), ctx->count_stages, nullptr, nullptr);
         LAUNCHED();
         ctx->idx_launches.push_back(cl);
         ctx->n_cols += cl.n_seg * ctx->split_a;

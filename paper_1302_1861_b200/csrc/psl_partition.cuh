@@ -291,9 +291,11 @@ __global__ void __launch_bounds__(kThreads, 2) k_count_raw(const ChunkDesc* __re
                                                           const __grid_constant__ DevBeam bm, uint32_t B,
                                                           uint32_t lo_mask, uint32_t* __restrict__ table,
                                                           uint32_t stride, SegStats* __restrict__ sstats,
-                                                          uint32_t n_stages, uint8_t* __restrict__ codes)
+                                                          uint32_t n_stages, uint8_t* __restrict__ codes,
+                                                          uint4* __restrict__ comp)
 {
     extern __shared__ __align__(128) uint8_t smem[];
+    __shared__ uint32_t s_comp[2][kRounds * kWarps];  // survivors per (round, warp) of the tile, by tile parity
     const CountSmem L = count_layout(kTile * kRecBytes, n_stages, B, g.n_ebins + 1);
     uint32_t* hist = reinterpret_cast<uint32_t*>(smem + L.hist);
     float* s_edges = reinterpret_cast<float*>(smem + L.edges);
@@ -322,6 +324,11 @@ __global__ void __launch_bounds__(kThreads, 2) k_count_raw(const ChunkDesc* __re
 
     ThreadStats st;
     uint32_t phase_bits = 0;
+    // survivors of a rejecting beam, compacted in load order into the segment's own region of `comp` (32-byte
+    // records {key, E, x, y, u, v, wt, src_index}, region = the segment's first record): what the scatter reads
+    const bool compact = !IDX && BEAM != 0 && comp != nullptr;
+    uint32_t comp_next = t0 * (uint32_t)kTile;
+    static_assert(kRounds * kWarps == 32, "one warp scan over the (round, warp) survivor counts");
     for (uint32_t i = 0; i < n; ++i) {
         const uint32_t stage = i % n_stages;
         uint32_t* raw = reinterpret_cast<uint32_t*>(smem + L.ring + stage * L.stage_bytes);
@@ -330,6 +337,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_count_raw(const ChunkDesc* __re
         // all of the thread's records first, then straight-line classification: independent chains interleave
         Rec rec[kRounds];
         bool have[kRounds];
+        uint32_t skey[kRounds];  // compact: the key of a survivor, kNone otherwise
 #pragma unroll
         for (int r = 0; r < kRounds; ++r) {
             const int idx = r * kThreads + threadIdx.x;
@@ -347,15 +355,42 @@ __global__ void __launch_bounds__(kThreads, 2) k_count_raw(const ChunkDesc* __re
             if (POS) st.n_out += have[r] & (cls == C_OUTSIDE);
             if (BEAM != 0) st.n_jaw += have[r] & (cls == C_JAW);
             if (BEAM == 2) st.n_zero += have[r] & (cls == C_ZERO);
+            skey[r] = kNone;
             if (have[r] & (cls == C_SURVIVOR)) {
                 st.n_surv += 1;
                 const uint32_t bucket = IDX ? (key & lo_mask) : key;
                 atomicAdd(&hist[(bucket << L.rlog) + (lane_id() & rmask)], 1u);
+                skey[r] = key;
             }
             // one byte per record for the scatter of a rejecting beam: its key (< 255) or 255 = dropped, so that the
             // jaw / zero-weight arithmetic is not repeated there
             if (!IDX && codes != nullptr && have[r])
                 codes[td.first_index + r * kThreads + threadIdx.x] = (uint8_t)(cls == C_SURVIVOR ? key : 255u);
+        }
+        if (!IDX && BEAM != 0) {
+            if (compact) {  // stable: tile order is (round, warp, lane)
+                uint32_t bal[kRounds];
+                uint32_t* sc = s_comp[i & 1u];
+#pragma unroll
+                for (int r = 0; r < kRounds; ++r) {
+                    bal[r] = __ballot_sync(0xFFFFFFFFu, skey[r] != kNone);
+                    if (lane_id() == 0) sc[r * kWarps + warp_id()] = __popc(bal[r]);
+                }
+                __syncthreads();
+                const uint32_t mine = sc[lane_id()];
+                const uint32_t inc = warp_incl_scan(mine);
+#pragma unroll
+                for (int r = 0; r < kRounds; ++r) {
+                    const uint32_t ex = __shfl_sync(0xFFFFFFFFu, inc - mine, r * kWarps + (int)warp_id());
+                    if (skey[r] != kNone) {
+                        uint4* dst = comp + (size_t)(comp_next + ex + __popc(bal[r] & lanemask_lt())) * 2;
+                        dst[0] = make_uint4(skey[r], __float_as_uint(rec[r].E), __float_as_uint(rec[r].x), __float_as_uint(rec[r].y));
+                        dst[1] = make_uint4(__float_as_uint(rec[r].u), __float_as_uint(rec[r].v), __float_as_uint(rec[r].wt),
+                                            td.first_index + r * kThreads + threadIdx.x);
+                    }
+                }
+                comp_next += __shfl_sync(0xFFFFFFFFu, inc, 31);
+            }
         }
         __syncthreads();  // every thread is done with the stage
         if (threadIdx.x == 0 && i + n_stages < n) {
