@@ -206,14 +206,16 @@ def run_reference(args):
 # ------------------------------------------------------------------------------------------------------
 # the CUDA arm
 # ------------------------------------------------------------------------------------------------------
-def algorithmic_bytes(cls, n, n_idx, m_sel, n_surv_beams, proj, index_mode=False):
+def algorithmic_bytes(cls, n, n_idx, m_sel, n_surv_beams, proj, index_mode=False, compacted=False):
     """algorithmic bytes one step's launches of kernel class `cls` must move"""
     out_b = SOA_BYTES + (8 if proj else 0)
     if cls == "count":
         # one read of every packed record; INDEX mode adds pass B's histogram, which reads the 4-byte key of every
-        # keyed record
-        return RECORD_BYTES * n + (4 * n_idx if index_mode else 0)
+        # keyed record; for a rejecting beam with few keys it also writes the survivors as 32-byte keyed records
+        return RECORD_BYTES * n + (4 * n_idx if index_mode else 0) + (32 * n_surv_beams if compacted else 0)
     if cls == "scatter":
+        if compacted:
+            return 32 * n_surv_beams + out_b * n_surv_beams  # read the compacted survivors, write their SoA
         return RECORD_BYTES * n + out_b * n_surv_beams  # read every record, write the survivors' SoA
     if cls == "index_a":
         return RECORD_BYTES * n + 32 * n_idx          # packed records in, 32-byte keyed records out
@@ -363,13 +365,16 @@ def run_ours(args):
     # ---- roofline of the dominant kernel -------------------------------------------------------------------
     peak, peak_src = measured_peaks()
     proj = bool(w.flags & P.OUT_PROJ)
+    # ONTHEFLY, K <= 256, a beam that rejects: the histogram kernel compacts the survivors and the scatter reads those
+    compacted = (w.mode == 0 and (w.n_keys + 7) // 8 * 8 <= 256 and os.environ.get("PSL_NO_COMPACT") is None
+                 and any(b is not None and (b.get("jaws") is not None or (w.flags & P.DROP_ZERO_WEIGHT)) for b in w.beams))
     kernels = {}
     for cls, (tot_ms, brackets) in prof.items():
         if brackets == 0 or cls in ("scan", "other"):
             if brackets:
                 kernels[cls] = {"ms_per_step": tot_ms / args.steps, "launches_per_step": brackets / args.steps}
             continue
-        per_step_bytes = algorithmic_bytes(cls, n, n_idx, m_sel_all, surv_all, proj, w.mode == 1)
+        per_step_bytes = algorithmic_bytes(cls, n, n_idx, m_sel_all, surv_all, proj, w.mode == 1, compacted)
         kernels[cls] = {"ms_per_step": tot_ms / args.steps, "launches_per_step": brackets / args.steps,
                         "avg_launch_ms": tot_ms / brackets,
                         "algorithmic_bytes_per_step": per_step_bytes,

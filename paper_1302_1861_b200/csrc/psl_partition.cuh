@@ -295,7 +295,9 @@ __global__ void __launch_bounds__(kThreads, 2) k_count_raw(const ChunkDesc* __re
                                                           uint4* __restrict__ comp)
 {
     extern __shared__ __align__(128) uint8_t smem[];
-    __shared__ uint32_t s_comp[2][kRounds * kWarps];  // survivors per (round, warp) of the tile, by tile parity
+    __shared__ uint32_t s_comp[2][kWarps];  // (tile tag << 8 | survivors) per warp, by tile parity
+    // a warp takes 128 consecutive records of the tile, 32 per round
+    auto rec_idx = [](int r) { return warp_id() * (uint32_t)kWarpSpan + (uint32_t)r * 32u + lane_id(); };
     const CountSmem L = count_layout(kTile * kRecBytes, n_stages, B, g.n_ebins + 1);
     uint32_t* hist = reinterpret_cast<uint32_t*>(smem + L.hist);
     float* s_edges = reinterpret_cast<float*>(smem + L.edges);
@@ -319,6 +321,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_count_raw(const ChunkDesc* __re
         }
     }
     for (uint32_t i = threadIdx.x; i < (B << L.rlog); i += kThreads) hist[i] = 0;
+    if (threadIdx.x < 2 * kWarps) (&s_comp[0][0])[threadIdx.x] = 0u;  // tag 0 = no tile: shared memory keeps the last launch's words
     stage_edges(g, s_edges);
     __syncthreads();
 
@@ -328,7 +331,6 @@ __global__ void __launch_bounds__(kThreads, 2) k_count_raw(const ChunkDesc* __re
     // records {key, E, x, y, u, v, wt, src_index}, region = the segment's first record): what the scatter reads
     const bool compact = !IDX && BEAM != 0 && comp != nullptr;
     uint32_t comp_next = t0 * (uint32_t)kTile;
-    static_assert(kRounds * kWarps == 32, "one warp scan over the (round, warp) survivor counts");
     for (uint32_t i = 0; i < n; ++i) {
         const uint32_t stage = i % n_stages;
         uint32_t* raw = reinterpret_cast<uint32_t*>(smem + L.ring + stage * L.stage_bytes);
@@ -340,7 +342,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_count_raw(const ChunkDesc* __re
         uint32_t skey[kRounds];  // compact: the key of a survivor, kNone otherwise
 #pragma unroll
         for (int r = 0; r < kRounds; ++r) {
-            const int idx = r * kThreads + threadIdx.x;
+            const int idx = (int)rec_idx(r);
             have[r] = idx < (int)td.count;
             rec[r] = rec_from_smem(raw, have[r] ? idx : 0);
         }
@@ -365,31 +367,44 @@ __global__ void __launch_bounds__(kThreads, 2) k_count_raw(const ChunkDesc* __re
             // one byte per record for the scatter of a rejecting beam: its key (< 255) or 255 = dropped, so that the
             // jaw / zero-weight arithmetic is not repeated there
             if (!IDX && codes != nullptr && have[r])
-                codes[td.first_index + r * kThreads + threadIdx.x] = (uint8_t)(cls == C_SURVIVOR ? key : 255u);
+                codes[td.first_index + rec_idx(r)] = (uint8_t)(cls == C_SURVIVOR ? key : 255u);
         }
         if (!IDX && BEAM != 0) {
-            if (compact) {  // stable: tile order is (round, warp, lane)
-                uint32_t bal[kRounds];
-                uint32_t* sc = s_comp[i & 1u];
+            if (compact) {
+                // Stable: a warp's 128 records are consecutive, so its survivors follow those of the warps before it.
+                // No barrier: every warp publishes (tile tag, survivors) in one word and spins only on the warps before
+                // it; the tile's total is read one tile later from the other parity's slots, complete by then.
+                volatile uint32_t* slot = s_comp[i & 1u];
+                if (i != 0) {
+                    const uint32_t pv = lane_id() < (uint32_t)kWarps ? (s_comp[(i & 1u) ^ 1u][lane_id()] & 0xFFu) : 0u;
+                    comp_next += __reduce_add_sync(0xFFFFFFFFu, pv);
+                }
+                uint32_t bal[kRounds], wc = 0;
 #pragma unroll
                 for (int r = 0; r < kRounds; ++r) {
                     bal[r] = __ballot_sync(0xFFFFFFFFu, skey[r] != kNone);
-                    if (lane_id() == 0) sc[r * kWarps + warp_id()] = __popc(bal[r]);
+                    wc += __popc(bal[r]);
                 }
-                __syncthreads();
-                const uint32_t mine = sc[lane_id()];
-                const uint32_t inc = warp_incl_scan(mine);
+                if (lane_id() == 0) slot[warp_id()] = ((i + 1u) << 8) | wc;
+                uint32_t v = 0;
+                if (lane_id() < warp_id()) {
+                    do { v = slot[lane_id()]; } while ((v >> 8) != i + 1u);
+                    v &= 0xFFu;
+                }
+                // Survivors are stored one by one (two 16-byte stores each): the kernel is issue-bound with a jaw test
+                // (62-67 % issue utilisation), and staging them in shared memory for whole-line stores -- per tile or
+                // per warp -- cost more instructions than the stores saved (measured: 0.36 ms against 0.33 ms).
+                uint32_t ex = comp_next + __reduce_add_sync(0xFFFFFFFFu, v);
 #pragma unroll
                 for (int r = 0; r < kRounds; ++r) {
-                    const uint32_t ex = __shfl_sync(0xFFFFFFFFu, inc - mine, r * kWarps + (int)warp_id());
                     if (skey[r] != kNone) {
-                        uint4* dst = comp + (size_t)(comp_next + ex + __popc(bal[r] & lanemask_lt())) * 2;
+                        uint4* dst = comp + (size_t)(ex + __popc(bal[r] & lanemask_lt())) * 2;
                         dst[0] = make_uint4(skey[r], __float_as_uint(rec[r].E), __float_as_uint(rec[r].x), __float_as_uint(rec[r].y));
                         dst[1] = make_uint4(__float_as_uint(rec[r].u), __float_as_uint(rec[r].v), __float_as_uint(rec[r].wt),
-                                            td.first_index + r * kThreads + threadIdx.x);
+                                            td.first_index + rec_idx(r));
                     }
+                    ex += __popc(bal[r]);
                 }
-                comp_next += __shfl_sync(0xFFFFFFFFu, inc, 31);
             }
         }
         __syncthreads();  // every thread is done with the stage
