@@ -327,10 +327,48 @@ def test_big_tiles_ragged_chunks_and_ring_wraparound():
     check(w_small, dirty(w_small.records(), 8), None, chunk=3000, mem="device")
 
 
-def test_small_tiles_with_a_rejecting_beam_at_scale():
-    """a beam with jaws takes the 1024-record-tile scatter (two CTAs per SM); several tiles per CTA"""
+def test_small_tiles_with_a_rejecting_beam_at_scale(monkeypatch):
+    """a beam with jaws and the survivor compaction switched off takes the 1024-record-tile scatter (two CTAs per
+    SM), which ranks from the histogram kernel's one byte per record; several tiles per CTA"""
+    monkeypatch.setenv("PSL_NO_COMPACT", "1")
     w = W.config(3, 1_500_000)
     check(w, w.records(), w.beams[0], chunk=500_000, mem="device", flags=P().OUT_PROJ, proj=True)
+
+
+def test_compacted_survivors_at_scale_and_against_the_other_path(monkeypatch):
+    """a beam with jaws and K <= 256: the histogram kernel compacts the survivors per segment and the scatter reads
+    only those (psl_compact.cuh).  Against the oracle, and byte for byte against the path without compaction."""
+    w = W.config(3, 1_500_000)
+    r = dirty(w.records(), 11)
+    a = check(w, r, w.beams[0], chunk=500_000, mem="device", flags=P().OUT_PROJ, proj=True)
+    monkeypatch.setenv("PSL_NO_COMPACT", "1")
+    b = library_result(run_library(w, r, w.beams[0], chunk=500_000, mem="device", flags=P().OUT_PROJ))
+    for k in ("counts", "offsets", "src_index", "E", "x", "y", "u", "v", "w", "wt", "xp", "yp"):
+        assert np.array_equal(a[k].view(np.uint32), b[k].view(np.uint32)), k
+    assert a["stats"] == b["stats"]
+
+
+def test_compacted_survivors_when_every_record_survives():
+    """jaws wider than the whole phase-space: a rejecting beam that rejects nothing.  Every warp of the histogram
+    kernel compacts all 128 of its records, every region is full, and the scatter's 4096-survivor tiles straddle
+    the regions of the two histogram CTAs per segment; ragged chunks leave ragged tiles in between."""
+    w = W.config(2, 2_400_000)
+    r = w.records()
+    lib = check(w, r, W.make_beam(jaws=(-20, 20, -20, 20)), chunk=3000 * 40, mem="device")
+    assert lib["n_survivors"] == len(r)
+    w_small = W.config(2, 70_001)
+    check(w_small, dirty(w_small.records(), 9), W.make_beam(jaws=(-20, 20, -20, 20), mu_weight=0.25), chunk=3000, mem="device")
+
+
+def test_compacted_survivors_sparse_and_with_the_zero_weight_policy():
+    """few survivors (config 1: 0.25 %): most segments compact nothing and their scatter CTAs have no tile; and the
+    zero-weight policy, which rejects after the fluence lookup"""
+    w = W.config(1)
+    check(w, dirty(w.records(), 12), w.beams[0], chunk=10_000, mem="device")
+    w3 = W.config(3, 600_000)
+    m = W.fluence_uniform(6)
+    m[40:120, :] = 0.0
+    check(w3, w3.records(), W.make_beam(jaws=(-15, 15, -15, 15), fluence=m, mu_weight=0.5), chunk=0, mem="pinned", flags=2)
 
 
 def test_unaligned_device_source_takes_the_manual_stage_fill():
