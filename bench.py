@@ -170,6 +170,42 @@ def time_oracle(w, rank_first, budget_s=10.0, max_sample=20_000_000):
     return n * reps / t_total, sample
 
 
+def time_oracle_all_cores(w, rank_first, n_sample=8_000_000):
+    """SURVEY 8(d)'s second CPU line: C independent oracle instances on C contiguous shards of the sample, one per
+    host core, run at the same time (the oracle itself stays single-threaded; ctypes drops the GIL in the call)"""
+    import threading
+
+    import workloads as W
+    from oracle import psl_oracle as O
+
+    cores = os.cpu_count() or 1
+    n = min(w.n_records, max(n_sample, min(cores * 200_000, 32_000_000)))
+    rec = W.generate(w.gen, rank_first, n)
+    per = (n + cores - 1) // cores
+    shards = [rec[i * per:min(n, (i + 1) * per)] for i in range(cores) if i * per < n]
+    orcs = [O.Oracle(w.grid, w.geometry, flags=w.flags) for _ in shards]
+    def work(o, s_):
+        for _ in range(reps):
+            oracle_step(o, s_, w.beams)
+
+    reps, dt = 1, 0.0
+    while True:  # repeat with more repetitions per instance until the run lasts about two seconds
+        threads = [threading.Thread(target=work, args=(o, s_)) for o, s_ in zip(orcs, shards)]
+        t0 = time.perf_counter()
+        for t in threads:
+            t.start()
+        for t in threads:
+            t.join()
+        dt = time.perf_counter() - t0
+        if dt >= 2.0 or reps >= 256:
+            break
+        reps = min(256, max(reps * 2, int(reps * 2.5 / max(dt, 1e-3))))
+    n *= reps
+    return {"value": n / dt, "unit": UNIT, "cores": len(shards), "kind": "oracle",
+            "sample": "%d independent single-threaded oracle instances, one per shard of the first %d records of %s, "
+                      "%d repetition(s) each, %.1f s wall" % (len(shards), n // reps, w.name, reps, dt)}
+
+
 def run_reference(args):
     """--impl reference: the oracle on the host cores, on the same config / metric / unit"""
     rank = int(os.environ.get("RANK", "0"))
@@ -407,7 +443,8 @@ def run_ours(args):
         if world == 1 and not args.no_cpu_baseline:
             v, sample = time_oracle(w, first_record)
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
-                                    "host_cores_available": os.cpu_count()}
+                                    "host_cores_available": os.cpu_count(),
+                                    "all_cores": time_oracle_all_cores(w, first_record)}
         print(json.dumps(line))
     ctx.destroy()
     if world > 1:

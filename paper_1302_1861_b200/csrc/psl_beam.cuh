@@ -52,6 +52,15 @@ __device__ __forceinline__ uint32_t seg_of(const uint32_t* __restrict__ vstart, 
     return lo;
 }
 
+// one 32-byte keyed record in ONE request (LDG.E.256, sm_100+): the two 16-byte halves as separate loads make every
+// warp touch each sector twice
+__device__ __forceinline__ void ldg_record(const uint4* p, uint4& a, uint4& b)
+{
+    asm volatile("ld.global.nc.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=r"(a.x), "=r"(a.y), "=r"(a.z), "=r"(a.w), "=r"(b.x), "=r"(b.y), "=r"(b.z), "=r"(b.w)
+                 : "l"(p));
+}
+
 constexpr int kBeamTile = 2048;                       // index records one CTA of the beam kernel compacts
 constexpr int kBeamRounds = kBeamTile / kThreads;      // 8
 constexpr int kBeamArrays = 12;  // E x y u v w wt xp yp src key + spare
@@ -96,8 +105,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_beam_compact(SegTable seg, IdxI
             const uint32_t vv = v0 + lv;
             const uint32_t sg = s_first == s_last ? s_first : seg_of(seg.vstart, s_first, s_last, vv);
             const uint32_t p = __ldg(seg.src + sg) + (vv - __ldg(seg.vstart + sg));
-            ra[r] = __ldg(in.aos + 2 * (size_t)p);
-            rb[r] = __ldg(in.aos + 2 * (size_t)p + 1);
+            ldg_record(in.aos + 2 * (size_t)p, ra[r], rb[r]);
         }
     }
     float wz[kBeamRounds], wt[kBeamRounds], xm[kBeamRounds], ym[kBeamRounds];
