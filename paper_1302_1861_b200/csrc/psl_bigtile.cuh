@@ -81,8 +81,9 @@ __global__ void __launch_bounds__(kBigThreads, 1) k_scatter_otf_big(const ChunkD
     const uint32_t n = t1 - t0;  // ring stages (tiles of kTile records) in this segment
 
     auto stage_ptr = [&](uint32_t i) { return reinterpret_cast<uint32_t*>(smem + L.ring + (i % kBigStages) * L.stage_bytes); };
+    ChunkDesc ccur = {nullptr, 0u, 0u, 0u, 0u};  // thread 0: the chunk of the tile it described last
     auto issue = [&](uint32_t i) {  // thread 0
-        TileDesc d = raw_tile(chunks, n_chunks, t0 + i);
+        TileDesc d = raw_tile(chunks, n_chunks, t0 + i, ccur);
         s_desc[i % kBigStages] = d;
         ring_issue(stage_ptr(i), &bars[i % kBigStages], d.ptr, d.count * kRecBytes);
     };

@@ -71,11 +71,12 @@ __global__ void __launch_bounds__(kThreads, 3) k_scatter_idx_a(const ChunkDesc* 
     uint32_t t0, t1;
     segment_of(sp, t0, t1);
     const uint32_t n = t1 - t0;
+    ChunkDesc ccur = {nullptr, 0u, 0u, 0u, 0u};  // thread 0: the chunk of the tile it described last
     if (threadIdx.x == 0) {
         for (int k = 0; k < kStagesIdxA; ++k) mbar_init(&bars[k], 1);
         mbar_fence_init();
         for (uint32_t k = 0; k < (uint32_t)kStagesIdxA && k < n; ++k) {
-            TileDesc d = raw_tile(chunks, n_chunks, t0 + k);
+            TileDesc d = raw_tile(chunks, n_chunks, t0 + k, ccur);
             s_desc[k] = d;
             ring_issue_stream(reinterpret_cast<uint32_t*>(smem + L.ring + k * L.stage_bytes), &bars[k], d.ptr, d.count * kRecBytes);
         }
@@ -161,7 +162,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_scatter_idx_a(const ChunkDesc* 
         zero_row(cnt + w * Bp, Bp);
         __syncthreads();  // the stage, skey and sdest are free again
         if (threadIdx.x == 0 && i + kStagesIdxA < n) {
-            TileDesc d = raw_tile(chunks, n_chunks, t0 + i + kStagesIdxA);
+            TileDesc d = raw_tile(chunks, n_chunks, t0 + i + kStagesIdxA, ccur);
             s_desc[stage] = d;
             ring_issue_stream(raw, &bars[stage], d.ptr, d.count * kRecBytes);
         }

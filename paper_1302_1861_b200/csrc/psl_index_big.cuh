@@ -87,8 +87,9 @@ __global__ void __launch_bounds__(kIdxBigThreads, 1) k_scatter_idx_big(const Chu
     uint32_t goff = 0;  // ring stages this CTA has consumed in earlier spans (stage and parity bookkeeping runs on)
     uint32_t t0 = 0, n = 0;
     auto stage_ptr = [&](uint32_t i) { return reinterpret_cast<uint32_t*>(smem + L.ring + ((goff + i) % kIdxBigStages) * L.stage_bytes); };
+    ChunkDesc ccur = {nullptr, 0u, 0u, 0u, 0u};  // thread 0: the chunk of the tile it described last
     auto issue = [&](uint32_t i) {  // thread 0
-        TileDesc d = KEYED ? keyed_tile(aos_in, n_rec, t0 + i) : raw_tile(chunks, n_chunks, t0 + i);
+        TileDesc d = KEYED ? keyed_tile(aos_in, n_rec, t0 + i) : raw_tile(chunks, n_chunks, t0 + i, ccur);
         s_desc[(goff + i) % kIdxBigStages] = d;
         ring_issue_stream(stage_ptr(i), &bars[(goff + i) % kIdxBigStages], d.ptr, d.count * kRecB);
     };

@@ -136,6 +136,27 @@ __device__ __forceinline__ TileDesc raw_tile(const ChunkDesc* __restrict__ chunk
     return d;
 }
 
+// The same with the chunk of the caller's previous tile kept in `cur` (registers; start it zeroed): consecutive tiles
+// nearly always share a chunk, and the search above is a chain of log2(n_chunks) dependent loads that thread 0 runs
+// between two barriers of every tile loop (105 chunks: 7 loads + the descriptor, four times per 4096-record tile).
+__device__ __forceinline__ TileDesc raw_tile(const ChunkDesc* __restrict__ chunks, uint32_t n_chunks, uint32_t t, ChunkDesc& cur)
+{
+    if (!(t >= cur.tile0 && (unsigned long long)(t - cur.tile0) * (unsigned long long)kTile < cur.n_records)) {
+        uint32_t lo = 0, hi = n_chunks - 1;
+        while (lo < hi) {
+            uint32_t mid = (lo + hi + 1) >> 1;
+            if (__ldg(&chunks[mid].tile0) <= t) lo = mid; else hi = mid - 1;
+        }
+        cur = chunks[lo];
+    }
+    const uint32_t local = (t - cur.tile0) * (uint32_t)kTile;
+    TileDesc d;
+    d.ptr = cur.ptr + (size_t)local * kRecBytes;
+    d.first_index = cur.first_index + local;
+    d.count = min((uint32_t)kTile, cur.n_records - local);
+    return d;
+}
+
 // the segment of CTA s: tiles [t0, t1)
 __device__ __forceinline__ void segment_of(const Span& sp, uint32_t& t0, uint32_t& t1)
 {
@@ -309,13 +330,14 @@ __global__ void __launch_bounds__(kThreads, 2) k_count_raw(const ChunkDesc* __re
     split_segment_of(sp, t0, t1);
     const uint32_t n = t1 - t0;
 
+    ChunkDesc ccur = {nullptr, 0u, 0u, 0u, 0u};  // thread 0: the chunk of the tile it described last
     griddep_launch();  // the scatter behind this kernel may set up and prefetch on SMs this grid has left
     griddep_wait();    // the chunk table (k_set_chunks) when this kernel was itself launched as a dependent
     if (threadIdx.x == 0) {
         for (uint32_t k = 0; k < n_stages; ++k) mbar_init(&bars[k], 1);
         mbar_fence_init();
         for (uint32_t k = 0; k < n_stages && k < n; ++k) {
-            TileDesc d = raw_tile(chunks, n_chunks, t0 + k);
+            TileDesc d = raw_tile(chunks, n_chunks, t0 + k, ccur);
             s_desc[k] = d;
             ring_issue(reinterpret_cast<uint32_t*>(smem + L.ring + k * L.stage_bytes), &bars[k], d.ptr, d.count * kRecBytes);
         }
@@ -409,7 +431,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_count_raw(const ChunkDesc* __re
         }
         __syncthreads();  // every thread is done with the stage
         if (threadIdx.x == 0 && i + n_stages < n) {
-            TileDesc d = raw_tile(chunks, n_chunks, t0 + i + n_stages);
+            TileDesc d = raw_tile(chunks, n_chunks, t0 + i + n_stages, ccur);
             s_desc[stage] = d;
             ring_issue(raw, &bars[stage], d.ptr, d.count * kRecBytes);
         }
@@ -804,7 +826,8 @@ __global__ void __launch_bounds__(kThreads, 2) k_scatter_otf(const ChunkDesc* __
     segment_of(sp, t0, t1);
     const uint32_t n = t1 - t0;
     uint32_t grun[8];
-    auto desc_of = [&](uint32_t t) { return raw_tile(chunks, n_chunks, t); };
+    ChunkDesc ccur = {nullptr, 0u, 0u, 0u, 0u};  // the chunk of the tile this thread described last
+    auto desc_of = [&](uint32_t t) { return raw_tile(chunks, n_chunks, t, ccur); };
     scatter_prologue<kStagesRaw>(smem, L, B, Bp, n, t0, kRecBytes, desc_of, table, stride, col, grun);
     if (fs.n_cols != 0) fused_first_slots<kWarps>(fs, table, stride, B, col, gcur, lstart, misc, grun);  // raw table
     stage_edges(g, s_edges);
@@ -913,7 +936,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_scatter_otf(const ChunkDesc* __
         }
         __syncthreads();  // the stage and perm/pdest are free again
         if (threadIdx.x == 0 && i + kStagesRaw < n) {
-            TileDesc d = raw_tile(chunks, n_chunks, t0 + i + kStagesRaw);
+            TileDesc d = raw_tile(chunks, n_chunks, t0 + i + kStagesRaw, ccur);
             s_desc[stage] = d;
             ring_issue(raw, &bars[stage], d.ptr, d.count * kRecBytes);
         }
