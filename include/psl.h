@@ -49,7 +49,10 @@ enum { PSL_EBIN_LINEAR = 0,   /* n_ebins uniform bins on [e_min, e_max] (PAPER.m
        PSL_EBIN_EDGES = 1 };  /* caller-supplied ascending edge table with n_ebins+1 entries */
 enum { PSL_MEM_PAGEABLE = 0, PSL_MEM_PINNED = 1, PSL_MEM_DEVICE = 2 };
 enum { PSL_OUT_PROJ = 1u,           /* also write xp, yp: the position at the fluence-map plane */
-       PSL_DROP_ZERO_WEIGHT = 2u }; /* drop survivors whose final weight is exactly 0 (default: keep) */
+       PSL_DROP_ZERO_WEIGHT = 2u,   /* drop survivors whose final weight is exactly 0 (default: keep) */
+       PSL_NO_COMPACT = 4u };       /* diagnostic, same results: ONTHEFLY with <= 256 keys and a rejecting beam takes the
+                                       two-pass path (histogram, then scatter over all records) instead of compacting
+                                       the survivors in the histogram pass; used for A/B runs and tests */
 
 /* One phase-space particle: 28 bytes, packed, little-endian.  type: 0 photon, 1 electron, 2 positron.
  * (u, v) are direction cosines; the third one is w = sqrt(1 - u^2 - v^2) > 0 (always downstream). */
@@ -78,7 +81,7 @@ typedef struct {
     uint64_t max_host_records; /* of those, how many may arrive from HOST memory (device landing zone) */
     uint64_t max_beam_records; /* INDEX mode: most records one beam's ROI may select; 0 = max_records */
     uint32_t max_chunks;       /* most psl_load_chunk calls between resets; 0 = 4096 */
-    uint32_t flags;            /* PSL_OUT_PROJ | PSL_DROP_ZERO_WEIGHT */
+    uint32_t flags;            /* PSL_OUT_PROJ | PSL_DROP_ZERO_WEIGHT | PSL_NO_COMPACT */
     int32_t device;            /* CUDA device ordinal */
     void* stream;              /* cudaStream_t owned by the caller (NULL = default stream) */
     void* workspace;           /* DEVICE memory owned by the caller, 256-byte aligned */
@@ -142,8 +145,8 @@ uint64_t psl_workspace_bytes(const psl_config* cfg);
 psl_status psl_create(const psl_config* cfg, psl_ctx** out);
 
 /* Append n records ("particle data are copied in chunks").  `records` is HOST pageable, HOST
- * pinned or DEVICE memory per mem_kind.  n must be a multiple of 4 except for the last chunk before a
- * build.  HOST chunks are copied on the internal copy stream into the workspace (pageable ones through two
+ * pinned or DEVICE memory per mem_kind.  n must be a multiple of 4 except for the last chunk loaded before
+ * psl_reset (PSL_ERR_ARG for any chunk after it).  HOST chunks are copied on the internal copy stream into the workspace (pageable ones through two
  * pinned staging buffers); the source must stay untouched until psl_wait_loads() or any later
  * synchronising call returns.  DEVICE chunks are BORROWED, not copied: they must stay valid and unchanged
  * until the next psl_reset/psl_destroy (ONTHEFLY) or until the index is finalised (INDEX).  In INDEX mode
@@ -180,7 +183,8 @@ psl_status psl_roi_from_jaws(const psl_geometry* g, const psl_beam* beam, float 
  * the beam's ROI ("any portion of its area"); rx0 > rx1 or ry0 > ry1 when nothing is selected. */
 psl_status psl_roi_bins(const psl_ctx* ctx, const psl_beam* beam, int32_t bins_out[4]);
 
-/* Forget all chunks and results (keeps the configuration and workspace). */
+/* Forget all chunks and results (keeps the configuration and workspace).  Blocks the HOST until every HOST chunk
+ * loaded so far has left its source buffer (as psl_wait_loads); work already enqueued on the stream is not waited for. */
 psl_status psl_reset(psl_ctx* ctx);
 
 void psl_destroy(psl_ctx* ctx);
@@ -193,14 +197,16 @@ uint64_t psl_kernel_launches(const psl_ctx* ctx);
 
 /* Optional device-side timing of the library's own kernels, by class, with CUDA events recorded on the
  * context's stream around each launch (a few microseconds of overhead per build while enabled). */
-enum { PSL_K_COUNT = 0,   /* histogram passes (a8) */
+enum { PSL_K_COUNT = 0,   /* histogram passes over raw records (a1-a4, a6, a8) */
        PSL_K_SCAN = 1,    /* exclusive scans (a9) */
        PSL_K_SCATTER = 2, /* ONTHEFLY decode + jaw + fluence + stable scatter (a1-a7, a10) */
        PSL_K_INDEX_A = 3, /* INDEX pass A scatter (a11) */
        PSL_K_INDEX_B = 4, /* INDEX pass B scatter (a11) */
        PSL_K_BEAM = 5,    /* per-beam ROI + jaw + fluence + compaction from the index (a5-a7, a10) */
        PSL_K_OTHER = 6,   /* offsets / statistics / tile descriptors */
-       PSL_K_CLASSES = 7 };
+       PSL_K_COUNT_KEYS = 7, /* INDEX pass B histogram over the keyed records (a8 of the second digit) */
+       PSL_K_SAMPLE = 8,  /* sampling layer over the index: budgets, round-robin gather */
+       PSL_K_CLASSES = 9 };
 typedef struct {
     double ms[PSL_K_CLASSES];         /* summed device time */
     uint64_t launches[PSL_K_CLASSES]; /* timed brackets (SCAN: one bracket = its three kernels) */

@@ -69,10 +69,21 @@ def build_lib(force: bool = False) -> str:
 _lib = None
 
 
+def use_library(path: Optional[str]) -> None:
+    """Load the oracle from another shared object (tests/test_oracle_mutations.py builds deliberately wrong copies
+    of psl_oracle.c to check that the pins catch them); None goes back to the real one."""
+    global _lib, _override
+    _override = path
+    _lib = None
+
+
+_override = None
+
+
 def _load():
     global _lib
     if _lib is None:
-        lib = C.CDLL(build_lib())
+        lib = C.CDLL(_override or build_lib())
         lib.orc_build.restype = C.c_uint64
         lib.orc_n_keys.restype = C.c_uint32
         lib.orc_bin_width.restype = C.c_float

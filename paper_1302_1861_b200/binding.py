@@ -19,7 +19,7 @@ from . import _build
 MODE_ONTHEFLY, MODE_INDEX = 0, 1
 EBIN_LINEAR, EBIN_EDGES = 0, 1
 MEM_PAGEABLE, MEM_PINNED, MEM_DEVICE = 0, 1, 2
-OUT_PROJ, DROP_ZERO_WEIGHT = 1, 2
+OUT_PROJ, DROP_ZERO_WEIGHT, NO_COMPACT = 1, 2, 4
 RECORD_BYTES = 28
 
 _STATUS = {0: "PSL_OK", 1: "PSL_ERR_ARG", 2: "PSL_ERR_STATE", 3: "PSL_ERR_CAPACITY", 4: "PSL_ERR_GEOMETRY",
@@ -77,11 +77,11 @@ class Batch(C.Structure):
                [("n_bins", C.c_uint32)]
 
 
-K_CLASSES = ("count", "scan", "scatter", "index_a", "index_b", "beam", "other")
+K_CLASSES = ("count", "scan", "scatter", "index_a", "index_b", "beam", "other", "count_keys", "sample")
 
 
 class Profile(C.Structure):
-    _fields_ = [("ms", C.c_double * 7), ("launches", C.c_uint64 * 7)]
+    _fields_ = [("ms", C.c_double * len(K_CLASSES)), ("launches", C.c_uint64 * len(K_CLASSES))]
 
 
 _lib = None
@@ -224,7 +224,7 @@ class PslContext:
             self._h = C.c_void_p()
             raise PslError(rc, self.lib.psl_last_error(None).decode())
         self._keep = []       # borrowed device chunks, host sources in flight
-        self._beam_keep = []  # device fluence maps
+        self._beam_keep = {}  # id(source array) -> (source array, device fluence map)
         self.n_types, self.n_ebins = grid["n_types"], grid["n_ebins"]
         self.n_pos = grid["n_xbins"] * grid["n_ybins"]
         self.n_keys = self.n_types * self.n_ebins * self.n_pos
@@ -254,13 +254,19 @@ class PslContext:
             out.jaw_x1, out.jaw_x2, out.jaw_y1, out.jaw_y2 = j
         fl = b.get("fluence")
         if fl is not None:
-            if isinstance(fl, np.ndarray):
-                fl = torch.from_numpy(np.ascontiguousarray(fl, dtype=np.float32))
-            with torch.cuda.stream(self.stream):
-                fl = fl.to(self.device, dtype=torch.float32).contiguous()
-            self._beam_keep.append(fl)
-            out.fluence = fl.data_ptr()
-            out.map_ny, out.map_nx = fl.shape
+            # one device copy per source array, reused by later builds of the same beam (bounded: the oldest go first)
+            hit = self._beam_keep.get(id(fl))
+            if hit is not None and hit[0] is fl:
+                dev_fl = hit[1]
+            else:
+                src = torch.from_numpy(np.ascontiguousarray(fl, dtype=np.float32)) if isinstance(fl, np.ndarray) else fl
+                with torch.cuda.stream(self.stream):
+                    dev_fl = src.to(self.device, dtype=torch.float32).contiguous()
+                while len(self._beam_keep) >= 64:
+                    self._beam_keep.pop(next(iter(self._beam_keep)))
+                self._beam_keep[id(fl)] = (fl, dev_fl)
+            out.fluence = dev_fl.data_ptr()
+            out.map_ny, out.map_nx = dev_fl.shape
         out.map_x0, out.map_y0 = b.get("map_x0", 0.0), b.get("map_y0", 0.0)
         out.map_dx, out.map_dy = b.get("map_dx", 1.0), b.get("map_dy", 1.0)
         out.has_roi = 0 if r is None else 1
@@ -268,6 +274,8 @@ class PslContext:
             out.roi_x1, out.roi_x2, out.roi_y1, out.roi_y2 = r
         out.mu_weight = b.get("mu_weight", 1.0)
         out.gantry_deg = b.get("gantry_deg", 0.0)
+        out.coll_deg = b.get("coll_deg", 0.0)
+        out.couch_deg = b.get("couch_deg", 0.0)
         return out
 
     # -- the C-ABI calls -----------------------------------------------------------------------------
@@ -350,7 +358,7 @@ class PslContext:
             self.lib.psl_destroy(self._h)
             self._h = C.c_void_p()
         self._keep = []
-        self._beam_keep = []
+        self._beam_keep = {}
 
     def __del__(self):
         try:

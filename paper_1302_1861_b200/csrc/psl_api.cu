@@ -104,7 +104,7 @@ psl_status derive(const psl_config* c, Derived* d, char* err)
     if (n_pos > 1 || c->mode == PSL_MODE_INDEX) {
         int32_t t;
         if (!(c->dx > 0 && c->dy > 0 && isfinite(c->dx) && isfinite(c->dy))) { set_err(err, "config: dx, dy must be positive"); return PSL_ERR_ARG; }
-        if (!is_integer_ratio(c->x_min, c->dx, &t) || !is_integer_ratio(c->y_min, c->dy, &t)) { set_err(err, "config: x_min/dx and y_min/dy must be integers"); return PSL_ERR_ARG; }
+        if (n_pos > 1 && (!is_integer_ratio(c->x_min, c->dx, &t) || !is_integer_ratio(c->y_min, c->dy, &t))) { set_err(err, "config: x_min/dx and y_min/dy must be integers"); return PSL_ERR_ARG; }
     }
     psl_status gs = check_geometry(c->geom, err);
     if (gs != PSL_OK) return gs;
@@ -119,8 +119,9 @@ psl_status derive(const psl_config* c, Derived* d, char* err)
     // ONTHEFLY builds in one launch over all chunks; INDEX counts chunk by chunk as the chunks land
     uint64_t cols_cap = kMaxSegments;
     if (c->mode == PSL_MODE_INDEX) {
+        // a chunk of nt tiles takes min(nt, segments per launch) x kIdxSplit columns: at most kIdxSplit per tile
         cols_cap = (uint64_t)d->max_chunks * kMaxSegments;
-        if (cols_cap > tiles_cap) cols_cap = tiles_cap;
+        if (cols_cap > (uint64_t)kIdxSplit * tiles_cap) cols_cap = (uint64_t)kIdxSplit * tiles_cap;
     }
     if (c->mode == PSL_MODE_ONTHEFLY) {
         if (K > kMaxBuckets) { set_err(err, "ONTHEFLY mode handles at most %d keys (got %llu); use PSL_MODE_INDEX", kMaxBuckets, (unsigned long long)K); return PSL_ERR_ARG; }
@@ -316,6 +317,7 @@ struct psl_ctx {
     uint32_t chunks_uploaded = 0;
     std::vector<ChunkLaunch> idx_launches;
     std::vector<SpanSeg> h_spans;  // INDEX: the per-chunk count launches, replayed by pass A's scatter
+    std::vector<uint32_t> h_idx_batch_off;  // INDEX: batch offsets of the bare index (n_batches+1)
     // state
     uint64_t n_records = 0, n_host_records = 0;
     uint32_t n_tiles = 0, n_chunks = 0, n_cols = 0;
@@ -486,8 +488,8 @@ psl_status make_beam(const psl_ctx* ctx, const psl_beam* b, DevBeam* out, char* 
 // bins c of [origin + c d, origin + (c+1) d) with positive-length overlap with (lo, hi)
 void select_axis(double origin, double d, int n, double lo, double hi, int* first, int* last)
 {
-    int f = (int)fmax(0.0, floor((lo - origin) / d) - 1.0);
-    if (!(lo - origin > 0)) f = 0;
+    const double fg = floor((lo - origin) / d) - 1.0;  // clamped in double: the ROI may lie far outside the grid
+    int f = !(fg > 0.0) ? 0 : (fg >= (double)n ? n : (int)fg);
     while (f < n && !(origin + (double)(f + 1) * d > lo)) ++f;
     double lg = floor((hi - origin) / d) + 1.0;
     int l = lg >= (double)n ? n - 1 : (lg < 0 ? -1 : (int)lg);
@@ -711,7 +713,7 @@ psl_status finalize_index(psl_ctx* ctx)
         uint32_t ntb = (uint32_t)((ctx->n_records + kTile - 1) / kTile);
         const uint32_t Sb = ntb < ctx->S_b ? ntb : ctx->S_b;
         {
-            Prof prof(ctx, PSL_K_COUNT);
+            Prof prof(ctx, PSL_K_COUNT_KEYS);
             k_count_keys<<<Sb * ctx->split_b, kThreads, ctx->sm_count_b, ctx->stream>>>(aos, scalar(ctx, SC_NIDX), d.B_hi, d.lo_bits, table_b,
                                                                                      kMaxSegments, ctx->split_b);
             LAUNCHED();
@@ -749,14 +751,16 @@ psl_status finalize_index(psl_ctx* ctx)
     CU(cudaStreamSynchronize(ctx->stream));
     ctx->idx_stats = *ctx->h_stats;
     ctx->n_idx = ctx->h_idx_offsets[d.K];
+    // the bare index's batch offsets: a host array of their own (h_batch_off is the target of every beam build's
+    // asynchronous copy)
+    ctx->h_idx_batch_off.resize(d.n_batches + 1);
+    for (uint32_t b = 0; b <= d.n_batches; ++b) ctx->h_idx_batch_off[b] = ctx->h_idx_offsets[(uint64_t)b * d.n_pos];
     ctx->indexed = true;
     return PSL_OK;
 }
 
 psl_status expose_index(psl_ctx* ctx)
 {
-    const Derived& d = ctx->d;
-    for (uint32_t b = 0; b <= d.n_batches; ++b) ctx->h_batch_off[b] = ctx->h_idx_offsets[(uint64_t)b * d.n_pos];
     if (!ctx->soa_view && ctx->n_idx > 0) {  // the index is kept as keyed records; the SoA arrays are made on demand
         k_index_to_soa<<<1184, 256, 0, ctx->stream>>>(at<uint4>(ctx, ctx->L.aos_index), scalar(ctx, SC_NIDX), idx_out(ctx));
         LAUNCHED();
@@ -1016,7 +1020,7 @@ psl_status psl_create(const psl_config* cfg, psl_ctx** out)
             ctx->S_otf = width(occ);
         }
         ctx->count_split = ctx->big_tiles ? 2 : 1;  // one scatter CTA per SM, two histogram CTAs
-        if (ctx->big_tiles && ctx->L.comp != 0 && getenv("PSL_NO_COMPACT") == nullptr) {
+        if (ctx->big_tiles && ctx->L.comp != 0 && !(cfg->flags & PSL_NO_COMPACT)) {
             int max_smem = 0;
             CUC(cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, cfg->device));
             ctx->sm_scatter_comp = comp_layout(d.K).total;
@@ -1064,6 +1068,7 @@ psl_status psl_reset(psl_ctx* ctx)
     if (!ctx) return PSL_ERR_ARG;
     CU(cudaSetDevice(ctx->cfg.device));
     // later host-chunk copies must not overtake kernels of an earlier build that still read the landing zone
+    CU(cudaStreamSynchronize(ctx->copy_stream));  // every HOST source buffer has been read: the caller may reuse them
     CU(cudaEventRecord(ctx->ev_main, ctx->stream));
     CU(cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_main, 0));
     ctx->n_records = ctx->n_host_records = 0;
@@ -1098,6 +1103,11 @@ psl_status psl_load_chunk(psl_ctx* ctx, const void* records, uint64_t n, int32_t
     if (ctx->n_chunks + 1 > ctx->d.max_chunks) { set_err(ctx->err, "load_chunk: more than max_chunks"); return PSL_ERR_CAPACITY; }
     const bool host = mem_kind != PSL_MEM_DEVICE;
     if (host && ctx->n_host_records + n > ctx->cfg.max_host_records) { set_err(ctx->err, "load_chunk: more host records than max_host_records"); return PSL_ERR_CAPACITY; }
+    const uint32_t nt = (uint32_t)((n + kTile - 1) / kTile);
+    if (ctx->cfg.mode == PSL_MODE_INDEX) {  // checked before anything is enqueued: a failing call leaves the context as it was
+        const uint32_t n_seg = nt < ctx->S_a ? nt : ctx->S_a;
+        if (ctx->n_cols + n_seg * ctx->split_a > ctx->d.cols_cap) { set_err(ctx->err, "load_chunk: out of table columns"); return PSL_ERR_CAPACITY; }
+    }
     CU(cudaSetDevice(ctx->cfg.device));
 
     const uint8_t* dev_ptr;
@@ -1129,7 +1139,6 @@ psl_status psl_load_chunk(psl_ctx* ctx, const void* records, uint64_t n, int32_t
         dev_ptr = static_cast<const uint8_t*>(records);
     }
 
-    const uint32_t nt = (uint32_t)((n + kTile - 1) / kTile);
     const uint32_t tile0 = ctx->n_tiles;
     ChunkDesc cd;
     cd.ptr = dev_ptr;
@@ -1151,7 +1160,6 @@ psl_status psl_load_chunk(psl_ctx* ctx, const void* records, uint64_t n, int32_t
         psl_ctx::ChunkLaunch cl;
         cl.span = {tile0, nt, ctx->n_cols, ctx->split_a};
         cl.n_seg = nt < ctx->S_a ? nt : ctx->S_a;
-        if (ctx->n_cols + cl.n_seg * ctx->split_a > ctx->d.cols_cap) { set_err(ctx->err, "load_chunk: out of table columns"); return PSL_ERR_CAPACITY; }
         Prof prof(ctx, PSL_K_COUNT);
         count_idx_fn(ctx->grid.has_pos != 0, ctx->grid.ebin_mode != 0)<<<cl.n_seg * ctx->split_a, kThreads, ctx->sm_count_raw, ctx->stream>>>(
             chunks, ctx->n_chunks + 1, cl.span, ctx->grid, none, ctx->d.B_lo, (1u << ctx->d.lo_bits) - 1u,
@@ -1219,8 +1227,9 @@ psl_status psl_get_batch(psl_ctx* ctx, int32_t t, int32_t ie, psl_batch* out)
     const Derived& d = ctx->d;
     const Layout& L = ctx->L;
     uint32_t b = whole ? 0u : (uint32_t)(t * ctx->cfg.n_ebins + ie);
-    uint32_t first = ctx->h_batch_off[b];
-    uint32_t last = ctx->h_batch_off[whole ? d.n_batches : b + 1];
+    const uint32_t* boff = ctx->result == RES_INDEX ? ctx->h_idx_batch_off.data() : ctx->h_batch_off;
+    uint32_t first = boff[b];
+    uint32_t last = boff[whole ? d.n_batches : b + 1];
     memset(out, 0, sizeof *out);
     out->first = first;
     out->count = last - first;

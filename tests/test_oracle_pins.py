@@ -548,3 +548,152 @@ def test_generator_shape_matches_recipe():
     assert np.argmax(hist) in (1, 2)  # mode near 0.5 MeV
     assert abs(ph.mean() - 1.0) < 0.02  # Gamma(2, 0.5) mean = 1 (truncation removes < 0.1 %)
     assert (r["wt"] == 1.0).all() and np.abs(r["x"]).max() < 20 and np.abs(r["y"]).max() < 20
+
+
+# ---------------------------------------------------------------------------------------------
+# x/y-asymmetric parameters: non-square grid, distinct jaw / map planes, non-square map.  Every pin above uses
+# n_xbins == n_ybins, dx == dy, a square map and z_jaw_x == z_jaw_y == z_map; the ones below are chosen so that
+# an x<->y slip in the key, the jaw planes, the map plane or the map's row stride fails at least one of them
+# (tests/test_oracle_mutations.py applies exactly those slips to a copy of the oracle and checks that they do).
+# SURVEY 8(c) steps 3, 4, 6, 7.
+# ---------------------------------------------------------------------------------------------
+ASYM_GRID = dict(n_types=2, n_ebins=3, n_xbins=12, n_ybins=5, x_min=-3.0, y_min=-0.5, dx=0.5, dy=0.25)
+ASYM_GEOMETRY = dict(z_src=-100.0, z_plane=0.0, z_jaw_x=40.0, z_jaw_y=60.0, z_map=80.0, z_iso=100.0)
+
+
+def test_non_square_grid_keys_enumerate_every_cell_exactly_once():
+    # 12 x 5 position bins of 0.5 x 0.25 cm from (-3, -0.5), 3 energy bins on [0, 6], 2 type divisions: one
+    # particle at the centre of every (t, ie, iy, ix) cell, written in key order => keys = 0 .. K-1
+    g = W._grid(**ASYM_GRID)
+    o = O.Oracle(g, W.GEOMETRY)
+    assert o.n_keys == 2 * 3 * 12 * 5
+    rows = []
+    for t in range(2):
+        for ie in range(3):
+            for iy in range(5):
+                for ix in range(12):
+                    rows.append((t, (ie + 0.5) * 2.0, -3.0 + (ix + 0.5) * 0.5, -0.5 + (iy + 0.5) * 0.25, 0, 0, 1))
+    r = recs(rows)
+    cls, keys = o.classify(r, None)
+    assert (cls == O.SURVIVOR).all()
+    assert np.array_equal(keys, np.arange(o.n_keys, dtype=np.uint32))
+    # the same through the whole build, fed in reverse: one record per key, slots = keys
+    res = o.build(r[::-1].copy(), None)
+    assert (res["counts"] == 1).all() and np.array_equal(res["offsets"], np.arange(o.n_keys + 1, dtype=np.uint32))
+    assert np.array_equal(res["src_index"], np.arange(o.n_keys, dtype=np.uint32)[::-1])
+    # grid edges per axis: x in [-3, 3), y in [-0.5, 0.75)
+    edge = recs([(0, 1.0, 2.99, 0.74, 0, 0, 1), (0, 1.0, 3.0, 0.0, 0, 0, 1), (0, 1.0, 0.0, 0.75, 0, 0, 1),
+                 (0, 1.0, -3.0, -0.5, 0, 0, 1), (0, 1.0, below(-3.0), 0.0, 0, 0, 1), (0, 1.0, 0.0, below(-0.5), 0, 0, 1),
+                 (0, 1.0, 0.8, 0.0, 0, 0, 1)])  # the last one: inside in x only if x uses n_xbins * dx, row 2, column 7
+    cls, keys = o.classify(edge, None)
+    assert list(cls) == [O.SURVIVOR, O.OUTSIDE_GRID, O.OUTSIDE_GRID, O.SURVIVOR, O.OUTSIDE_GRID, O.OUTSIDE_GRID, O.SURVIVOR]
+    assert keys[0] == 4 * 12 + 11 and keys[3] == 0 and keys[6] == 2 * 12 + 7
+
+
+def test_non_square_grid_roi_rows_and_columns():
+    g = W._grid(**ASYM_GRID)
+    o = O.Oracle(g, W.GEOMETRY)
+    # x: [-1.2, 0.6) touches columns 3 (-1.5..-1.0) .. 7 (0.5..1.0); y: [0.0, 0.3) rows 2 (0..0.25), 3 (0.25..0.5)
+    assert o.roi_bins(W.make_beam(roi=(-1.2, 0.6, 0.0, 0.3))) == (3, 7, 2, 3)
+    rows = [(0, 1.0, -3.0 + (ix + 0.5) * 0.5, -0.5 + (iy + 0.5) * 0.25, 0, 0, 1) for iy in range(5) for ix in range(12)]
+    cls, keys = o.classify(recs(rows), W.make_beam(roi=(-1.2, 0.6, 0.0, 0.3)))
+    want = np.array([O.SURVIVOR if (3 <= ix <= 7 and 2 <= iy <= 3) else O.ROI_SKIPPED for iy in range(5) for ix in range(12)])
+    assert np.array_equal(cls, want)
+
+
+def _ideal_rays(n, seed, half_x, half_y):
+    """point-source rays (no angular jitter) through a half_x x half_y rectangle of the scoring plane"""
+    return W.generate(W.GenParams(seed=seed, sigma_deg=0.0, half_x=half_x, half_y=half_y), 0, n)
+
+
+def test_distinct_planes_each_axis_projects_to_its_own_plane():
+    # z_src = -100, z_plane = 0, z_jaw_x = 40, z_jaw_y = 60, z_map = 80, z_iso = 100: an ideal ray through (x, y)
+    # is at x * (z - z_src) / (z_plane - z_src) on the plane z
+    o = O.Oracle(grid_te(), ASYM_GEOMETRY)
+    r = _ideal_rays(50_000, 41, 12.0, 9.0)
+    x, y = r["x"].astype(np.float64), r["y"].astype(np.float64)
+    xj, yj = o.jaw_points(r)
+    far = (np.abs(x) > 0.5) & (np.abs(y) > 0.5)
+    assert np.allclose(xj[far], 1.4 * x[far], rtol=2e-6, atol=0)
+    assert np.allclose(yj[far], 1.6 * y[far], rtol=2e-6, atol=0)
+    assert not np.allclose(xj[far], 1.6 * x[far], rtol=1e-3) and not np.allclose(yj[far], 1.4 * y[far], rtol=1e-3)
+    res = o.build(r, W.make_beam(mu_weight=1.0))  # no jaws: everything survives, xm/ym for every record
+    s = res["src_index"]
+    f = far[s]
+    assert np.allclose(res["xm"][f], 1.8 * x[s][f], rtol=2e-6, atol=0)
+    assert np.allclose(res["ym"][f], 1.8 * y[s][f], rtol=2e-6, atol=0)
+    # jaw edges, given at the isocentre, scale to each axis' own plane: x by 140/200, y by 160/200
+    assert o.jaw_edge(10.0, 40.0) == pytest.approx(7.0, rel=1e-7) and o.jaw_edge(10.0, 60.0) == pytest.approx(8.0, rel=1e-7)
+
+
+def test_distinct_planes_jaw_box_accepts_only_with_the_right_plane_per_axis():
+    o = O.Oracle(grid_te(), ASYM_GEOMETRY)
+    beam = W.make_beam(jaws=(-10.0, 10.0, -10.0, 10.0))
+    # pencil rays (u = v = 0) stay at (x, y): the aperture at the jaw planes is [-7, 7) x [-8, 8)
+    pts = [(6.9, 7.9), (7.1, 0.0), (0.0, 8.1), (-7.0, -8.0), (below(-7.0), 0.0), (0.0, below(-8.0)), (7.5, 7.5), (6.9, -7.5)]
+    cls, _ = o.classify(recs([(0, 1.0, px, py, 0.0, 0.0, 1.0) for px, py in pts]), beam)
+    J, S = O.JAW_REJECTED, O.SURVIVOR
+    assert list(cls) == [S, J, J, S, J, J, J, S]
+    # ideal point-source rays: the field edge seen from the source is |x|, |y| < 5 at the scoring plane whatever the
+    # jaw planes are -- but only if each axis is projected to the plane its edges were scaled to
+    r = _ideal_rays(100_000, 42, 6.0, 6.0)
+    res = o.build(r, beam, want_classes=True)
+    x, y = r["x"].astype(np.float64), r["y"].astype(np.float64)
+    clear = (np.abs(np.abs(x) - 5.0) > 1e-4) & (np.abs(np.abs(y) - 5.0) > 1e-4)
+    want = (np.abs(x) < 5.0) & (np.abs(y) < 5.0)
+    assert clear.mean() > 0.999
+    assert np.array_equal((res["classes"] == S)[clear], want[clear])
+    # hand-placed: x = 4.7 passes (1.4 * 4.7 = 6.58 < 7) and would fail on the y plane (1.6 * 4.7 = 7.52);
+    #              y = 5.4 fails (1.6 * 5.4 = 8.64 >= 8) and would pass on the x plane (1.4 * 5.4 = 7.56 < 8)
+    def ray(px, py):
+        d = np.array([px, py, 100.0])
+        d /= np.linalg.norm(d)
+        return (0, 1.0, px, py, d[0], d[1], 1.0)
+
+    cls, _ = o.classify(recs([ray(4.7, 0.0), ray(0.0, 5.4), ray(4.7, 4.7), ray(0.0, -4.9)]), beam)
+    assert list(cls) == [S, J, S, S]
+
+
+def test_non_square_map_index_map_recovers_the_pixel():
+    # 96 columns of 0.25 cm from x = -12, 160 rows of 0.5 cm from y = -40, at z_map = 80 where an ideal ray through
+    # (x, y) sits at (1.8 x, 1.8 y); F[py, px] = py * 96 + px (exact in fp32)
+    o = O.Oracle(grid_te(), ASYM_GEOMETRY)
+    nx, ny = 96, 160
+    m = np.arange(nx * ny, dtype=np.float32).reshape(ny, nx)
+    beam = W.make_beam(fluence=m, map_x0=-12.0, map_y0=-40.0, map_dx=0.25, map_dy=0.5)
+    r = _ideal_rays(100_000, 43, 8.0, 24.0)  # +-14.4 x +-43.2 at the map plane: some rays miss the map
+    res = o.build(r, beam)
+    assert res["n_survivors"] == len(r)  # no jaws: nothing is rejected, zero-weight records are kept
+    s = res["src_index"]
+    xm, ym = 1.8 * r["x"][s].astype(np.float64), 1.8 * r["y"][s].astype(np.float64)
+    fx, fy = (xm + 12.0) / 0.25, (ym + 40.0) / 0.5
+    clear = (np.abs(fx - np.round(fx)) > 1e-3) & (np.abs(fy - np.round(fy)) > 1e-3)
+    px, py = np.floor(fx), np.floor(fy)
+    inside = (px >= 0) & (px < nx) & (py >= 0) & (py < ny)
+    want = np.where(inside, py * nx + px, 0.0).astype(np.float32)
+    assert clear.mean() > 0.98 and 0.5 < inside.mean() < 0.95
+    assert np.array_equal(res["wt"][clear], want[clear])
+    # direct probes of the lookup: row stride is map_nx, x picks the column, y the row
+    assert o.fluence_at(beam, -11.9, -39.9) == 0.0
+    assert o.fluence_at(beam, -11.9 + 0.25 * 5, -39.9) == 5.0
+    assert o.fluence_at(beam, -11.9, -39.9 + 0.5 * 3) == 3.0 * 96
+    assert o.fluence_at(beam, 11.9, 39.9) == 159.0 * 96 + 95
+    assert o.fluence_at(beam, 12.1, 0.0) == 0.0 and o.fluence_at(beam, 0.0, 40.1) == 0.0  # off the map
+    assert o.fluence_at(beam, 0.0, 30.0) == 140.0 * 96 + 48  # y beyond +-12 is still on this 80-cm-tall map
+
+
+def test_asymmetric_everything_index_route_equals_direct_route():
+    # non-square grid + distinct planes + non-square map + ROI through the whole build, both routes
+    g = W._grid(**dict(ASYM_GRID, n_types=3, n_ebins=8, n_xbins=48, n_ybins=20, x_min=-12.0, y_min=-2.5))
+    o = O.Oracle(g, ASYM_GEOMETRY)
+    r = _dirty_records(W.Workload("asym", 40_000, W.GenParams(7, half_x=13.0, half_y=3.0), W.MODE_INDEX, g), 40_000, 5)
+    m = W.fluence_uniform(3, nx=96, ny=40)
+    beam = W.make_beam(jaws=(-9.0, 11.0, -3.0, 2.0), fluence=m, map_x0=-12.0, map_y0=-10.0, map_dx=0.25, map_dy=0.5,
+                       roi=(-6.2, 7.9, -1.3, 1.1), mu_weight=0.5)
+    direct = o.build(r, beam, want_classes=True)
+    index = o.build(r, None)
+    keep = direct["classes"][index["src_index"]] == O.SURVIVOR
+    assert np.array_equal(index["src_index"][keep], direct["src_index"])
+    assert 100 < direct["n_survivors"] < direct["stats"]["n_in"] - direct["stats"]["n_roi_skipped"]
+    sel = o.roi_bins(beam)
+    assert sel == (11, 39, 4, 14)  # x: (-6.2+12)/0.5 = 11.6 -> 11, (7.9+12)/0.5 = 39.8 -> 39; y: 1.2/0.25 -> 4, 3.6/0.25 -> 14

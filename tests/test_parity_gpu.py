@@ -327,22 +327,20 @@ def test_big_tiles_ragged_chunks_and_ring_wraparound():
     check(w_small, dirty(w_small.records(), 8), None, chunk=3000, mem="device")
 
 
-def test_small_tiles_with_a_rejecting_beam_at_scale(monkeypatch):
-    """a beam with jaws and the survivor compaction switched off takes the 1024-record-tile scatter (two CTAs per
-    SM), which ranks from the histogram kernel's one byte per record; several tiles per CTA"""
-    monkeypatch.setenv("PSL_NO_COMPACT", "1")
+def test_small_tiles_with_a_rejecting_beam_at_scale():
+    """a beam with jaws and the survivor compaction switched off (PSL_NO_COMPACT) takes the 1024-record-tile scatter
+    (two CTAs per SM), which ranks from the histogram kernel's one byte per record; several tiles per CTA"""
     w = W.config(3, 1_500_000)
-    check(w, w.records(), w.beams[0], chunk=500_000, mem="device", flags=P().OUT_PROJ, proj=True)
+    check(w, w.records(), w.beams[0], chunk=500_000, mem="device", flags=P().OUT_PROJ | P().NO_COMPACT, proj=True)
 
 
-def test_compacted_survivors_at_scale_and_against_the_other_path(monkeypatch):
+def test_compacted_survivors_at_scale_and_against_the_other_path():
     """a beam with jaws and K <= 256: the histogram kernel compacts the survivors per segment and the scatter reads
     only those (psl_compact.cuh).  Against the oracle, and byte for byte against the path without compaction."""
     w = W.config(3, 1_500_000)
     r = dirty(w.records(), 11)
     a = check(w, r, w.beams[0], chunk=500_000, mem="device", flags=P().OUT_PROJ, proj=True)
-    monkeypatch.setenv("PSL_NO_COMPACT", "1")
-    b = library_result(run_library(w, r, w.beams[0], chunk=500_000, mem="device", flags=P().OUT_PROJ))
+    b = library_result(run_library(w, r, w.beams[0], chunk=500_000, mem="device", flags=P().OUT_PROJ | P().NO_COMPACT))
     for k in ("counts", "offsets", "src_index", "E", "x", "y", "u", "v", "w", "wt", "xp", "yp"):
         assert np.array_equal(a[k].view(np.uint32), b[k].view(np.uint32)), k
     assert a["stats"] == b["stats"]
@@ -504,4 +502,133 @@ def test_config5_streamed_at_1e8_records_nine_beams():
             assert int(c.sum().item()) == st["n_survivors"] == int(o[-1].item())
             assert st["n_in"] == n and st["n_survivors"] + st["n_jaw_rejected"] + st["n_roi_skipped"] + st["n_invalid"] + \
                 st["n_outside_grid"] + st["n_zero_weight"] == n
+    ctx.destroy()
+
+
+# ---------------------------------------------------------------------------------------------
+# x/y-asymmetric configurations: n_xbins != n_ybins, dx != dy, x_min != y_min, z_jaw_x != z_jaw_y != z_map,
+# map_nx != map_ny, map_dx != map_dy, map_x0 != map_y0 (every other case in this file is symmetric in x and y, so a
+# swapped pair in the kernels or in make_beam would pass it); mirrors tests/test_oracle_pins.py's asymmetric pins
+# ---------------------------------------------------------------------------------------------
+ASYM_GEOMETRY = dict(z_src=-100.0, z_plane=0.0, z_jaw_x=40.0, z_jaw_y=60.0, z_map=80.0, z_iso=100.0)
+
+
+def asym_beam(roi=None, seed=3):
+    return W.make_beam(jaws=(-9.0, 11.0, -3.0, 2.0), fluence=W.fluence_uniform(seed, nx=96, ny=40), map_x0=-12.0,
+                       map_y0=-10.0, map_dx=0.25, map_dy=0.5, roi=roi, mu_weight=0.5)
+
+
+@pytest.mark.parametrize("keys", ["few", "many"])
+def test_asymmetric_grid_planes_and_map_onthefly(keys):
+    """ONTHEFLY with position bins: 160 keys (4096-record tiles, compacted survivors for the rejecting beam) and
+    1920 keys (1024-record tiles); method 1 (no beam), a rejecting beam, a beam that only weights"""
+    shape = dict(n_types=2, n_ebins=2, n_xbins=8, n_ybins=5, x_min=-12.0, y_min=-3.0, dx=3.0, dy=1.0) if keys == "few" else \
+        dict(n_types=2, n_ebins=4, n_xbins=48, n_ybins=5, x_min=-12.0, y_min=-3.0, dx=0.5, dy=1.0)
+    g = W._grid(**shape)
+    w = W.Workload("asym_otf", 300_000, W.GenParams(17, half_x=13.0, half_y=3.0), W.MODE_ONTHEFLY, g, geometry=ASYM_GEOMETRY)
+    r = dirty(w.records(), 31)
+    nomap = W.make_beam(jaws=(-9.0, 11.0, -3.0, 2.0), mu_weight=0.25)
+    weight_only = dict(asym_beam(), jaws=None)
+    for beam in (None, asym_beam(), nomap, weight_only):
+        lib = check(w, r, beam, chunk=70_000, flags=P().OUT_PROJ, proj=True)
+        assert lib["n_survivors"] > 1000
+    # the x and y extents differ: a record at (10, 0) is inside, one at (0, 10) is outside
+    probe = np.zeros(8, dtype=W.RECORD_DTYPE)
+    probe[:] = (0, 1.0, 0.0, 0.0, 0.0, 0.0, 1.0)
+    probe["x"][:4], probe["y"][4:] = 10.0, 10.0
+    lib = check(w, probe, None)
+    assert lib["n_survivors"] == 4 and lib["stats"]["n_outside_grid"] == 4
+
+
+def test_asymmetric_grid_planes_and_map_index():
+    """INDEX: 48 x 20 position bins of 0.5 x 0.25 cm from (-12, -2.5), the bare index, then beams whose ROI row and
+    column ranges differ, with PSL_OUT_PROJ"""
+    g = W._grid(n_ebins=8, n_xbins=48, n_ybins=20, x_min=-12.0, y_min=-2.5, dx=0.5, dy=0.25)
+    w = W.Workload("asym_idx", 400_000, W.GenParams(18, half_x=13.0, half_y=3.0), W.MODE_INDEX, g, geometry=ASYM_GEOMETRY)
+    r = dirty(w.records(), 32)
+    orc = O.Oracle(g, ASYM_GEOMETRY)
+    ctx = run_library(w, r, None, chunk=150_000, flags=P().OUT_PROJ)
+    assert_matches_oracle(library_result(ctx), orc.build(r, None), index_only=True)
+    for roi in ((-6.2, 7.9, -1.3, 1.1), (-12.0, 12.0, 0.0, 0.25), (3.0, 3.5, -2.5, 2.5), None):
+        beam = asym_beam(roi)
+        ctx.build_batches(beam)
+        lib = library_result(ctx)
+        assert_matches_oracle(lib, orc.build(r, beam), proj=True)
+        if roi is not None:
+            assert ctx.roi_bins(beam) == orc.roi_bins(beam)
+        assert lib["n_survivors"] > 50
+    assert ctx.roi_bins(asym_beam((-6.2, 7.9, -1.3, 1.1))) == (11, 39, 4, 14)
+    ctx.destroy()
+
+
+def test_index_mode_with_an_energy_edge_table():
+    """INDEX + PSL_EBIN_EDGES (k_count_raw<IDX, POS, EDGES>, pass A with the edge search): config 1's 32 log-spaced
+    bins over a non-square position grid"""
+    g = W._grid(ebin_mode=W.EBIN_EDGES, n_ebins=32, e_min=0.01, e_max=6.0, e_edges=W.log_edges(0.01, 6.0, 32),
+                n_xbins=40, n_ybins=16, x_min=-20.0, y_min=-16.0, dx=1.0, dy=2.0)
+    w = W.Workload("idx_edges", 600_000, W.GenParams(19), W.MODE_INDEX, g)
+    r = dirty(w.records(), 33)
+    orc = O.Oracle(g, w.geometry)
+    ctx = run_library(w, r, None, chunk=200_000)
+    assert_matches_oracle(library_result(ctx), orc.build(r, None), index_only=True)
+    beam = W.make_beam(jaws=(-9.0, 5.0, -4.0, 12.0), fluence=W.fluence_uniform(4), roi=(-5.5, 3.5, -3.0, 7.0))
+    ctx.build_batches(beam)
+    assert_matches_oracle(library_result(ctx), orc.build(r, beam))
+    ctx.destroy()
+    # no position bins at all: INDEX over (type, energy) only, edge table
+    g1 = W._grid(ebin_mode=W.EBIN_EDGES, n_ebins=32, e_min=0.01, e_max=6.0, e_edges=W.log_edges(0.01, 6.0, 32))
+    w1 = W.Workload("idx_edges_nopos", 100_000, W.GenParams(20), W.MODE_INDEX, g1)
+    r1 = w1.records()
+    ctx = run_library(w1, r1, None)
+    assert_matches_oracle(library_result(ctx), O.Oracle(g1, w1.geometry).build(r1, None), index_only=True)
+    ctx.destroy()
+
+
+def test_index_mid_size_chunks_use_two_table_columns_per_tile():
+    """1e7 records in 100 000-record chunks: 98 tiles per chunk, each cut into 98 segments x 2 histogram CTAs = 196
+    table columns, i.e. twice the tile count (the capacity of the column table must allow for it)"""
+    w = W.config(4, 10_000_000)
+    p = P()
+    import torch
+
+    n, chunk = w.n_records, 100_000
+    host = torch.empty(n * 28, dtype=torch.uint8).pin_memory()
+    W.generate_into(w.gen, 0, n, host.data_ptr(), threads=8)
+    dev = host.cuda()
+    ctx = p.PslContext(w.grid, w.geometry, w.mode, max_records=n)
+    for f in range(0, n, chunk):
+        ctx.load_chunk(dev[f * 28:(f + chunk) * 28], p.MEM_DEVICE)
+    ctx.build_batches(w.beams[0])
+    r = host.numpy().view(W.RECORD_DTYPE)
+    assert_matches_oracle(library_result(ctx), O.Oracle(w.grid, w.geometry).build(r, w.beams[0]))
+    ctx.destroy()
+
+
+def test_beam_then_bare_index_without_a_sync_in_between():
+    """psl_build_batches(beam) leaves an asynchronous copy of its batch offsets in flight; the bare index exposed right
+    after it must report the index's own batches"""
+    w = W.config(4, 300_000)
+    r = w.records()
+    ctx = run_library(w, r, None)
+    orc = O.Oracle(w.grid, w.geometry).build(r, None)
+    for _ in range(20):
+        ctx.build_batches(w.beams[0])
+        ctx.build_batches(None)
+        b = ctx.get_batch(0, 5)
+        k0 = 5 * 6400
+        assert b["first"] == orc["offsets"][k0] and b["count"] == orc["offsets"][k0 + 6400] - orc["offsets"][k0]
+    ctx.destroy()
+
+
+def test_roi_far_outside_the_grid_is_empty_and_fast():
+    import time
+
+    w = W.config(4, 10_000)
+    ctx = run_library(w, w.records(), None)
+    t0 = time.perf_counter()
+    for roi in ((1e12, 2e12, -1.0, 1.0), (-2e12, -1e12, -1.0, 1.0), (-1.0, 1.0, 1e30, 2e30), (-1e30, 1e30, -1e30, 1e30)):
+        beam = W.make_beam(jaws=(-5, 5, -5, 5), roi=roi)
+        ctx.build_batches(beam)
+        assert_matches_oracle(library_result(ctx), O.Oracle(w.grid, w.geometry).build(w.records(), beam))
+    assert time.perf_counter() - t0 < 5.0
     ctx.destroy()

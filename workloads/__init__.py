@@ -167,11 +167,13 @@ def fluence_segments(seed: int, nx: int = 160, ny: int = 160) -> np.ndarray:
 
 
 def make_beam(jaws=None, fluence=None, map_x0=-20.0, map_y0=-20.0, map_d=0.25, roi=None, mu_weight=1.0,
-              gantry_deg=0.0) -> Dict:
+              gantry_deg=0.0, coll_deg=0.0, couch_deg=0.0, map_dx=None, map_dy=None) -> Dict:
     """A per-field description: jaws = (x1, x2, y1, y2) at isocentre or None; fluence = 2-D fp32
-    array [ny, nx] or None; roi = (x1, x2, y1, y2) at the scoring plane or None."""
-    return dict(jaws=jaws, fluence=fluence, map_x0=map_x0, map_y0=map_y0, map_dx=map_d, map_dy=map_d,
-                roi=roi, mu_weight=mu_weight, gantry_deg=gantry_deg)
+    array [ny, nx] or None (pixel size map_d, or map_dx x map_dy when they differ); roi = (x1, x2, y1, y2)
+    at the scoring plane or None; the three angles in degrees."""
+    return dict(jaws=jaws, fluence=fluence, map_x0=map_x0, map_y0=map_y0,
+                map_dx=map_d if map_dx is None else map_dx, map_dy=map_d if map_dy is None else map_dy,
+                roi=roi, mu_weight=mu_weight, gantry_deg=gantry_deg, coll_deg=coll_deg, couch_deg=couch_deg)
 
 
 @dataclass
