@@ -150,7 +150,8 @@ psl_status psl_create(const psl_config* cfg, psl_ctx** out);
  * pinned staging buffers); the source must stay untouched until psl_wait_loads() or any later
  * synchronising call returns.  DEVICE chunks are BORROWED, not copied: they must stay valid and unchanged
  * until the next psl_reset/psl_destroy (ONTHEFLY) or until the index is finalised (INDEX).  In INDEX mode
- * the chunk's keys are counted as soon as it lands, overlapping the next chunk's transfer. */
+ * a HOST chunk's keys are counted as soon as it lands, overlapping the next chunk's transfer; DEVICE chunks are
+ * counted together by one launch when the next HOST chunk arrives or the index is finalised. */
 psl_status psl_load_chunk(psl_ctx* ctx, const void* records, uint64_t n, int32_t mem_kind);
 
 /* Block the HOST until every chunk loaded so far has left its source buffer. */

@@ -321,6 +321,7 @@ struct psl_ctx {
     // state
     uint64_t n_records = 0, n_host_records = 0;
     uint32_t n_tiles = 0, n_chunks = 0, n_cols = 0;
+    uint32_t tiles_counted = 0, cols_bound = 0;  // INDEX: tiles already histogrammed; columns if every chunk were counted alone
     bool ragged = false;  // a chunk with n % 4 != 0 was loaded: no more chunks may follow
     bool indexed = false, soa_view = false;
     int result = RES_NONE;
@@ -542,6 +543,51 @@ SoAOut soa_out(psl_ctx* ctx, const uint64_t off[10])
     return o;
 }
 
+// chunk descriptors not yet on the device: uploaded 128 at a time (they travel as a kernel argument)
+psl_status upload_chunks(psl_ctx* ctx)
+{
+    ChunkDesc* chunks = at<ChunkDesc>(ctx, ctx->L.chunks);
+    for (size_t f = 0; f < ctx->pending_chunks.size(); f += 128) {
+        ChunkBatch cb;
+        const uint32_t m = (uint32_t)(ctx->pending_chunks.size() - f < 128 ? ctx->pending_chunks.size() - f : 128);
+        memcpy(cb.d, ctx->pending_chunks.data() + f, m * sizeof(ChunkDesc));
+        k_set_chunks<<<1, 128, 0, ctx->stream>>>(chunks + ctx->chunks_uploaded, cb, m);
+        LAUNCHED();
+        ctx->chunks_uploaded += m;
+    }
+    ctx->pending_chunks.clear();
+    return PSL_OK;
+}
+
+// INDEX: a8 for pass A over every tile loaded since the last count, in ONE launch.  HOST chunks are counted as they
+// land (the launch overlaps the transfer of the next chunk); DEVICE chunks wait here until a HOST chunk or the index
+// build flushes them, so a phase-space that is already resident is counted by one launch, not one per chunk
+// (105 launches of 48 us at config 5 cost 1.5 ms of tails and launch gaps).
+psl_status count_pending_tiles(psl_ctx* ctx)
+{
+    const uint32_t nt = ctx->n_tiles - ctx->tiles_counted;
+    if (nt == 0) return PSL_OK;
+    psl_status s = upload_chunks(ctx);
+    if (s != PSL_OK) return s;
+    DevBeam none;
+    memset(&none, 0, sizeof none);
+    psl_ctx::ChunkLaunch cl;
+    cl.span = {ctx->tiles_counted, nt, ctx->n_cols, ctx->split_a};
+    cl.n_seg = nt < ctx->S_a ? nt : ctx->S_a;
+    if (ctx->n_cols + cl.n_seg * ctx->split_a > ctx->d.cols_cap) { set_err(ctx->err, "out of table columns"); return PSL_ERR_CAPACITY; }
+    {
+        Prof prof(ctx, PSL_K_COUNT);
+        count_idx_fn(ctx->grid.has_pos != 0, ctx->grid.ebin_mode != 0)<<<cl.n_seg * ctx->split_a, kThreads, ctx->sm_count_raw, ctx->stream>>>(
+            at<ChunkDesc>(ctx, ctx->L.chunks), ctx->n_chunks, cl.span, ctx->grid, none, ctx->d.B_lo, (1u << ctx->d.lo_bits) - 1u,
+            at<uint32_t>(ctx, ctx->L.table_a), ctx->d.cols_cap, at<SegStats>(ctx, ctx->L.sstats), ctx->count_stages, nullptr, nullptr);
+        LAUNCHED();
+    }
+    ctx->idx_launches.push_back(cl);
+    ctx->n_cols += cl.n_seg * ctx->split_a;
+    ctx->tiles_counted = ctx->n_tiles;
+    return PSL_OK;
+}
+
 psl_status build_onthefly(psl_ctx* ctx, const DevBeam& bm)
 {
     const Derived& d = ctx->d;
@@ -561,15 +607,10 @@ psl_status build_onthefly(psl_ctx* ctx, const DevBeam& bm)
         CU(cudaMemsetAsync(stats, 0, sizeof(DevStats), ctx->stream));
     } else {
         ChunkDesc* chunks = at<ChunkDesc>(ctx, L.chunks);
-        for (size_t f = 0; f < ctx->pending_chunks.size(); f += 128) {
-            ChunkBatch cb;
-            const uint32_t m = (uint32_t)(ctx->pending_chunks.size() - f < 128 ? ctx->pending_chunks.size() - f : 128);
-            memcpy(cb.d, ctx->pending_chunks.data() + f, m * sizeof(ChunkDesc));
-            k_set_chunks<<<1, 128, 0, ctx->stream>>>(chunks + ctx->chunks_uploaded, cb, m);
-            LAUNCHED();
-            ctx->chunks_uploaded += m;
+        {
+            psl_status us = upload_chunks(ctx);
+            if (us != PSL_OK) return us;
         }
-        ctx->pending_chunks.clear();
         SegStats* ss = at<SegStats>(ctx, L.sstats);
         const bool pos = ctx->grid.has_pos != 0, edges = ctx->grid.ebin_mode != 0, proj = bm.has_map || bm.out_proj;
         const int bv = beam_variant(bm);
@@ -668,6 +709,10 @@ psl_status finalize_index(psl_ctx* ctx)
     uint32_t* idx_batch = at<uint32_t>(ctx, L.idx_batch_off);
     DevStats* stats = at<DevStats>(ctx, L.stats);
     const uint32_t nt = ctx->n_tiles;
+    {
+        psl_status cs = count_pending_tiles(ctx);  // DEVICE chunks loaded since the last HOST chunk
+        if (cs != PSL_OK) return cs;
+    }
     if (nt == 0) {
         CU(cudaMemsetAsync(idx_offsets, 0, (uint64_t)(d.K + 1) * 4, ctx->stream));
         CU(cudaMemsetAsync(idx_counts, 0, (uint64_t)d.K * 4, ctx->stream));
@@ -1073,6 +1118,7 @@ psl_status psl_reset(psl_ctx* ctx)
     CU(cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_main, 0));
     ctx->n_records = ctx->n_host_records = 0;
     ctx->n_tiles = ctx->n_chunks = ctx->n_cols = 0;
+    ctx->tiles_counted = ctx->cols_bound = 0;
     ctx->idx_launches.clear();
     ctx->pending_chunks.clear();
     ctx->chunks_uploaded = 0;
@@ -1106,7 +1152,8 @@ psl_status psl_load_chunk(psl_ctx* ctx, const void* records, uint64_t n, int32_t
     const uint32_t nt = (uint32_t)((n + kTile - 1) / kTile);
     if (ctx->cfg.mode == PSL_MODE_INDEX) {  // checked before anything is enqueued: a failing call leaves the context as it was
         const uint32_t n_seg = nt < ctx->S_a ? nt : ctx->S_a;
-        if (ctx->n_cols + n_seg * ctx->split_a > ctx->d.cols_cap) { set_err(ctx->err, "load_chunk: out of table columns"); return PSL_ERR_CAPACITY; }
+        if (ctx->cols_bound + n_seg * ctx->split_a > ctx->d.cols_cap) { set_err(ctx->err, "load_chunk: out of table columns"); return PSL_ERR_CAPACITY; }
+        ctx->cols_bound += n_seg * ctx->split_a;  // chunks counted together take no more columns than counted alone
     }
     CU(cudaSetDevice(ctx->cfg.device));
 
@@ -1146,34 +1193,14 @@ psl_status psl_load_chunk(psl_ctx* ctx, const void* records, uint64_t n, int32_t
     cd.n_records = (uint32_t)n;
     cd.tile0 = tile0;
     cd.pad = 0;
-    ChunkDesc* chunks = at<ChunkDesc>(ctx, ctx->L.chunks);
-    if (ctx->cfg.mode == PSL_MODE_INDEX) {
-        k_set_chunk<<<1, 1, 0, ctx->stream>>>(chunks + ctx->n_chunks, cd);  // the descriptor travels as a kernel argument
-        LAUNCHED();
-    } else {
-        ctx->pending_chunks.push_back(cd);  // ONTHEFLY reads the table only at build time: uploaded there, 128 at a time
-    }
-    if (ctx->cfg.mode == PSL_MODE_INDEX) {
-        // a8 for pass A, chunk by chunk: overlaps the transfer of the next chunk
-        DevBeam none;
-        memset(&none, 0, sizeof none);
-        psl_ctx::ChunkLaunch cl;
-        cl.span = {tile0, nt, ctx->n_cols, ctx->split_a};
-        cl.n_seg = nt < ctx->S_a ? nt : ctx->S_a;
-        Prof prof(ctx, PSL_K_COUNT);
-        count_idx_fn(ctx->grid.has_pos != 0, ctx->grid.ebin_mode != 0)<<<cl.n_seg * ctx->split_a, kThreads, ctx->sm_count_raw, ctx->stream>>>(
-            chunks, ctx->n_chunks + 1, cl.span, ctx->grid, none, ctx->d.B_lo, (1u << ctx->d.lo_bits) - 1u,
-            at<uint32_t>(ctx, ctx->L.table_a), ctx->d.cols_cap, at<SegStats>(ctx, ctx->L.sstats), ctx->count_stages, nullptr, nullptr);
-        LAUNCHED();
-        ctx->idx_launches.push_back(cl);
-        ctx->n_cols += cl.n_seg * ctx->split_a;
-    }
+    ctx->pending_chunks.push_back(cd);  // uploaded 128 at a time by the next launch that reads the chunk table
     ctx->n_records += n;
     if (host) ctx->n_host_records += n;
     ctx->n_tiles += nt;
     ctx->n_chunks += 1;
     if (n % 4) ctx->ragged = true;
     ctx->result = RES_NONE;
+    if (ctx->cfg.mode == PSL_MODE_INDEX && host) return count_pending_tiles(ctx);  // overlaps the next chunk's transfer
     return PSL_OK;
 }
 

@@ -161,12 +161,12 @@ __global__ void __launch_bounds__(kBigThreads, 1) k_scatter_otf_big(const ChunkD
                     packed[h + r] = (idx < (int)td.count && cls == C_SURVIVOR) ? key : kNone;
                 }
             }
+        }
+        {
+            uint32_t rk[kBigRounds];
+            warp_rank_claim<kBigRounds>(packed, rk, cnt + w * Bp);
 #pragma unroll
-            for (int r = 0; r < kBigRounds; ++r) {
-                uint32_t bucket = packed[r];
-                uint32_t rank = warp_rank(bucket, cnt + w * Bp);
-                packed[r] = bucket == kNone ? kNone : ((bucket << 9) | rank);
-            }
+            for (int r = 0; r < kBigRounds; ++r) packed[r] = packed[r] == kNone ? kNone : ((packed[r] << 9) | rk[r]);
         }
         __syncthreads();
         const uint32_t n_part = finish_ranks<true, kBigWarps>(cnt, B, Bp, gcur, lstart, misc, grun);

@@ -120,12 +120,12 @@ __global__ void __launch_bounds__(kThreads, 3) k_scatter_idx_a(const ChunkDesc* 
                 int cls = classify<POS, EDGES, 0>(g, bm, rec[r], s_edges, key);
                 packed[r] = (idx < (int)td.count && cls == C_SURVIVOR) ? key : kNone;
             }
+            uint32_t bk[kRounds], rk[kRounds];
 #pragma unroll
-            for (int r = 0; r < kRounds; ++r) {
-                uint32_t key = packed[r];
-                uint32_t rank = warp_rank(key == kNone ? kNone : (key & lo_mask), cnt + w * Bp);
-                packed[r] = key == kNone ? kNone : ((key << 9) | rank);
-            }
+            for (int r = 0; r < kRounds; ++r) bk[r] = packed[r] == kNone ? kNone : (packed[r] & lo_mask);
+            warp_rank_claim<kRounds>(bk, rk, cnt + w * Bp);
+#pragma unroll
+            for (int r = 0; r < kRounds; ++r) packed[r] = packed[r] == kNone ? kNone : ((packed[r] << 9) | rk[r]);
         }
         __syncthreads();
         finish_ranks<false>(cnt, B, Bp, run, nullptr, misc, grun);
@@ -281,11 +281,11 @@ __global__ void __launch_bounds__(kThreads, 4) k_scatter_idx_b(const uint4* __re
             const uint32_t idx = w * kWarpSpan + r * 32 + lane_id();
             packed[r] = idx < count ? (raw[idx * 8] >> lo_bits) : kNone;
         }
+        {
+            uint32_t rk[kRounds];
+            warp_rank_claim<kRounds>(packed, rk, cnt + w * Bp);
 #pragma unroll
-        for (int r = 0; r < kRounds; ++r) {
-            uint32_t bucket = packed[r];
-            uint32_t rank = warp_rank(bucket, cnt + w * Bp);
-            packed[r] = bucket == kNone ? kNone : ((bucket << 9) | rank);
+            for (int r = 0; r < kRounds; ++r) packed[r] = packed[r] == kNone ? kNone : ((packed[r] << 9) | rk[r]);
         }
         __syncthreads();
         finish_ranks<false>(cnt, B, Bp, run, nullptr, misc, grun);

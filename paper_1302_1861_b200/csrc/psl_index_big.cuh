@@ -36,10 +36,10 @@ __host__ __device__ inline IdxBigSmem idx_big_layout(bool keyed, uint32_t B, uin
     const uint32_t stages = keyed ? kIdxBigStagesKeyed : kIdxBigStagesRaw;
     L.ring = p;   p += stages * L.stage_bytes;
     L.cnt = p;    p += round_up(kIdxBigWarps * round_up(B, 8) * 2, 16);
-    L.gcur = p;   p += round_up(B * 4, 16);
-    L.lstart = p; p += round_up(B * 4, 16);
-    L.perm = p;   p += kIdxBigTile * 2;                   // tile-sorted slot -> record in tile
-    L.pbkt = p;   p += kIdxBigTile * 2;                   // tile-sorted slot -> bucket
+    L.gcur = p;   p += round_up(B, 8) * 4;                // Bp entries: finish_ranks_pair writes whole 16-byte groups
+    L.lstart = p; p += round_up(B, 8) * 4;
+    L.perm = p;   p += kIdxBigTile * 4;                   // tile-sorted slot -> bucket << 12 | record in tile
+    L.pbkt = p;
     L.edges = p;  p += round_up(n_edges * 4, 16);
     L.misc = p;   p += 64 * 4;
     L.desc = p;   p += stages * 16;
@@ -75,8 +75,7 @@ __global__ void __launch_bounds__(kIdxBigThreads, 1) k_scatter_idx_big(const Chu
     uint16_t* cnt = reinterpret_cast<uint16_t*>(smem + L.cnt);
     uint32_t* gcur = reinterpret_cast<uint32_t*>(smem + L.gcur);
     uint32_t* lstart = reinterpret_cast<uint32_t*>(smem + L.lstart);
-    uint16_t* perm = reinterpret_cast<uint16_t*>(smem + L.perm);
-    uint16_t* pbkt = reinterpret_cast<uint16_t*>(smem + L.pbkt);
+    uint32_t* slot = reinterpret_cast<uint32_t*>(smem + L.perm);  // tile-sorted slot -> bucket << 12 | record in tile
     float* s_edges = reinterpret_cast<float*>(smem + L.edges);
     uint32_t* misc = reinterpret_cast<uint32_t*>(smem + L.misc);
     TileDesc* s_desc = reinterpret_cast<TileDesc*>(smem + L.desc);
@@ -105,6 +104,8 @@ __global__ void __launch_bounds__(kIdxBigThreads, 1) k_scatter_idx_big(const Chu
     __syncthreads();
 
     const uint32_t n_iter = KEYED ? 1u : n_spans;
+    uint32_t* const ring = reinterpret_cast<uint32_t*>(smem + L.ring);
+    const uint32_t stage_words = L.stage_bytes / 4;
     for (uint32_t si = 0; si < n_iter; ++si) {
     uint32_t S = gridDim.x;
     if (KEYED) {
@@ -124,24 +125,38 @@ __global__ void __launch_bounds__(kIdxBigThreads, 1) k_scatter_idx_big(const Chu
     }
     if (threadIdx.x == 0)
         for (uint32_t k = 0; k < (uint32_t)kIdxBigStages && k < n; ++k) issue(k);
-    uint32_t grun[8];  // thread t keeps the running first free slot of buckets 8t..8t+7
+    uint32_t grun[8];  // the pair of threads (2g, 2g+1) keeps the running first free slot of buckets 8g..8g+7
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
-        uint32_t b = threadIdx.x * 8 + k;
+        uint32_t b = (threadIdx.x >> 1) * 8 + k;
         grun[k] = b < B ? table[(size_t)b * stride + col] : 0u;
     }
     __syncthreads();
 
     for (uint32_t base = 0; base < n; base += kIdxBigQ) {
         const uint32_t nq = min((uint32_t)kIdxBigQ, n - base);
+        // the tile's four ring stages: word offset into the ring and load-order index of the first record
+        const uint32_t s0 = (goff + base) % kIdxBigStages;
+        const uint32_t s1 = s0 + 1 < kIdxBigStages ? s0 + 1 : s0 + 1 - kIdxBigStages;
+        const uint32_t s2 = s0 + 2 < kIdxBigStages ? s0 + 2 : s0 + 2 - kIdxBigStages;
+        const uint32_t s3 = s0 + 3 < kIdxBigStages ? s0 + 3 : s0 + 3 - kIdxBigStages;
+        const uint32_t o0 = s0 * stage_words, o1 = s1 * stage_words, o2 = s2 * stage_words, o3 = s3 * stage_words;
+        uint32_t f0 = 0, f1 = 0, f2 = 0, f3 = 0;
+        if (!KEYED) {
+            f0 = s_desc[s0].first_index;
+            if (nq > 1) f1 = s_desc[s1].first_index;
+            if (nq > 2) f2 = s_desc[s2].first_index;
+            if (nq > 3) f3 = s_desc[s3].first_index;
+        }
         // stages TMA could not fill (unaligned source, ragged last tile): fetched by all threads, then the
         // stage's barrier is completed by hand so that every stage flips its phase once per use
         bool manual = false;
         for (uint32_t q = 0; q < nq; ++q) {
-            const TileDesc d = s_desc[(goff + base + q) % kIdxBigStages];
+            const uint32_t sq = q == 0 ? s0 : (q == 1 ? s1 : (q == 2 ? s2 : s3));
+            const TileDesc d = s_desc[sq];
             if (!bulk_ok(d.ptr, d.count * kRecB)) {
                 const uint32_t* src = reinterpret_cast<const uint32_t*>(d.ptr);
-                uint32_t* dst = stage_ptr(base + q);
+                uint32_t* dst = ring + sq * stage_words;
                 for (uint32_t k = threadIdx.x; k < d.count * (kRecB / 4); k += kIdxBigThreads) dst[k] = __ldg(src + k);
                 manual = true;
             }
@@ -150,27 +165,28 @@ __global__ void __launch_bounds__(kIdxBigThreads, 1) k_scatter_idx_big(const Chu
             __syncthreads();
             if (threadIdx.x == 0)
                 for (uint32_t q = 0; q < nq; ++q) {
-                    const TileDesc d = s_desc[(goff + base + q) % kIdxBigStages];
-                    if (!bulk_ok(d.ptr, d.count * kRecB)) mbar_arrive(&bars[(goff + base + q) % kIdxBigStages]);
+                    const uint32_t sq = q == 0 ? s0 : (q == 1 ? s1 : (q == 2 ? s2 : s3));
+                    const TileDesc d = s_desc[sq];
+                    if (!bulk_ok(d.ptr, d.count * kRecB)) mbar_arrive(&bars[sq]);
                 }
         }
 
-        // buckets and stable ranks inside the warp's 512 records (half of ring stage base + w / 2)
-        uint32_t packed[kIdxBigRounds];
+        // buckets and stable ranks inside the warp's 256 records (a quarter of ring stage base + w / 4)
+        uint32_t bkt[kIdxBigRounds], rnk[kIdxBigRounds];
 #pragma unroll
-        for (int r = 0; r < kIdxBigRounds; ++r) packed[r] = kNone;
+        for (int r = 0; r < kIdxBigRounds; ++r) bkt[r] = kNone;
         const uint32_t q = w / (kIdxBigWarps / kIdxBigQ);
         if (q < nq) {
-            const uint32_t i = base + q;
-            const TileDesc td = s_desc[(goff + i) % kIdxBigStages];
-            mbar_wait(&bars[(goff + i) % kIdxBigStages], ((goff + i) / kIdxBigStages) & 1u);
-            uint32_t* raw = stage_ptr(i);
+            const uint32_t sq = q == 0 ? s0 : (q == 1 ? s1 : (q == 2 ? s2 : s3));
+            const uint32_t count = s_desc[sq].count;
+            mbar_wait(&bars[sq], ((goff + base + q) / kIdxBigStages) & 1u);
+            uint32_t* raw = ring + sq * stage_words;
             const uint32_t first = (w % (kIdxBigWarps / kIdxBigQ)) * kIdxBigSpan;
             if (KEYED) {
 #pragma unroll
                 for (int r = 0; r < kIdxBigRounds; ++r) {
                     const uint32_t idx = first + r * 32 + lane_id();
-                    packed[r] = idx < td.count ? (raw[idx * 8] >> lo_bits) : kNone;
+                    bkt[r] = idx < count ? (raw[idx * 8] >> lo_bits) : kNone;
                 }
             } else {
 #pragma unroll
@@ -179,63 +195,59 @@ __global__ void __launch_bounds__(kIdxBigThreads, 1) k_scatter_idx_big(const Chu
 #pragma unroll
                     for (int r = 0; r < 4; ++r) {
                         const uint32_t idx = first + (h + r) * 32 + lane_id();
-                        rec[r] = rec_from_smem(raw, idx < td.count ? (int)idx : 0);
+                        rec[r] = rec_from_smem(raw, idx < count ? (int)idx : 0);
                     }
 #pragma unroll
                     for (int r = 0; r < 4; ++r) {
                         const uint32_t idx = first + (h + r) * 32 + lane_id();
                         uint32_t key;
                         const int cls = classify<POS, EDGES, 0>(g, bm, rec[r], s_edges, key);
-                        const bool keep = idx < td.count && cls == C_SURVIVOR;
+                        const bool keep = idx < count && cls == C_SURVIVOR;
                         // the key takes the place of the type word of the staged record (the type is part of the key)
-                        if (idx < td.count) raw[idx * kRecWords] = keep ? key : kNone;
-                        packed[h + r] = keep ? (key & lo_mask) : kNone;
+                        if (idx < count) raw[idx * kRecWords] = keep ? key : kNone;
+                        bkt[h + r] = keep ? (key & lo_mask) : kNone;
                     }
                 }
             }
-#pragma unroll
-            for (int r = 0; r < kIdxBigRounds; ++r) {
-                const uint32_t bucket = packed[r];
-                const uint32_t rank = warp_rank(bucket, cnt + w * Bp);
-                packed[r] = bucket == kNone ? kNone : ((bucket << 10) | rank);  // rank < 256
-            }
         }
+        warp_rank_claim<kIdxBigRounds>(bkt, rnk, cnt + w * Bp);
         __syncthreads();
-        const uint32_t n_part = finish_ranks<true, kIdxBigWarps>(cnt, B, Bp, gcur, lstart, misc, grun);
+        const uint32_t n_part = finish_ranks_pair(cnt, Bp, gcur, lstart, misc, grun);
 
         // tile-sorted order
 #pragma unroll
         for (int r = 0; r < kIdxBigRounds; ++r) {
-            if (packed[r] != kNone) {
-                const uint32_t bucket = packed[r] >> 10, rank = packed[r] & 1023u;
-                const uint32_t p = lstart[bucket] + cnt[w * Bp + bucket] + rank;
-                perm[p] = (uint16_t)(w * kIdxBigSpan + r * 32 + lane_id());
-                pbkt[p] = (uint16_t)bucket;
+            if (bkt[r] != kNone) {
+                const uint32_t p = lstart[bkt[r]] + cnt[w * Bp + bkt[r]] + rnk[r];
+                slot[p] = (bkt[r] << 12) | (w * kIdxBigSpan + r * 32 + lane_id());  // bucket | record in tile
             }
         }
         __syncwarp();
         zero_row(cnt + w * Bp, Bp);
         __syncthreads();
-
-        // write-out: consecutive threads write consecutive 16-byte halves of consecutive tile-sorted slots, so a
-        // run of records of one bucket leaves as one request per 128-byte line
-        for (uint32_t m = threadIdx.x; m < 2 * n_part; m += kIdxBigThreads) {
-            const uint32_t j = m >> 1, half = m & 1u;
-            const uint32_t bucket = pbkt[j];
+        // write-out: thread j takes tile-sorted slots j, j + 512, ...: one 32-byte store request per record, so a run
+        // of records of one bucket leaves as one request per 128-byte line
+#pragma unroll 2
+        for (uint32_t j = threadIdx.x; j < n_part; j += kIdxBigThreads) {
+            const uint32_t sv = slot[j];
+            const uint32_t bucket = sv >> 12, irec = sv & 4095u;
             const uint32_t dest = gcur[bucket] + (j - lstart[bucket]);
-            const uint32_t irec = perm[j];
-            const uint32_t i = base + irec / kTile, ir = irec % kTile;
-            uint4 v;
+            const uint32_t qq = irec / kTile, ir = irec % kTile;
+            const uint32_t off = qq == 0 ? o0 : (qq == 1 ? o1 : (qq == 2 ? o2 : o3));
+            uint4 a, b;
             if (KEYED) {
-                v = reinterpret_cast<const uint4*>(stage_ptr(i))[2 * ir + half];
+                const uint4* p = reinterpret_cast<const uint4*>(ring + off) + 2 * ir;
+                a = p[0];
+                b = p[1];
             } else {
-                const uint32_t* p = stage_ptr(i) + ir * kRecWords;
-                if (half == 0) v = make_uint4(p[0], p[1], p[2], p[3]);
-                else v = make_uint4(p[4], p[5], p[6], s_desc[(goff + i) % kIdxBigStages].first_index + ir);
+                const uint32_t* p = ring + off + ir * kRecWords;
+                const uint32_t fi = qq == 0 ? f0 : (qq == 1 ? f1 : (qq == 2 ? f2 : f3));
+                a = make_uint4(p[0], p[1], p[2], p[3]);
+                b = make_uint4(p[4], p[5], p[6], fi + ir);
             }
-            aos_out[2 * (size_t)dest + half] = v;
+            stg_record(aos_out + 2 * (size_t)dest, a, b);
         }
-        __syncthreads();  // the tile's stages, perm and pbkt are free again
+        __syncthreads();  // the tile's stages and the slot list are free again
         if (threadIdx.x == 0)
             for (uint32_t k = 0; k < nq; ++k)
                 if (base + kIdxBigStages + k < n) issue(base + kIdxBigStages + k);
