@@ -50,7 +50,18 @@ class _Beam(C.Structure):
         ("has_roi", C.c_int32),
         ("roi_x1", C.c_float), ("roi_x2", C.c_float), ("roi_y1", C.c_float), ("roi_y2", C.c_float),
         ("mu_weight", C.c_float),
+        ("gantry_deg", C.c_float), ("coll_deg", C.c_float), ("couch_deg", C.c_float),
     ]
+
+
+class _Plan(C.Structure):
+    _fields_ = [("n_simulate", C.c_uint64), ("seed", C.c_uint64), ("rr_group", C.c_uint32), ("apr", C.c_uint32),
+                ("phantom_lo", C.c_float * 3), ("phantom_hi", C.c_float * 3)]
+
+
+class _EmitStats(C.Structure):
+    _fields_ = [(n, C.c_uint64) for n in ("n_list", "n_jaw_rejected", "n_zero_weight", "n_missed", "n_launched")] + \
+               [("sum_wt", C.c_double)]
 
 
 class _Stats(C.Structure):
@@ -95,6 +106,15 @@ def _load():
         lib.orc_w.argtypes = [C.c_float, C.c_float]
         lib.orc_fluence_at.restype = C.c_float
         lib.orc_fluence_at.argtypes = [C.c_void_p, C.c_float, C.c_float]
+        lib.orc_mix64.restype = C.c_uint64
+        lib.orc_mix64.argtypes = [C.c_uint64]
+        lib.orc_rng32.restype = C.c_uint32
+        lib.orc_rng32.argtypes = [C.c_uint64, C.c_uint64, C.c_uint64]
+        lib.orc_plan_total.restype = C.c_uint64
+        lib.orc_sample_batch.restype = C.c_uint64
+        lib.orc_emit.restype = C.c_uint64
+        lib.orc_flush_schedule.restype = C.c_uint64
+        lib.orc_surface.restype = C.c_int
         lib.orc_record_bytes.restype = C.c_uint32
         assert lib.orc_record_bytes() == 28
         _lib = lib
@@ -142,7 +162,7 @@ class Oracle:
             None if fl is None else fl.ctypes.data, nx, ny,
             b.get("map_x0", 0.0), b.get("map_y0", 0.0), b.get("map_dx", 1.0), b.get("map_dy", 1.0),
             0 if r is None else 1, *(r if r is not None else (0, 0, 0, 0)),
-            b.get("mu_weight", 1.0),
+            b.get("mu_weight", 1.0), b.get("gantry_deg", 0.0), b.get("coll_deg", 0.0), b.get("couch_deg", 0.0),
         )
 
     @staticmethod
@@ -241,3 +261,104 @@ class Oracle:
         if want_classes:
             out.update(classes=cls[:n], keys=keys[:n])
         return out
+
+    # -- sampling layer, field transform, APR, capacity-N emission ------------------
+    def _beams(self, beams):
+        arr = (_Beam * len(beams))(*[self.beam(b) for b in beams])
+        return arr
+
+    @staticmethod
+    def plan(n_simulate: int, seed: int = 1, rr_group: int = 4, phantom=((-15.0, -15.0, -15.0), (15.0, 15.0, 15.0))):
+        p = _Plan(n_simulate, seed, rr_group, 0)
+        p.phantom_lo[:] = phantom[0]
+        p.phantom_hi[:] = phantom[1]
+        return p
+
+    def mix64(self, z: int) -> int:
+        return int(self.lib.orc_mix64(C.c_uint64(z & (2 ** 64 - 1))))
+
+    def rng32(self, seed: int, a: int, b: int) -> int:
+        return int(self.lib.orc_rng32(C.c_uint64(seed), C.c_uint64(a), C.c_uint64(b)))
+
+    def plan_total(self, beams, counts: np.ndarray) -> int:
+        counts = np.ascontiguousarray(counts, dtype=np.uint32)
+        return int(self.lib.orc_plan_total(C.byref(self.cfg), self._beams(beams), C.c_uint32(len(beams)), _ptr(counts)))
+
+    def plan_budgets(self, beams, counts: np.ndarray, n_simulate: int):
+        """(budget[K], mask[K]): particles to simulate from PSL k for each field that selects it; the fields"""
+        counts = np.ascontiguousarray(counts, dtype=np.uint32)
+        budget = np.empty(self.n_keys, np.uint32)
+        mask = np.empty(self.n_keys, np.uint32)
+        self.lib.orc_plan_budgets(C.byref(self.cfg), self._beams(beams), C.c_uint32(len(beams)), _ptr(counts),
+                                  C.c_uint64(n_simulate), _ptr(budget), _ptr(mask))
+        return budget, mask
+
+    def sample_batch(self, beams, counts, offsets, plan, t: int, ie: int, cap: int):
+        counts = np.ascontiguousarray(counts, dtype=np.uint32)
+        offsets = np.ascontiguousarray(offsets, dtype=np.uint32)
+        slot = np.empty(max(cap, 1), np.uint32)
+        beam = np.empty(max(cap, 1), np.uint8)
+        n = int(self.lib.orc_sample_batch(C.byref(self.cfg), self._beams(beams), C.c_uint32(len(beams)), _ptr(counts),
+                                          _ptr(offsets), C.byref(plan), C.c_int32(t), C.c_int32(ie), _ptr(slot),
+                                          _ptr(beam), C.c_uint64(cap)))
+        assert n <= cap, "launch list longer than the capacity given"
+        return slot[:n], beam[:n]
+
+    def emit(self, beams, plan, index: Dict, slot: np.ndarray, beam_id: np.ndarray) -> Dict:
+        """index: the bare index (build(records, None)); slot / beam_id: a launch list"""
+        n = len(slot)
+        slot = np.ascontiguousarray(slot, np.uint32)
+        beam_id = np.ascontiguousarray(beam_id, np.uint8)
+        f = {k: np.empty(max(n, 1), np.float32) for k in ("E", "X", "Y", "Z", "U", "V", "W", "wt")}
+        src = np.empty(max(n, 1), np.uint32)
+        ob = np.empty(max(n, 1), np.uint8)
+        st = _EmitStats()
+        m = int(self.lib.orc_emit(
+            C.byref(self.cfg), self._beams(beams), C.c_uint32(len(beams)), C.byref(plan),
+            *[_ptr(np.ascontiguousarray(index[k])) for k in ("E", "x", "y", "u", "v", "wt")],
+            _ptr(np.ascontiguousarray(index["src_index"])), _ptr(slot), _ptr(beam_id), C.c_uint64(n),
+            *[_ptr(f[k]) for k in ("E", "X", "Y", "Z", "U", "V", "W", "wt")], _ptr(src), _ptr(ob), C.byref(st)))
+        out = {k: v[:m] for k, v in f.items()}
+        out.update(src_index=src[:m], beam=ob[:m], n_launched=m,
+                   stats={name: getattr(st, name) for name, _ in _EmitStats._fields_})
+        return out
+
+    def beam_matrix(self, beam: Dict) -> np.ndarray:
+        b = self.beam(beam)
+        m = (C.c_float * 9)()
+        self.lib.orc_beam_matrix(C.byref(b), m)
+        return np.array(m, dtype=np.float32).reshape(3, 3)
+
+    def rotate(self, M: np.ndarray, v) -> np.ndarray:
+        m = (C.c_float * 9)(*np.asarray(M, np.float32).reshape(-1))
+        a = (C.c_float * 3)(*v)
+        o = (C.c_float * 3)()
+        self.lib.orc_rotate(m, a, o)
+        return np.array(o, dtype=np.float32)
+
+    def surface(self, P, D, lo, hi):
+        a, d, l, h, o = [(C.c_float * 3)(*v) for v in (P, D, lo, hi, (0, 0, 0))]
+        hit = int(self.lib.orc_surface(a, d, l, h, o))
+        return hit, np.array(o, dtype=np.float32)
+
+    def apr_cos_sin(self, r: int):
+        c, s_ = C.c_float(), C.c_float()
+        self.lib.orc_apr_cos_sin(C.c_uint32(r), C.byref(c), C.byref(s_))
+        return c.value, s_.value
+
+    def apr(self, seed: int, records: np.ndarray, first_index: int = 0) -> np.ndarray:
+        rec = self._rec(records)
+        out = np.empty_like(rec)
+        self.lib.orc_apr_all(C.c_uint64(seed), C.c_uint64(first_index), _ptr(rec), C.c_uint64(len(rec)), _ptr(out))
+        return out
+
+    def flush_schedule(self, build: Dict, capacity: int):
+        """events (key, first slot, count) of the capacity-N emission for a build made with want_classes=True"""
+        n = len(build["classes"])
+        cap = n // max(capacity, 1) + self.n_keys + 1
+        ek, ef, ec = (np.empty(cap, np.uint32) for _ in range(3))
+        ne = int(self.lib.orc_flush_schedule(C.c_uint32(self.n_keys), C.c_uint64(n), _ptr(np.ascontiguousarray(build["classes"])),
+                                             _ptr(np.ascontiguousarray(build["keys"])),
+                                             _ptr(np.ascontiguousarray(build["offsets"])), C.c_uint32(capacity), _ptr(ek),
+                                             _ptr(ef), _ptr(ec), C.c_uint64(cap)))
+        return ek[:ne], ef[:ne], ec[:ne]

@@ -164,7 +164,7 @@ __global__ void __launch_bounds__(kBigThreads, 1) k_scatter_otf_big(const ChunkD
         }
         {
             uint32_t rk[kBigRounds];
-            warp_rank_claim<kBigRounds>(packed, rk, cnt + w * Bp);
+            warp_rank_match<kBigRounds>(packed, rk, cnt + w * Bp);
 #pragma unroll
             for (int r = 0; r < kBigRounds; ++r) packed[r] = packed[r] == kNone ? kNone : ((packed[r] << 9) | rk[r]);
         }

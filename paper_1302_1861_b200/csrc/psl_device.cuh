@@ -395,6 +395,29 @@ __device__ __forceinline__ void warp_rank_claim(const uint32_t (&bucket)[R], uin
     }
 }
 
+// The same contract with MATCH.ANY: for the ONTHEFLY kernels.  Their <= 2048 (type, energy) keys follow the energy
+// spectrum, a round of 32 records holds ~20 colliding pairs, and MATCH.ANY's cost falls with the number of distinct
+// values while the claim loop's grows with the number of collisions (measured at config 2: scatter 0.203 ms with
+// MATCH.ANY, 0.222 ms with claims).  Counters are plain counts here (no claim bits).
+template <int R>
+__device__ __forceinline__ void warp_rank_match(const uint32_t (&bucket)[R], uint32_t (&rank)[R], uint16_t* cnt)
+{
+    uint32_t peers[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) peers[r] = __match_any_sync(0xFFFFFFFFu, bucket[r]);
+    const uint32_t lt = lanemask_lt();
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const bool act = bucket[r] != kNone;
+        const uint32_t before = __popc(peers[r] & lt);
+        const uint32_t base = act ? cnt[bucket[r]] : 0u;  // every peer reads the same word
+        __syncwarp();
+        if (act && before == 0u) cnt[bucket[r]] = (uint16_t)(base + __popc(peers[r]));
+        __syncwarp();
+        rank[r] = base + before;
+    }
+}
+
 // one 32-byte record in ONE store request (STG.E.256, sm_100+); dst must be 32-byte aligned
 __device__ __forceinline__ void stg_record(uint4* dst, const uint4& a, const uint4& b)
 {

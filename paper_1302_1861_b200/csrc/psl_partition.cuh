@@ -944,7 +944,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_scatter_otf(const ChunkDesc* __
         }
         {
             uint32_t rk[kRounds];
-            warp_rank_claim<kRounds>(packed, rk, cnt + w * Bp);  // ranks: round r before round r + 1
+            warp_rank_match<kRounds>(packed, rk, cnt + w * Bp);  // ranks: round r before round r + 1
 #pragma unroll
             for (int r = 0; r < kRounds; ++r) packed[r] = packed[r] == kNone ? kNone : ((packed[r] << 9) | rk[r]);
         }
