@@ -50,7 +50,10 @@ enum { PSL_EBIN_LINEAR = 0,   /* n_ebins uniform bins on [e_min, e_max] (PAPER.m
 enum { PSL_MEM_PAGEABLE = 0, PSL_MEM_PINNED = 1, PSL_MEM_DEVICE = 2 };
 enum { PSL_OUT_PROJ = 1u,           /* also write xp, yp: the position at the fluence-map plane */
        PSL_DROP_ZERO_WEIGHT = 2u,   /* drop survivors whose final weight is exactly 0 (default: keep) */
-       PSL_NO_COMPACT = 4u };       /* diagnostic, same results: ONTHEFLY with <= 256 keys and a rejecting beam takes the
+       PSL_NO_COMPACT = 4u,
+       PSL_APR = 8u };              /* INDEX mode: azimuthal particle redistribution of every record
+                                       before it is binned: record i of the load order turns about the beam axis by
+                                       2 pi r / 2^32, r from psl_config.apr_seed and i; position and direction together */       /* diagnostic, same results: ONTHEFLY with <= 256 keys and a rejecting beam takes the
                                        two-pass path (histogram, then scatter over all records) instead of compacting
                                        the survivors in the histogram pass; used for A/B runs and tests */
 
@@ -81,7 +84,10 @@ typedef struct {
     uint64_t max_host_records; /* of those, how many may arrive from HOST memory (device landing zone) */
     uint64_t max_beam_records; /* INDEX mode: most records one beam's ROI may select; 0 = max_records */
     uint32_t max_chunks;       /* most psl_load_chunk calls between resets; 0 = 4096 */
-    uint32_t flags;            /* PSL_OUT_PROJ | PSL_DROP_ZERO_WEIGHT | PSL_NO_COMPACT */
+    uint32_t flags;            /* PSL_OUT_PROJ | PSL_DROP_ZERO_WEIGHT | PSL_NO_COMPACT | PSL_APR */
+    uint64_t apr_seed;         /* PSL_APR: seed of the redistribution angles */
+    uint64_t max_launch_records; /* INDEX mode: longest launch list psl_sample_batch may build (0 = sampling layer unused);
+                                    ONTHEFLY mode: most bin shipments psl_flush_schedule may report (0 = unused) */
     int32_t device;            /* CUDA device ordinal */
     void* stream;              /* cudaStream_t owned by the caller (NULL = default stream) */
     void* workspace;           /* DEVICE memory owned by the caller, 256-byte aligned */
@@ -183,6 +189,63 @@ psl_status psl_roi_from_jaws(const psl_geometry* g, const psl_beam* beam, float 
 /* HOST only.  The inclusive rectangle {rx0, rx1, ry0, ry1} of position bins with positive-area overlap with
  * the beam's ROI ("any portion of its area"); rx0 > rx1 or ry0 > ry1 when nothing is selected. */
 psl_status psl_roi_bins(const psl_ctx* ctx, const psl_beam* beam, int32_t bins_out[4]);
+
+/* ---- From the index to transport launches (sec. 2.3.3) -------------------
+ * A plan = the fields of a treatment plan + how many particles to simulate.  psl_plan_set gives every selected PSL its
+ * share; psl_sample_batch then builds, for one (type, energy) division, the launch list (which index particle, for
+ * which field, in the order the paper's reading loop visits them) and turns it into transport-ready particles. */
+typedef struct {
+    uint32_t struct_size;  /* sizeof(psl_plan), checked */
+    uint32_t n_beams;      /* 1..32 */
+    const psl_beam* beams; /* HOST array of n_beams fields (their fluence maps DEVICE); copied by psl_plan_set */
+    uint64_t n_simulate;   /* N_total^simulated: particles to simulate over all fields */
+    uint64_t seed;         /* of the random starts and field assignments; give every GPU of a job its own */
+    uint32_t rr_group;     /* particles read from a PSL at a time ("a few"); >= 1 */
+    uint32_t reserved;     /* 0 */
+    float phantom_lo[3], phantom_hi[3]; /* the patient phantom: an axis-aligned box in the patient frame, cm, origin at
+                                           the isocentre.  Patient frame: p = Rz(-couch) Ry(gantry) Rz(collimator) p_b with
+                                           p_b = (x, y, z_iso - z_plane), direction (u, v, -w) (reading S5) */
+} psl_plan;
+
+/* Budgets: N_total^psl = sum over fields of the particles in the PSLs each selects; every selected PSL k
+ * gives floor(n_simulate * counts[k] / N_total^psl) particles to EACH field that selects it.  Needs a finalised index
+ * (psl_build_batches once).  Synchronises.  *n_total_psl and *list_len (HOST, n_types * n_ebins entries owned by the
+ * context, valid until the next psl_plan_set / psl_reset: the launch-list length of every division) may be NULL. */
+psl_status psl_plan_set(psl_ctx* ctx, const psl_plan* plan, uint64_t* n_total_psl, const uint64_t** list_len);
+
+/* DEVICE pointers to budget[K] and field mask[K] (bit i: field i selects the PSL) of the current plan. */
+psl_status psl_plan_tables(psl_ctx* ctx, const uint32_t** budget, const uint32_t** mask);
+
+/* The launch of one division.  All pointers DEVICE, BORROWED, valid until the next psl_sample_batch / psl_plan_set /
+ * psl_reset / psl_destroy. */
+typedef struct {
+    uint32_t n_list;   /* entries of the launch list */
+    uint32_t n_launch; /* of those: passed their field's jaws (and PSL_DROP_ZERO_WEIGHT) and reach the phantom */
+    const uint32_t* slot;  /* n_list: position of the particle in the index (psl_build_batches(NULL) order) */
+    const uint8_t* beam;   /* n_list: the field it was assigned to */
+    const float *E, *X, *Y, *Z, *U, *V, *W, *wt; /* n_launch, in list order: energy, entry point on the phantom surface and
+                                                    direction in the patient frame, weight (wt * F) * mu of its field */
+    const uint32_t* src_index; /* n_launch: load-order index of the record */
+    const uint8_t* beam_of;    /* n_launch: field */
+    uint64_t n_jaw_rejected, n_zero_weight, n_missed; /* list entries dropped, by reason (tested in this order) */
+} psl_launch;
+
+/* Round-robin over the division's selected PSLs in spatial order, rr_group reads from each per round until its share
+ * (budget x fields that selected it) is used up; a PSL's first read starts at a random particle and wraps around; every
+ * read goes to one of the PSL's fields at random.  Then per entry: jaw test of its field
+ * (PAPER.md:55), fluence-map and MU weight, rotations and projection to the phantom surface
+ * (PAPER.md:105).  PSL_ERR_CAPACITY if the list is longer than max_launch_records.  Synchronises. */
+psl_status psl_sample_batch(psl_ctx* ctx, int32_t t, int32_t ie, psl_launch* out);
+
+/* ---- Bins of capacity N (methods 1 and 2) ---------------------------------------------------------------
+ * The shipments of the latest ONTHEFLY build had its bins been sent to the transport engine whenever one held
+ * `capacity` particles: shipment e = `count[e]` particles of key `key[e]`, output slots [first[e], first[e] + count[e]),
+ * in the order the bins fill up as the records arrive; the partially filled bins go last, in key order. */
+typedef struct {
+    uint32_t n_events;
+    const uint32_t *key, *first, *count; /* DEVICE, BORROWED until the next build / psl_reset */
+} psl_flush;
+psl_status psl_flush_schedule(psl_ctx* ctx, uint32_t capacity, psl_flush* out);
 
 /* Forget all chunks and results (keeps the configuration and workspace).  Blocks the HOST until every HOST chunk
  * loaded so far has left its source buffer (as psl_wait_loads); work already enqueued on the stream is not waited for. */

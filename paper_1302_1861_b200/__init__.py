@@ -7,12 +7,12 @@ built library or without a CUDA device raises.
 """
 from .binding import (  # noqa: F401
     EBIN_EDGES, EBIN_LINEAR, MEM_DEVICE, MEM_PAGEABLE, MEM_PINNED, MODE_INDEX, MODE_ONTHEFLY, OUT_PROJ,
-    DROP_ZERO_WEIGHT, NO_COMPACT, PslContext, PslError, exported_symbols, library_path, load_library, psl_roi_from_jaws,
+    DROP_ZERO_WEIGHT, NO_COMPACT, APR, PslContext, PslError, exported_symbols, library_path, load_library, psl_roi_from_jaws,
     workspace_bytes,
 )
 
 __all__ = [
     "PslContext", "PslError", "load_library", "library_path", "exported_symbols", "workspace_bytes",
     "psl_roi_from_jaws", "MODE_ONTHEFLY", "MODE_INDEX", "EBIN_LINEAR", "EBIN_EDGES", "MEM_PAGEABLE", "MEM_PINNED",
-    "MEM_DEVICE", "OUT_PROJ", "DROP_ZERO_WEIGHT", "NO_COMPACT",
+    "MEM_DEVICE", "OUT_PROJ", "DROP_ZERO_WEIGHT", "NO_COMPACT", "APR",
 ]

@@ -19,7 +19,7 @@ from . import _build
 MODE_ONTHEFLY, MODE_INDEX = 0, 1
 EBIN_LINEAR, EBIN_EDGES = 0, 1
 MEM_PAGEABLE, MEM_PINNED, MEM_DEVICE = 0, 1, 2
-OUT_PROJ, DROP_ZERO_WEIGHT, NO_COMPACT = 1, 2, 4
+OUT_PROJ, DROP_ZERO_WEIGHT, NO_COMPACT, APR = 1, 2, 4, 8
 RECORD_BYTES = 28
 
 _STATUS = {0: "PSL_OK", 1: "PSL_ERR_ARG", 2: "PSL_ERR_STATE", 3: "PSL_ERR_CAPACITY", 4: "PSL_ERR_GEOMETRY",
@@ -46,6 +46,7 @@ class Config(C.Structure):
         ("geom", Geometry),
         ("max_records", C.c_uint64), ("max_host_records", C.c_uint64), ("max_beam_records", C.c_uint64),
         ("max_chunks", C.c_uint32), ("flags", C.c_uint32),
+        ("apr_seed", C.c_uint64), ("max_launch_records", C.c_uint64),
         ("device", C.c_int32), ("stream", C.c_void_p), ("workspace", C.c_void_p), ("workspace_bytes", C.c_uint64),
     ]
 
@@ -75,6 +76,22 @@ class Batch(C.Structure):
     _fields_ = [("first", C.c_uint32), ("count", C.c_uint32)] + \
                [(n, C.c_void_p) for n in ("E", "x", "y", "u", "v", "w", "wt", "xp", "yp", "src_index", "bin_offsets")] + \
                [("n_bins", C.c_uint32)]
+
+
+class Plan(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("n_beams", C.c_uint32), ("beams", C.c_void_p), ("n_simulate", C.c_uint64),
+                ("seed", C.c_uint64), ("rr_group", C.c_uint32), ("reserved", C.c_uint32),
+                ("phantom_lo", C.c_float * 3), ("phantom_hi", C.c_float * 3)]
+
+
+class Launch(C.Structure):
+    _fields_ = [("n_list", C.c_uint32), ("n_launch", C.c_uint32), ("slot", C.c_void_p), ("beam", C.c_void_p)] + \
+               [(n, C.c_void_p) for n in ("E", "X", "Y", "Z", "U", "V", "W", "wt", "src_index", "beam_of")] + \
+               [(n, C.c_uint64) for n in ("n_jaw_rejected", "n_zero_weight", "n_missed")]
+
+
+class Flush(C.Structure):
+    _fields_ = [("n_events", C.c_uint32), ("key", C.c_void_p), ("first", C.c_void_p), ("count", C.c_void_p)]
 
 
 K_CLASSES = ("count", "scan", "scatter", "index_a", "index_b", "beam", "other", "count_keys", "sample")
@@ -130,6 +147,14 @@ def load_library(build: bool = True):
     lib.psl_roi_from_jaws.argtypes = [P(Geometry), P(Beam), C.c_float, P(C.c_float * 4)]
     lib.psl_roi_bins.restype = C.c_int
     lib.psl_roi_bins.argtypes = [C.c_void_p, P(Beam), P(C.c_int32 * 4)]
+    lib.psl_plan_set.restype = C.c_int
+    lib.psl_plan_set.argtypes = [C.c_void_p, P(Plan), P(C.c_uint64), P(P(C.c_uint64))]
+    lib.psl_plan_tables.restype = C.c_int
+    lib.psl_plan_tables.argtypes = [C.c_void_p, P(C.c_void_p), P(C.c_void_p)]
+    lib.psl_sample_batch.restype = C.c_int
+    lib.psl_sample_batch.argtypes = [C.c_void_p, C.c_int32, C.c_int32, P(Launch)]
+    lib.psl_flush_schedule.restype = C.c_int
+    lib.psl_flush_schedule.argtypes = [C.c_void_p, C.c_uint32, P(Flush)]
     lib.psl_reset.restype = C.c_int
     lib.psl_reset.argtypes = [C.c_void_p]
     lib.psl_destroy.restype = None
@@ -151,7 +176,8 @@ def _geometry(g: Dict) -> Geometry:
 
 
 def make_config(grid: Dict, geometry: Dict, mode: int, max_records: int, max_host_records: Optional[int] = None,
-                max_beam_records: int = 0, max_chunks: int = 0, flags: int = 0, device: int = 0):
+                max_beam_records: int = 0, max_chunks: int = 0, flags: int = 0, device: int = 0,
+                max_launch_records: int = 0, apr_seed: int = 0):
     """(Config, keepalive) for a workloads-style grid / geometry description."""
     edges = None
     if grid["ebin_mode"] == EBIN_EDGES:
@@ -172,6 +198,8 @@ def make_config(grid: Dict, geometry: Dict, mode: int, max_records: int, max_hos
     cfg.max_beam_records = max_beam_records
     cfg.max_chunks = max_chunks
     cfg.flags = flags
+    cfg.apr_seed = apr_seed
+    cfg.max_launch_records = max_launch_records
     cfg.device = device
     return cfg, edges
 
@@ -199,7 +227,7 @@ class PslContext:
 
     def __init__(self, grid: Dict, geometry: Dict, mode: int, max_records: int,
                  max_host_records: Optional[int] = None, max_beam_records: int = 0, max_chunks: int = 0,
-                 flags: int = 0, device: int = 0, stream=None):
+                 flags: int = 0, device: int = 0, stream=None, max_launch_records: int = 0, apr_seed: int = 0):
         import torch
 
         self.torch = torch
@@ -208,7 +236,7 @@ class PslContext:
             raise PslError(5, "no CUDA device: libpsl_b200 has no CPU path")
         self.device = torch.device("cuda", device)
         self.cfg, self._edges = make_config(grid, geometry, mode, max_records, max_host_records, max_beam_records,
-                                            max_chunks, flags, device)
+                                            max_chunks, flags, device, max_launch_records, apr_seed)
         need = int(self.lib.psl_workspace_bytes(C.byref(self.cfg)))
         if need == 0:
             raise PslError(1, self.lib.psl_last_error(None).decode())
@@ -238,9 +266,10 @@ class PslContext:
         """zero-copy tensor over a borrowed workspace pointer"""
         if not ptr:
             return None
+        size = 1 if dtype == self.torch.uint8 else 4
         off = ptr - self.workspace.data_ptr()
-        assert 0 <= off and off + 4 * count <= self.workspace.numel()
-        return self.workspace[off:off + 4 * count].view(dtype)
+        assert 0 <= off and off + size * count <= self.workspace.numel()
+        return self.workspace[off:off + size * count].view(dtype)
 
     def beam(self, b: Optional[Dict]) -> Optional[Beam]:
         """marshal a workloads-style beam dict; uploads the fluence map to the device"""
@@ -336,6 +365,50 @@ class PslContext:
         out = (C.c_int32 * 4)()
         self._check(self.lib.psl_roi_bins(self._h, C.byref(b), C.byref(out)))
         return tuple(int(v) for v in out)
+
+    # -- plan -> launch lists -> transport-ready particles; capacity-N shipments -----------------
+    def plan_set(self, beams, n_simulate: int, seed: int = 1, rr_group: int = 4,
+                 phantom=((-15.0, -15.0, -15.0), (15.0, 15.0, 15.0))):
+        """returns (N_total^psl, [launch-list length of every (type, energy) division])"""
+        arr = (Beam * len(beams))(*[b if isinstance(b, Beam) else self.beam(b) for b in beams])
+        p = Plan()
+        p.struct_size = C.sizeof(Plan)
+        p.n_beams = len(beams)
+        p.beams = C.cast(arr, C.c_void_p)
+        p.n_simulate, p.seed, p.rr_group = n_simulate, seed, rr_group
+        p.phantom_lo[:] = phantom[0]
+        p.phantom_hi[:] = phantom[1]
+        total = C.c_uint64()
+        lens = C.POINTER(C.c_uint64)()
+        self._check(self.lib.psl_plan_set(self._h, C.byref(p), C.byref(total), C.byref(lens)))
+        nb = self.n_types * self.n_ebins
+        return int(total.value), [int(lens[i]) for i in range(nb)]
+
+    def plan_tables(self):
+        b, m = C.c_void_p(), C.c_void_p()
+        self._check(self.lib.psl_plan_tables(self._h, C.byref(b), C.byref(m)))
+        return self._view(b.value, self.n_keys, self.torch.int32), self._view(m.value, self.n_keys, self.torch.int32)
+
+    def sample_batch(self, t: int, ie: int) -> Dict:
+        torch = self.torch
+        l = Launch()
+        self._check(self.lib.psl_sample_batch(self._h, t, ie, C.byref(l)))
+        out = {"n_list": l.n_list, "n_launch": l.n_launch, "n_jaw_rejected": l.n_jaw_rejected,
+               "n_zero_weight": l.n_zero_weight, "n_missed": l.n_missed}
+        out["slot"] = self._view(l.slot, l.n_list, torch.int32)
+        out["beam"] = self._view(l.beam, l.n_list, torch.uint8)
+        for name in ("E", "X", "Y", "Z", "U", "V", "W", "wt"):
+            out[name] = self._view(getattr(l, name), l.n_launch, torch.float32)
+        out["src_index"] = self._view(l.src_index, l.n_launch, torch.int32)
+        out["beam_of"] = self._view(l.beam_of, l.n_launch, torch.uint8)
+        return out
+
+    def flush_schedule(self, capacity: int) -> Dict:
+        f = Flush()
+        self._check(self.lib.psl_flush_schedule(self._h, capacity, C.byref(f)))
+        return {"n_events": f.n_events, "key": self._view(f.key, f.n_events, self.torch.int32),
+                "first": self._view(f.first, f.n_events, self.torch.int32),
+                "count": self._view(f.count, f.n_events, self.torch.int32)}
 
     def reset(self):
         self._check(self.lib.psl_reset(self._h))

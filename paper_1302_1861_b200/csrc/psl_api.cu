@@ -22,6 +22,7 @@
 #include "psl_index_big.cuh"
 #include "psl_device.cuh"
 #include "psl_partition.cuh"
+#include "psl_plan.cuh"
 
 using namespace psl;
 
@@ -44,6 +45,11 @@ struct Layout {
              idx_batch_off = 0;
     uint64_t seg = 0, beam_out[10] = {0}, beam_keys = 0, beam_offsets = 0, beam_counts = 0, lookback = 0, bstats = 0,
              beam_stats = 0;
+    // INDEX, sampling layer (max_launch_records > 0)
+    uint64_t plan_budget = 0, plan_mask = 0, plan_len = 0, plan_rounds = 0, plan_total = 0, plan_beams = 0, l_slot = 0, l_beam = 0,
+             l_out[8] = {0}, l_src = 0, l_beam_of = 0, l_state = 0, l_stats = 0;
+    // ONTHEFLY, capacity-N emission (max_launch_records > 0)
+    uint64_t f_full = 0, f_part = 0, f_totals = 0, f_trig = 0, f_tkey = 0, f_tfirst = 0, f_key = 0, f_first = 0, f_count = 0;
 };
 
 struct Derived {
@@ -111,6 +117,8 @@ psl_status derive(const psl_config* c, Derived* d, char* err)
     uint64_t K = (uint64_t)c->n_types * c->n_ebins * n_pos;
     if (c->max_records == 0 || c->max_records >= (1ull << 32)) { set_err(err, "config.max_records must be 1..2^32-1"); return PSL_ERR_ARG; }
     if (c->max_host_records > c->max_records) { set_err(err, "config.max_host_records > max_records"); return PSL_ERR_ARG; }
+    if (c->max_launch_records >= (1ull << 32)) { set_err(err, "config.max_launch_records must be < 2^32"); return PSL_ERR_ARG; }
+    if ((c->flags & PSL_APR) && c->mode != PSL_MODE_INDEX) { set_err(err, "PSL_APR needs PSL_MODE_INDEX"); return PSL_ERR_ARG; }
     d->K = (uint32_t)K;
     d->n_pos = (uint32_t)n_pos;
     d->n_batches = (uint32_t)(c->n_types * c->n_ebins);
@@ -178,6 +186,12 @@ void plan(const psl_config* c, const Derived& d, Layout* L)
         for (int i = 0; i < 10; ++i) L->out[i] = ((i == 7 || i == 8) && !proj) ? 0 : take(&cur, N * 4);
         L->offsets = take(&cur, (uint64_t)(d.K + 1) * 4);
         L->counts = take(&cur, (uint64_t)d.K * 4);
+        if (c->max_launch_records) {
+            const uint64_t E = c->max_launch_records;
+            L->f_full = take(&cur, (uint64_t)d.K * 4); L->f_part = take(&cur, (uint64_t)d.K * 4); L->f_totals = take(&cur, 8);
+            L->f_trig = take(&cur, E * 4); L->f_tkey = take(&cur, E * 4); L->f_tfirst = take(&cur, E * 4);
+            L->f_key = take(&cur, E * 4); L->f_first = take(&cur, E * 4); L->f_count = take(&cur, E * 4);
+        }
         L->codes = take(&cur, N);  // one byte per record: the histogram kernel's verdict for the scatter of a rejecting beam
         // few keys: the survivors of a rejecting beam, compacted per histogram segment (32 B each, a segment's region
         // starts at its first record, so only the survivors' share of it is ever touched)
@@ -204,6 +218,18 @@ void plan(const psl_config* c, const Derived& d, Layout* L)
         L->lookback = take(&cur, bt * 8);
         L->bstats = take(&cur, bt * sizeof(BeamTileStats));
         L->beam_stats = take(&cur, sizeof(DevBeamStats));
+        if (c->max_launch_records) {
+            const uint64_t E = c->max_launch_records;
+            L->plan_budget = take(&cur, (uint64_t)d.K * 4); L->plan_mask = take(&cur, (uint64_t)d.K * 4);
+            L->plan_len = take(&cur, (uint64_t)d.n_batches * 8); L->plan_rounds = take(&cur, (uint64_t)d.n_batches * 8);
+            L->plan_total = take(&cur, 8);
+            L->plan_beams = take(&cur, (uint64_t)kMaxPlanBeams * sizeof(PlanBeam));
+            L->l_slot = take(&cur, E * 4); L->l_beam = take(&cur, E);
+            for (int i = 0; i < 8; ++i) L->l_out[i] = take(&cur, E * 4);
+            L->l_src = take(&cur, E * 4); L->l_beam_of = take(&cur, E);
+            L->l_state = take(&cur, ((E + kEmitTile - 1) / kEmitTile + 1) * 8);
+            L->l_stats = take(&cur, sizeof(LaunchStats) + 16);  // + the tile counter
+        }
     }
     L->total = cur;
 }
@@ -318,6 +344,14 @@ struct psl_ctx {
     std::vector<ChunkLaunch> idx_launches;
     std::vector<SpanSeg> h_spans;  // INDEX: the per-chunk count launches, replayed by pass A's scatter
     std::vector<uint32_t> h_idx_batch_off;  // INDEX: batch offsets of the bare index (n_batches+1)
+    // sampling layer
+    bool plan_set = false;
+    psl_plan plan = {};
+    PlanSel plan_sel = {};
+    std::vector<PlanBeam> h_plan_beams;
+    unsigned long long* h_plan = nullptr;  // pinned: [0] N_total, [1 .. n_batches] list lengths, then the rounds
+    LaunchStats* h_launch_stats = nullptr;
+    uint32_t* h_flush_totals = nullptr;
     // state
     uint64_t n_records = 0, n_host_records = 0;
     uint32_t n_tiles = 0, n_chunks = 0, n_cols = 0;
@@ -436,6 +470,8 @@ DevGrid make_grid(const psl_config& c, const Derived& d, const float* dev_edges)
         g.inv_dy = (float)(1.0 / (double)c.dy);
     }
     g.n_pos = d.n_pos;
+    g.apr = (c.flags & PSL_APR) ? 1u : 0u;
+    g.apr_seed = c.apr_seed;
     return g;
 }
 
@@ -968,7 +1004,7 @@ void psl_destroy(psl_ctx* ctx)
     }
     for (cudaEvent_t e : ctx->event_pool) cudaEventDestroy(e);
     void* hp[] = {ctx->h_stage[0], ctx->h_stage[1], ctx->h_batch_off, ctx->h_idx_offsets, ctx->h_seg, ctx->h_stats,
-                  ctx->h_beam_stats, ctx->h_scalars};
+                  ctx->h_beam_stats, ctx->h_scalars, ctx->h_plan, ctx->h_launch_stats, ctx->h_flush_totals};
     for (void* p : hp)
         if (p) cudaFreeHost(p);
     delete ctx;
@@ -1026,6 +1062,11 @@ psl_status psl_create(const psl_config* cfg, psl_ctx** out)
     CUC(cudaMemsetAsync(at<uint8_t>(ctx, L.scalars), 0, 64, ctx->stream));
     CUC(cudaHostAlloc(&ctx->h_beam_stats, sizeof(DevBeamStats), cudaHostAllocDefault));
     CUC(cudaHostAlloc(&ctx->h_scalars, 64, cudaHostAllocDefault));
+    if (cfg->max_launch_records) {
+        CUC(cudaHostAlloc(&ctx->h_plan, (uint64_t)(2 * d.n_batches + 1) * 8, cudaHostAllocDefault));
+        CUC(cudaHostAlloc(&ctx->h_launch_stats, sizeof(LaunchStats), cudaHostAllocDefault));
+        CUC(cudaHostAlloc(&ctx->h_flush_totals, 8, cudaHostAllocDefault));
+    }
     if (cfg->mode == PSL_MODE_INDEX) {
         CUC(cudaHostAlloc(&ctx->h_idx_offsets, (uint64_t)(d.K + 1) * 4, cudaHostAllocDefault));
         CUC(cudaHostAlloc(&ctx->h_seg, (uint64_t)(3 * d.max_seg + 1) * 4, cudaHostAllocDefault));
@@ -1127,6 +1168,7 @@ psl_status psl_reset(psl_ctx* ctx)
     ctx->soa_view = false;
     ctx->result = RES_NONE;
     ctx->n_idx = ctx->last_M = 0;
+    ctx->plan_set = false;
     return PSL_OK;
 }
 
@@ -1305,6 +1347,187 @@ psl_status psl_profile_read(psl_ctx* ctx, psl_profile* out)
         ctx->event_pool.push_back(br.b);
     }
     ctx->brackets.clear();
+    return PSL_OK;
+}
+
+// patient-frame rotation of a field: Rz(-couch) Ry(gantry) Rz(collimator), formed in double, rounded once
+static void field_matrix(const psl_beam& b, float M[9])
+{
+    const double rad = 3.14159265358979323846 / 180.0;
+    const double a[3] = {(double)b.coll_deg * rad, (double)b.gantry_deg * rad, -(double)b.couch_deg * rad};
+    double R[3][9];
+    for (int i = 0; i < 3; ++i) {
+        const double c = cos(a[i]), s_ = sin(a[i]);
+        if (i == 1) { const double m[9] = {c, 0, s_, 0, 1, 0, -s_, 0, c}; memcpy(R[i], m, sizeof m); }
+        else { const double m[9] = {c, -s_, 0, s_, c, 0, 0, 0, 1}; memcpy(R[i], m, sizeof m); }
+    }
+    double GC[9], T[9];
+    for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j) {
+            GC[3 * i + j] = 0;
+            for (int k = 0; k < 3; ++k) GC[3 * i + j] += R[1][3 * i + k] * R[0][3 * k + j];
+        }
+    for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j) {
+            T[3 * i + j] = 0;
+            for (int k = 0; k < 3; ++k) T[3 * i + j] += R[2][3 * i + k] * GC[3 * k + j];
+        }
+    for (int i = 0; i < 9; ++i) M[i] = (float)T[i];
+}
+
+psl_status psl_plan_set(psl_ctx* ctx, const psl_plan* plan, uint64_t* n_total_psl, const uint64_t** list_len)
+{
+    if (!ctx || !plan) return PSL_ERR_ARG;
+    if (plan->struct_size != sizeof(psl_plan)) { set_err(ctx->err, "plan.struct_size %u != %zu", plan->struct_size, sizeof(psl_plan)); return PSL_ERR_ARG; }
+    if (ctx->cfg.mode != PSL_MODE_INDEX || ctx->cfg.max_launch_records == 0) { set_err(ctx->err, "plan_set: needs PSL_MODE_INDEX and max_launch_records > 0"); return PSL_ERR_STATE; }
+    if (!ctx->indexed) { set_err(ctx->err, "plan_set: build the index first (psl_build_batches)"); return PSL_ERR_STATE; }
+    if (plan->n_beams < 1 || plan->n_beams > (uint32_t)kMaxPlanBeams || !plan->beams) { set_err(ctx->err, "plan: 1..%d fields", kMaxPlanBeams); return PSL_ERR_ARG; }
+    if (plan->rr_group < 1) { set_err(ctx->err, "plan.rr_group must be >= 1"); return PSL_ERR_ARG; }
+    for (int a = 0; a < 3; ++a)
+        if (!(isfinite(plan->phantom_lo[a]) && isfinite(plan->phantom_hi[a]) && plan->phantom_lo[a] < plan->phantom_hi[a])) { set_err(ctx->err, "plan: phantom box"); return PSL_ERR_ARG; }
+    CU(cudaSetDevice(ctx->cfg.device));
+    const Derived& d = ctx->d;
+    const Layout& L = ctx->L;
+    PlanSel sel;
+    memset(&sel, 0, sizeof sel);
+    sel.n_beams = plan->n_beams;
+    sel.bx0 = ctx->cfg.n_xbins; sel.bx1 = -1; sel.by0 = ctx->cfg.n_ybins; sel.by1 = -1;
+    std::vector<PlanBeam> pbs(plan->n_beams);
+    for (uint32_t i = 0; i < plan->n_beams; ++i) {
+        const psl_beam& b = plan->beams[i];
+        if (!(isfinite(b.gantry_deg) && isfinite(b.coll_deg) && isfinite(b.couch_deg))) { set_err(ctx->err, "plan: field %u has a non-finite angle", i); return PSL_ERR_ARG; }
+        memset(&pbs[i], 0, sizeof(PlanBeam));
+        psl_status ms = make_beam(ctx, &b, &pbs[i].b, ctx->err);
+        if (ms != PSL_OK) return ms;
+        field_matrix(b, pbs[i].M);
+        roi_bins(ctx->cfg, &b, sel.sel[i]);
+        if (sel.sel[i][0] <= sel.sel[i][1] && sel.sel[i][2] <= sel.sel[i][3]) {
+            sel.bx0 = sel.sel[i][0] < sel.bx0 ? sel.sel[i][0] : sel.bx0; sel.bx1 = sel.sel[i][1] > sel.bx1 ? sel.sel[i][1] : sel.bx1;
+            sel.by0 = sel.sel[i][2] < sel.by0 ? sel.sel[i][2] : sel.by0; sel.by1 = sel.sel[i][3] > sel.by1 ? sel.sel[i][3] : sel.by1;
+        }
+    }
+    ctx->h_plan_beams = pbs;  // lives as long as the context: the copy below is asynchronous
+    ctx->plan = *plan;
+    ctx->plan.beams = nullptr;
+    ctx->plan_sel = sel;
+    unsigned long long* total = at<unsigned long long>(ctx, L.plan_total);
+    CU(cudaMemcpyAsync(at<PlanBeam>(ctx, L.plan_beams), ctx->h_plan_beams.data(), pbs.size() * sizeof(PlanBeam), cudaMemcpyHostToDevice, ctx->stream));
+    CU(cudaMemsetAsync(total, 0, 8, ctx->stream));
+    {
+        Prof prof(ctx, PSL_K_SAMPLE);
+        k_plan_total<<<592, 256, 0, ctx->stream>>>(at<uint32_t>(ctx, L.idx_counts), d.K, d.n_pos, (uint32_t)ctx->cfg.n_xbins, sel, total);
+        LAUNCHED();
+        k_plan_budgets<<<d.n_batches, 256, 0, ctx->stream>>>(at<uint32_t>(ctx, L.idx_counts), d.n_pos, (uint32_t)ctx->cfg.n_xbins, sel,
+                                                            (unsigned long long)plan->n_simulate, total, plan->rr_group,
+                                                            at<uint32_t>(ctx, L.plan_budget), at<uint32_t>(ctx, L.plan_mask),
+                                                            at<unsigned long long>(ctx, L.plan_len), at<unsigned long long>(ctx, L.plan_rounds));
+        LAUNCHED();
+    }
+    CU(cudaMemcpyAsync(ctx->h_plan, total, 8, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaMemcpyAsync(ctx->h_plan + 1, at<uint8_t>(ctx, L.plan_len), (uint64_t)d.n_batches * 8, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaMemcpyAsync(ctx->h_plan + 1 + d.n_batches, at<uint8_t>(ctx, L.plan_rounds), (uint64_t)d.n_batches * 8, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    ctx->plan_set = true;
+    if (n_total_psl) *n_total_psl = ctx->h_plan[0];
+    if (list_len) *list_len = reinterpret_cast<const uint64_t*>(ctx->h_plan + 1);
+    return PSL_OK;
+}
+
+psl_status psl_plan_tables(psl_ctx* ctx, const uint32_t** budget, const uint32_t** mask)
+{
+    if (!ctx) return PSL_ERR_ARG;
+    if (!ctx->plan_set) { set_err(ctx->err, "plan_tables: no plan"); return PSL_ERR_STATE; }
+    if (budget) *budget = at<uint32_t>(ctx, ctx->L.plan_budget);
+    if (mask) *mask = at<uint32_t>(ctx, ctx->L.plan_mask);
+    return PSL_OK;
+}
+
+psl_status psl_sample_batch(psl_ctx* ctx, int32_t t, int32_t ie, psl_launch* out)
+{
+    if (!ctx || !out) return PSL_ERR_ARG;
+    if (!ctx->plan_set) { set_err(ctx->err, "sample_batch: psl_plan_set first"); return PSL_ERR_STATE; }
+    if (t < 0 || t >= ctx->cfg.n_types || ie < 0 || ie >= ctx->cfg.n_ebins) { set_err(ctx->err, "sample_batch: (t, ie) out of range"); return PSL_ERR_ARG; }
+    CU(cudaSetDevice(ctx->cfg.device));
+    const Derived& d = ctx->d;
+    const Layout& L = ctx->L;
+    const uint32_t b = (uint32_t)(t * ctx->cfg.n_ebins + ie);
+    const unsigned long long len = ctx->h_plan[1 + b], rounds = ctx->h_plan[1 + d.n_batches + b];
+    if (len > ctx->cfg.max_launch_records) {
+        set_err(ctx->err, "sample_batch: the launch list has %llu entries, more than max_launch_records %llu", len, (unsigned long long)ctx->cfg.max_launch_records);
+        return PSL_ERR_CAPACITY;
+    }
+    memset(out, 0, sizeof *out);
+    LaunchStats* stats = at<LaunchStats>(ctx, L.l_stats);
+    uint32_t* counter = reinterpret_cast<uint32_t*>(stats + 1);
+    uint32_t* slot = at<uint32_t>(ctx, L.l_slot);
+    uint8_t* beam = at<uint8_t>(ctx, L.l_beam);
+    CU(cudaMemsetAsync(stats, 0, sizeof(LaunchStats) + 16, ctx->stream));
+    if (len > 0) {
+        const PlanSel& sel = ctx->plan_sel;
+        const uint32_t nt = (uint32_t)((len + kEmitTile - 1) / kEmitTile);
+        CU(cudaMemsetAsync(at<uint8_t>(ctx, L.l_state), 0, (uint64_t)nt * 8, ctx->stream));
+        LaunchOut lo;
+        lo.E = at<float>(ctx, L.l_out[0]); lo.X = at<float>(ctx, L.l_out[1]); lo.Y = at<float>(ctx, L.l_out[2]); lo.Z = at<float>(ctx, L.l_out[3]);
+        lo.U = at<float>(ctx, L.l_out[4]); lo.V = at<float>(ctx, L.l_out[5]); lo.W = at<float>(ctx, L.l_out[6]); lo.wt = at<float>(ctx, L.l_out[7]);
+        lo.src = at<uint32_t>(ctx, L.l_src); lo.beam = at<uint8_t>(ctx, L.l_beam_of);
+        PhantomBox box;
+        for (int a = 0; a < 3; ++a) { box.lo[a] = ctx->plan.phantom_lo[a]; box.hi[a] = ctx->plan.phantom_hi[a]; }
+        Prof prof(ctx, PSL_K_SAMPLE);
+        const uint32_t grid = (uint32_t)(rounds < 1184ull ? rounds : 1184ull);
+        k_sample_batch<<<grid, 256, 0, ctx->stream>>>(at<uint32_t>(ctx, L.idx_counts), at<uint32_t>(ctx, L.idx_offsets),
+                                                      at<uint32_t>(ctx, L.plan_budget), at<uint32_t>(ctx, L.plan_mask), b * d.n_pos,
+                                                      (uint32_t)ctx->cfg.n_xbins, sel.bx0, sel.bx1, sel.by0, sel.by1, ctx->plan.rr_group,
+                                                      (unsigned long long)ctx->plan.seed, at<unsigned long long>(ctx, L.plan_rounds) + b,
+                                                      slot, beam);
+        LAUNCHED();
+        k_emit<<<nt, kThreads, 0, ctx->stream>>>(at<uint4>(ctx, L.aos_index), slot, beam, (uint32_t)len, at<PlanBeam>(ctx, L.plan_beams),
+                                                 ctx->plan.n_beams, ctx->cfg.geom.z_iso - ctx->cfg.geom.z_plane,
+                                                 (ctx->cfg.flags & PSL_DROP_ZERO_WEIGHT) ? 1u : 0u, box, lo,
+                                                 at<unsigned long long>(ctx, L.l_state), counter, stats);
+        LAUNCHED();
+        out->slot = slot; out->beam = beam;
+        out->E = lo.E; out->X = lo.X; out->Y = lo.Y; out->Z = lo.Z; out->U = lo.U; out->V = lo.V; out->W = lo.W; out->wt = lo.wt;
+        out->src_index = lo.src; out->beam_of = lo.beam;
+    }
+    CU(cudaMemcpyAsync(ctx->h_launch_stats, stats, sizeof(LaunchStats), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    out->n_list = (uint32_t)len;
+    out->n_launch = (uint32_t)ctx->h_launch_stats->n_launched;
+    out->n_jaw_rejected = ctx->h_launch_stats->n_jaw;
+    out->n_zero_weight = ctx->h_launch_stats->n_zero;
+    out->n_missed = ctx->h_launch_stats->n_missed;
+    return PSL_OK;
+}
+
+psl_status psl_flush_schedule(psl_ctx* ctx, uint32_t capacity, psl_flush* out)
+{
+    if (!ctx || !out) return PSL_ERR_ARG;
+    if (ctx->cfg.mode != PSL_MODE_ONTHEFLY || ctx->cfg.max_launch_records == 0) { set_err(ctx->err, "flush_schedule: needs PSL_MODE_ONTHEFLY and max_launch_records > 0"); return PSL_ERR_STATE; }
+    if (ctx->result != RES_OTF) { set_err(ctx->err, "flush_schedule: no build yet"); return PSL_ERR_STATE; }
+    if (capacity < 1) { set_err(ctx->err, "flush_schedule: capacity must be >= 1"); return PSL_ERR_ARG; }
+    CU(cudaSetDevice(ctx->cfg.device));
+    const Derived& d = ctx->d;
+    const Layout& L = ctx->L;
+    const uint32_t cap = (uint32_t)ctx->cfg.max_launch_records;
+    uint32_t* totals = at<uint32_t>(ctx, L.f_totals);
+    FlushOut fo = {at<uint32_t>(ctx, L.f_key), at<uint32_t>(ctx, L.f_first), at<uint32_t>(ctx, L.f_count)};
+    {
+        Prof prof(ctx, PSL_K_OTHER);
+        k_flush_plan<<<1, 1024, 0, ctx->stream>>>(at<uint32_t>(ctx, L.counts), d.K, capacity, at<uint32_t>(ctx, L.f_full), at<uint32_t>(ctx, L.f_part), totals);
+        LAUNCHED();
+        k_flush_events<<<d.K < 592u ? d.K : 592u, 256, 0, ctx->stream>>>(at<uint32_t>(ctx, L.counts), at<uint32_t>(ctx, L.offsets), at<uint32_t>(ctx, L.out[9]),
+                                                                          d.K, capacity, at<uint32_t>(ctx, L.f_full), at<uint32_t>(ctx, L.f_part), totals, cap,
+                                                                          at<uint32_t>(ctx, L.f_trig), at<uint32_t>(ctx, L.f_tkey), at<uint32_t>(ctx, L.f_tfirst), fo);
+        LAUNCHED();
+        k_flush_order<<<592, 256, 0, ctx->stream>>>(at<uint32_t>(ctx, L.f_trig), at<uint32_t>(ctx, L.f_tkey), at<uint32_t>(ctx, L.f_tfirst), totals, cap, capacity, fo);
+        LAUNCHED();
+    }
+    CU(cudaMemcpyAsync(ctx->h_flush_totals, totals, 8, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    const unsigned long long ne = (unsigned long long)ctx->h_flush_totals[0] + ctx->h_flush_totals[1];
+    if (ne > cap) { set_err(ctx->err, "flush_schedule: %llu shipments, more than max_launch_records %u", ne, cap); return PSL_ERR_CAPACITY; }
+    out->n_events = (uint32_t)ne;
+    out->key = fo.key; out->first = fo.first; out->count = fo.count;
     return PSL_OK;
 }
 

@@ -32,7 +32,28 @@ struct DevGrid {
     int32_t has_pos, n_xbins, n_ybins, ix0, iy0;
     float inv_dx, inv_dy;
     uint32_t n_pos;
+    uint32_t apr;                  // PSL_APR: azimuthal particle redistribution before binning (INDEX mode)
+    unsigned long long apr_seed;
 };
+
+// counter-based generator (reading S2): the output function of splitmix64 applied to (seed, a), then to (that, b)
+constexpr unsigned long long kGamma64 = 0x9E3779B97F4A7C15ull;
+
+__host__ __device__ __forceinline__ unsigned long long mix64(unsigned long long z)
+{
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+    return z ^ (z >> 31);
+}
+__host__ __device__ __forceinline__ uint32_t rng32(unsigned long long seed, unsigned long long a, unsigned long long b)
+{
+    const unsigned long long h = mix64(seed + kGamma64 * (a + 1ull));
+    return (uint32_t)(mix64(h + kGamma64 * (b + 1ull)) >> 32);
+}
+__host__ __device__ __forceinline__ uint32_t below(uint32_t r, uint32_t n)
+{
+    return (uint32_t)(((unsigned long long)r * (unsigned long long)n) >> 32);
+}
 
 struct DevBeam {
     int32_t has_beam, has_jaws;
@@ -146,6 +167,41 @@ __device__ __forceinline__ float final_weight(const DevBeam& b, float wt, float 
     if (axis_bin(xm, b.inv_mdx, b.px0, b.map_nx, px) && axis_bin(ym, b.inv_mdy, b.py0, b.map_ny, py))
         F = __ldg(b.fluence + (size_t)py * (size_t)b.map_nx + (size_t)px);
     return __fmul_rn(__fmul_rn(wt, F), b.mu);
+}
+
+// Azimuthal particle redistribution: record `index` of the load order turns by 2 pi r / 2^32 about the
+// beam axis, r = rng32(seed, index, 0) -- position and direction by the same angle.  cos and sin in fp32 by fixed
+// operations (reading S7): nearest quarter turn, remainder |a| <= pi/4, Taylor polynomials in Horner form.
+__device__ __forceinline__ void apr_cos_sin(uint32_t r, float& c, float& s)
+{
+    const uint32_t k = (uint32_t)(((unsigned long long)r + 0x20000000ull) >> 30);
+    const int32_t rem = (int32_t)(r - (k << 30));
+    const float a = __fmul_rn((float)rem, 1.46291807926715968e-9f);  // pi / 2^31
+    const float a2 = __fmul_rn(a, a);
+    float t = __fmul_rn(2.75573192239858925e-6f, a2);
+    t = __fmul_rn(__fadd_rn(t, -1.98412698412698413e-4f), a2);
+    t = __fmul_rn(__fadd_rn(t, 8.33333333333333322e-3f), a2);
+    t = __fmul_rn(__fadd_rn(t, -1.66666666666666657e-1f), a2);
+    const float sn = __fadd_rn(a, __fmul_rn(t, a));
+    float q = __fmul_rn(2.48015873015873016e-5f, a2);
+    q = __fmul_rn(__fadd_rn(q, -1.38888888888888894e-3f), a2);
+    q = __fmul_rn(__fadd_rn(q, 4.16666666666666644e-2f), a2);
+    q = __fmul_rn(__fadd_rn(q, -0.5f), a2);
+    const float cs = __fadd_rn(1.0f, q);
+    const uint32_t kk = k & 3u;
+    c = kk == 0 ? cs : (kk == 1 ? -sn : (kk == 2 ? -cs : sn));
+    s = kk == 0 ? sn : (kk == 1 ? cs : (kk == 2 ? -sn : -cs));
+}
+
+__device__ __forceinline__ void apr_apply(unsigned long long seed, uint32_t index, Rec& r)
+{
+    float c, s;
+    apr_cos_sin(rng32(seed, index, 0), c, s);
+    const float x = __fsub_rn(__fmul_rn(r.x, c), __fmul_rn(r.y, s));
+    const float y = __fadd_rn(__fmul_rn(r.x, s), __fmul_rn(r.y, c));
+    const float u = __fsub_rn(__fmul_rn(r.u, c), __fmul_rn(r.v, s));
+    const float v = __fadd_rn(__fmul_rn(r.u, s), __fmul_rn(r.v, c));
+    r.x = x; r.y = y; r.u = u; r.v = v;
 }
 
 // Steps 1-4 (+6, +8 when a beam is given) for one raw record.  Returns the class; key is valid for every

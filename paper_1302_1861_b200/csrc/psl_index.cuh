@@ -112,6 +112,14 @@ __global__ void __launch_bounds__(kThreads, 3) k_scatter_idx_a(const ChunkDesc* 
             for (int r = 0; r < kRounds; ++r) {
                 int idx = w * kWarpSpan + r * 32 + lane_id();
                 rec[r] = rec_from_smem(raw, idx < (int)td.count ? idx : 0);
+                if (g.apr) {
+                    apr_apply(g.apr_seed, td.first_index + (uint32_t)idx, rec[r]);
+                    if (idx < (int)td.count) {
+                        uint32_t* p = raw + idx * kRecWords;
+                        p[2] = __float_as_uint(rec[r].x); p[3] = __float_as_uint(rec[r].y);
+                        p[4] = __float_as_uint(rec[r].u); p[5] = __float_as_uint(rec[r].v);
+                    }
+                }
             }
 #pragma unroll
             for (int r = 0; r < kRounds; ++r) {

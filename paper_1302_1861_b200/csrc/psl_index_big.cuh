@@ -196,6 +196,14 @@ __global__ void __launch_bounds__(kIdxBigThreads, 1) k_scatter_idx_big(const Chu
                     for (int r = 0; r < 4; ++r) {
                         const uint32_t idx = first + (h + r) * 32 + lane_id();
                         rec[r] = rec_from_smem(raw, idx < count ? (int)idx : 0);
+                        if (g.apr) {  // the redistributed position and direction are what the index stores
+                            apr_apply(g.apr_seed, s_desc[sq].first_index + idx, rec[r]);
+                            if (idx < count) {
+                                uint32_t* p = raw + idx * kRecWords;
+                                p[2] = __float_as_uint(rec[r].x); p[3] = __float_as_uint(rec[r].y);
+                                p[4] = __float_as_uint(rec[r].u); p[5] = __float_as_uint(rec[r].v);
+                            }
+                        }
                     }
 #pragma unroll
                     for (int r = 0; r < 4; ++r) {

@@ -429,6 +429,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_count_raw(const ChunkDesc* __re
             const int idx = (int)rec_idx(r);
             have[r] = idx < (int)td.count;
             rec[r] = rec_from_smem(raw, have[r] ? idx : 0);
+            if (IDX && g.apr) apr_apply(g.apr_seed, td.first_index + (uint32_t)idx, rec[r]);
         }
 #pragma unroll
         for (int r = 0; r < kRounds; ++r) {
