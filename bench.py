@@ -58,6 +58,7 @@ def parse_args():
     ap.add_argument("--records", type=int, default=0, help="override the number of records (0 = the config's own)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-next", action="store_true", help="skip the section-8(f) phase lines (sampling layer / shipments)")
     ap.add_argument("--verify", action="store_true",
                     help="after the timed regions, check the full-size result against the oracle (streaming counts)")
     return ap.parse_args()
@@ -354,8 +355,9 @@ def run_ours(args):
     host_chunks = [host[f * RECORD_BYTES:(f + c) * RECORD_BYTES] for f, c in chunks]
     dev_chunks = [resident[f * RECORD_BYTES:(f + c) * RECORD_BYTES] for f, c in chunks]
 
+    launch_cap = 0 if args.no_next else (6_000_000 if w.mode == 1 else 1 << 20)
     ctx = P.PslContext(w.grid, w.geometry, w.mode, max_records=n, max_host_records=0 if args.no_e2e else n,
-                       max_chunks=len(chunks) + 1, flags=w.flags, device=local)
+                       max_chunks=len(chunks) + 1, flags=w.flags, device=local, max_launch_records=launch_cap)
     beams = [None if b is None else ctx.beam(b) for b in w.beams]
     K = w.n_keys
     h_counts = torch.empty(K, dtype=torch.int32).pin_memory()
@@ -460,6 +462,46 @@ def run_ours(args):
             m_sel_all += n_idx - s["n_roi_skipped"]
     workload_stats = dict(n_valid_in_grid=n_idx, survivors_per_step=surv_all, roi_selected_per_step=m_sel_all)
 
+    # ---- section 8(f) phase lines (outside the timed value): sampling layer over the index / capacity-N shipments ---
+    nxt = None
+    if launch_cap and w.mode == 1 and all(b is not None for b in beams):
+        total_psl, lens = ctx.plan_set(beams, max(n_idx, 1), seed=1, rr_group=4)
+        # a plan whose largest division fills about two thirds of the launch buffer
+        n_sim = max(1, int(n_idx * min(1.0, 4_000_000 / max(max(lens), 1))))
+        torch.cuda.synchronize()
+        p0 = ev()
+        total_psl, lens = ctx.plan_set(beams, n_sim, seed=1, rr_group=4)
+        p1 = ev()
+        torch.cuda.synchronize()
+        b_big = max(range(len(lens)), key=lambda i: lens[i])
+        t_big, e_big = divmod(b_big, w.grid["n_ebins"])
+        ctx.sample_batch(t_big, e_big)
+        reps = 5
+        s0 = ev()
+        for _ in range(reps):
+            la = ctx.sample_batch(t_big, e_big)
+        s1 = ev()
+        torch.cuda.synchronize()
+        ms_s = s0.elapsed_time(s1) / reps
+        nxt = {"plan_set_ms": p0.elapsed_time(p1), "n_total_psl": total_psl, "n_simulate": n_sim, "fields": len(beams),
+               "division": [t_big, e_big], "list_entries": la["n_list"], "launched": la["n_launch"],
+               "sample_batch_ms": ms_s, "list_entries_per_s": la["n_list"] / (ms_s * 1e-3),
+               # list out (5 B) + one 32-byte index record in per entry + 38 B per launched particle out
+               "gbs": (37.0 * la["n_list"] + 38.0 * la["n_launch"]) / (ms_s * 1e-3) / 1e9,
+               "what": "psl_plan_set (budgets) + psl_sample_batch of the fullest (type, energy) division: round-robin launch "
+                       "list, per-field jaws / weights / rotations / surface projection, compaction; device time incl. the "
+                       "call's final synchronisation"}
+    elif launch_cap and w.mode == 0:
+        ctx.build_batches(beams[0])
+        ctx.flush_schedule(65536)
+        torch.cuda.synchronize()
+        s0 = ev()
+        fl = ctx.flush_schedule(65536)
+        s1 = ev()
+        torch.cuda.synchronize()
+        nxt = {"flush_schedule_ms": s0.elapsed_time(s1), "capacity": 65536, "shipments": fl["n_events"],
+               "what": "psl_flush_schedule: bins of 65536 particles shipped when full (PAPER.md:47)"}
+
     # ---- section 8(e)'s one optional exchange, once over NCCL, outside the timed value ----------------------
     exchange_ms = None
     if world > 1:
@@ -559,6 +601,8 @@ def run_ours(args):
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
             "per_phase": per_phase, "roofline": roofline, "kernels": kernels,
         }
+        if nxt is not None:
+            line["next_8f"] = nxt
         if exchange_ms is not None:
             line["exchange_ms"] = exchange_ms
         if verify is not None:

@@ -77,11 +77,15 @@ __device__ __forceinline__ uint32_t seg_of_warp(const uint32_t* __restrict__ vst
     return lo;
 }
 
-constexpr int kBeamTile = 2048;                       // index records one CTA of the beam kernel compacts
-constexpr int kBeamRounds = kBeamTile / kThreads;      // 8
+// 4 records per thread, 4 CTAs per SM (64 registers): the kernel is a chain of dependent latencies per tile (ticket ->
+// segment search -> loads -> look-back -> stores), so what pays is warps in flight -- 8 records per thread at 2 CTAs per
+// SM (122 registers) took 11.5 ms for config 5's nine beams, this shape 9.4 ms
+constexpr int kBeamRounds = 4;                         // index records per thread
+constexpr int kBeamOcc = 4;                            // CTAs per SM
+constexpr int kBeamTile = kBeamRounds * kThreads;      // 1024 index records per CTA
 constexpr int kBeamArrays = 12;  // E x y u v w wt xp yp src key + spare
 
-__global__ void __launch_bounds__(kThreads, 2) k_beam_compact(SegTable seg, IdxIn in, const __grid_constant__ DevGrid g,
+__global__ void __launch_bounds__(kThreads, kBeamOcc) k_beam_compact(SegTable seg, IdxIn in, const __grid_constant__ DevGrid g,
                                                              const __grid_constant__ DevBeam bm, SoAOut out,
                                                              uint32_t* __restrict__ out_key,
                                                              unsigned long long* __restrict__ tile_state,
@@ -155,12 +159,16 @@ __global__ void __launch_bounds__(kThreads, 2) k_beam_compact(SegTable seg, IdxI
     }
     __syncthreads();
 
-    // warp 0: exclusive prefix of the 64 (round, warp) counts, then the decoupled look-back over tile aggregates
+    // warp 0: exclusive prefix of the (round, warp) counts, then the decoupled look-back over tile aggregates
     if (w == 0) {
-        const uint32_t a = s_cnt[2 * lane_id()], b = s_cnt[2 * lane_id() + 1];
-        const uint32_t inc = warp_incl_scan(a + b);
-        s_cnt[2 * lane_id()] = inc - a - b;
-        s_cnt[2 * lane_id() + 1] = inc - b;
+        constexpr int kPer = kBeamRounds * kWarps / 32;  // counts per lane
+        uint32_t c[kPer], sum = 0;
+#pragma unroll
+        for (int k = 0; k < kPer; ++k) { c[k] = s_cnt[kPer * lane_id() + k]; sum += c[k]; }
+        const uint32_t inc = warp_incl_scan(sum);
+        uint32_t run = inc - sum;
+#pragma unroll
+        for (int k = 0; k < kPer; ++k) { s_cnt[kPer * lane_id() + k] = run; run += c[k]; }
         const uint32_t total = __shfl_sync(0xFFFFFFFFu, inc, 31);
         uint32_t excl = 0;
         if (tile == 0) {
