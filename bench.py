@@ -356,7 +356,7 @@ def run_ours(args):
     dev_chunks = [resident[f * RECORD_BYTES:(f + c) * RECORD_BYTES] for f, c in chunks]
 
     launch_cap = 0 if args.no_next else (6_000_000 if w.mode == 1 else 1 << 20)
-    ctx = P.PslContext(w.grid, w.geometry, w.mode, max_records=n, max_host_records=0 if args.no_e2e else n,
+    ctx = P.PslContext(w.grid, w.geometry, w.mode, max_records=n, max_host_records=0 if (args.no_e2e and not args.verify) else n,
                        max_chunks=len(chunks) + 1, flags=w.flags, device=local, max_launch_records=launch_cap)
     beams = [None if b is None else ctx.beam(b) for b in w.beams]
     K = w.n_keys

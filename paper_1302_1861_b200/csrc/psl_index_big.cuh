@@ -244,9 +244,13 @@ __global__ void __launch_bounds__(kIdxBigThreads, 1) k_scatter_idx_big(const Chu
             const uint32_t off = qq == 0 ? o0 : (qq == 1 ? o1 : (qq == 2 ? o2 : o3));
             uint4 a, b;
             if (KEYED) {
+#ifdef PSL_X_GGATHER
+                ldg_record(aos_in + 2 * ((size_t)(t0 + base + qq) * kTile + ir), a, b);
+#else
                 const uint4* p = reinterpret_cast<const uint4*>(ring + off) + 2 * ir;
                 a = p[0];
                 b = p[1];
+#endif
             } else {
                 const uint32_t* p = ring + off + ir * kRecWords;
                 const uint32_t fi = qq == 0 ? f0 : (qq == 1 ? f1 : (qq == 2 ? f2 : f3));
