@@ -1122,8 +1122,8 @@ psl_status psl_create(const psl_config* cfg, psl_ctx** out)
         ctx->sm_count_raw = count_layout(kTile * kRecBytes, ctx->count_stages, d.B_lo, ne).total;
         int max_smem = 0;
         CUC(cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, cfg->device));
-        ctx->idx_big_a = idx_big_layout(false, d.B_lo, ne).total + 1024 <= (uint32_t)max_smem;
-        ctx->idx_big_b = idx_big_layout(true, d.B_hi, ne).total + 1024 <= (uint32_t)max_smem;
+        ctx->idx_big_a = idx_big_layout(false, d.B_lo, ne).total <= (uint32_t)max_smem;  // these kernels have no static shared memory
+        ctx->idx_big_b = idx_big_layout(true, d.B_hi, ne).total <= (uint32_t)max_smem;
         ctx->split_a = ctx->idx_big_a ? kIdxSplit : 1;
         ctx->split_b = ctx->idx_big_b ? kIdxSplit : 1;
         ctx->sm_idx_a = ctx->idx_big_a ? idx_big_layout(false, d.B_lo, ne).total : idx_a_layout(d.B_lo, ne).total;

@@ -404,20 +404,21 @@ __device__ __forceinline__ double warp_sum_double(double v)
 
 // Stable rank of a record inside its warp's slice of the tile: records of one warp arrive in rounds of 32 consecutive
 // records; `cnt` is the warp's private running count per bucket (uint16 per bucket, zeroed per tile).  Lanes with
-// bucket == kNone take no part.  Must be called by all 32 lanes.  Ranks WITHOUT MATCH.ANY.  Measured on B200: one __match_any_sync costs ~2 cycles per distinct value on a unit
-// the whole SM shares -- ~58 cycles per warp instruction with ~1000 buckets, 1.8 cycles per record, a third of an INDEX
-// pass.  Here the lanes of a round CLAIM their bucket instead: the top 5 bits of the warp's private 16-bit counter take
-// the lane id (the low 11 bits keep the count; a warp ranks at most 2047 records of a bucket per tile), one store wins,
-// every lane reads the word back; a lane that reads its own id has the bucket to itself or won it.  Losers exist only
-// when two lanes of the round share a bucket: those buckets are resolved one at a time with a ballot (few of them),
-// or with one MATCH.ANY when there are many.  ~27-31 cycles per round at 1200 buckets, 39-45 at 192 (MATCH: 57-69).
-// The counters must be read through kRankCountMask by whoever sums them (finish_ranks*).
+// bucket == kNone take no part.  Must be called by all 32 lanes.  Ranks WITHOUT MATCH.ANY.  Measured on B200: one
+// __match_any_sync costs ~2 cycles per distinct value on a unit the whole SM shares -- ~58 cycles per warp instruction
+// with ~1000 buckets, 1.8 cycles per record, a third of an INDEX pass.  Here the lanes of a round CLAIM their bucket
+// instead: the top 5 bits of the warp's private 16-bit counter take the lane id (the low 11 bits keep the count; a warp
+// ranks at most 2047 records of a bucket per tile), one store wins, every lane reads the word back; a lane that reads
+// its own id has the bucket to itself or won it.  Losers exist only when lanes of the round share a bucket: each
+// loser ORs its lane bit into its winner's word of `grp` (32 words per warp, all zero between calls), and every lane
+// reads its winner's word: the peer mask of all colliding buckets at once (config 4: pass B 3.40 -> 3.04 ms against
+// resolving one bucket per ballot).  The counters must be read through kRankCountMask by whoever sums them.
 constexpr uint32_t kRankCountBits = 11;
 constexpr uint32_t kRankCountMask = (1u << kRankCountBits) - 1u;
 constexpr uint32_t kRankCountMask2 = kRankCountMask | (kRankCountMask << 16);  // two packed counters
 
 template <int R>
-__device__ __forceinline__ void warp_rank_claim(const uint32_t (&bucket)[R], uint32_t (&rank)[R], uint16_t* cnt)
+__device__ __forceinline__ void warp_rank_claim(const uint32_t (&bucket)[R], uint32_t (&rank)[R], uint16_t* cnt, uint32_t* grp)
 {
     const uint32_t lane = lane_id(), lt = lanemask_lt();
 #pragma unroll
@@ -429,20 +430,14 @@ __device__ __forceinline__ void warp_rank_claim(const uint32_t (&bucket)[R], uin
         if (act) cnt[b] = (uint16_t)(base | (lane << kRankCountBits));
         __syncwarp();
         const uint32_t win = act ? ((uint32_t)cnt[b] >> kRankCountBits) : lane;
-        uint32_t losers = __ballot_sync(0xFFFFFFFFu, win != lane);
         uint32_t peers = 1u << lane;
-        if (losers != 0u) {  // warp-uniform
-            if (__popc(losers) > 4) {
-                peers = __match_any_sync(0xFFFFFFFFu, b);
-            } else {
-                do {
-                    const int L = __ffs(losers) - 1;
-                    const uint32_t bL = __shfl_sync(0xFFFFFFFFu, b, L);
-                    const uint32_t m = __ballot_sync(0xFFFFFFFFu, b == bL);
-                    if (b == bL) peers = m;
-                    losers &= ~m;
-                } while (losers != 0u);
-            }
+        if (__any_sync(0xFFFFFFFFu, win != lane)) {
+            if (win != lane) atomicOr(&grp[win], 1u << lane);
+            __syncwarp();
+            const uint32_t m = grp[win];
+            if (m != 0u) peers = m | (1u << win);
+            __syncwarp();
+            if (win == lane && m != 0u) grp[lane] = 0u;
         }
         const uint32_t before = __popc(peers & lt);
         if (act && before == 0u) cnt[b] = (uint16_t)(base + __popc(peers));  // the lowest peer; claim bits cleared

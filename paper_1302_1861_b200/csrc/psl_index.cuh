@@ -57,6 +57,8 @@ __global__ void __launch_bounds__(kThreads, 3) k_scatter_idx_a(const ChunkDesc* 
                                                               uint32_t stride, uint4* __restrict__ aos)
 {
     extern __shared__ __align__(128) uint8_t smem[];
+    __shared__ uint32_t s_grp[kWarps][32];  // warp_rank_claim's group words
+    s_grp[threadIdx.x >> 5][threadIdx.x & 31] = 0u;
     const IdxASmem L = idx_a_layout(B, g.n_ebins + 1);
     uint32_t* run = reinterpret_cast<uint32_t*>(smem + L.run);
     uint32_t* skey = reinterpret_cast<uint32_t*>(smem + L.skey);
@@ -131,7 +133,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_scatter_idx_a(const ChunkDesc* 
             uint32_t bk[kRounds], rk[kRounds];
 #pragma unroll
             for (int r = 0; r < kRounds; ++r) bk[r] = packed[r] == kNone ? kNone : (packed[r] & lo_mask);
-            warp_rank_claim<kRounds>(bk, rk, cnt + w * Bp);
+            warp_rank_claim<kRounds>(bk, rk, cnt + w * Bp, s_grp[w]);
 #pragma unroll
             for (int r = 0; r < kRounds; ++r) packed[r] = packed[r] == kNone ? kNone : ((packed[r] << 9) | rk[r]);
         }
@@ -239,6 +241,8 @@ __global__ void __launch_bounds__(kThreads, 4) k_scatter_idx_b(const uint4* __re
                                                               uint32_t stride, uint4* __restrict__ aos_out)
 {
     extern __shared__ __align__(128) uint8_t smem[];
+    __shared__ uint32_t s_grp[kWarps][32];  // warp_rank_claim's group words
+    s_grp[threadIdx.x >> 5][threadIdx.x & 31] = 0u;
     const IdxBSmem L = idx_b_layout(B);
     uint32_t* ring = reinterpret_cast<uint32_t*>(smem + L.ring);
     uint32_t* run = reinterpret_cast<uint32_t*>(smem + L.run);
@@ -291,7 +295,7 @@ __global__ void __launch_bounds__(kThreads, 4) k_scatter_idx_b(const uint4* __re
         }
         {
             uint32_t rk[kRounds];
-            warp_rank_claim<kRounds>(packed, rk, cnt + w * Bp);
+            warp_rank_claim<kRounds>(packed, rk, cnt + w * Bp, s_grp[w]);
 #pragma unroll
             for (int r = 0; r < kRounds; ++r) packed[r] = packed[r] == kNone ? kNone : ((packed[r] << 9) | rk[r]);
         }

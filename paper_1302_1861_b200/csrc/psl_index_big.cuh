@@ -25,7 +25,7 @@ constexpr int kIdxBigSpan = kIdxBigTile / kIdxBigWarps;   // 256 records per war
 constexpr int kIdxBigRounds = kIdxBigSpan / 32;           // 8
 
 struct IdxBigSmem {
-    uint32_t ring, stage_bytes, cnt, gcur, lstart, perm, pbkt, edges, misc, desc, bars, total;
+    uint32_t ring, stage_bytes, cnt, gcur, lstart, perm, pbkt, edges, misc, grp, desc, bars, total;
 };
 
 __host__ __device__ inline IdxBigSmem idx_big_layout(bool keyed, uint32_t B, uint32_t n_edges)
@@ -42,6 +42,7 @@ __host__ __device__ inline IdxBigSmem idx_big_layout(bool keyed, uint32_t B, uin
     L.pbkt = p;
     L.edges = p;  p += round_up(n_edges * 4, 16);
     L.misc = p;   p += 64 * 4;
+    L.grp = p;    p += kIdxBigWarps * 32 * 4;
     L.desc = p;   p += stages * 16;
     L.bars = p;   p += stages * 8;
     L.total = p;
@@ -78,9 +79,11 @@ __global__ void __launch_bounds__(kIdxBigThreads, 1) k_scatter_idx_big(const Chu
     uint32_t* slot = reinterpret_cast<uint32_t*>(smem + L.perm);  // tile-sorted slot -> bucket << 12 | record in tile
     float* s_edges = reinterpret_cast<float*>(smem + L.edges);
     uint32_t* misc = reinterpret_cast<uint32_t*>(smem + L.misc);
+    uint32_t* grp = reinterpret_cast<uint32_t*>(smem + L.grp);  // warp_rank_claim's group words, 32 per warp
     TileDesc* s_desc = reinterpret_cast<TileDesc*>(smem + L.desc);
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + L.bars);
     const uint32_t w = warp_id();
+    grp[threadIdx.x] = 0u;
     const uint32_t lo_mask = (1u << lo_bits) - 1u;
     const uint32_t n_rec = KEYED ? *n_ptr : 0u;
     uint32_t goff = 0;  // ring stages this CTA has consumed in earlier spans (stage and parity bookkeeping runs on)
@@ -218,7 +221,7 @@ __global__ void __launch_bounds__(kIdxBigThreads, 1) k_scatter_idx_big(const Chu
                 }
             }
         }
-        warp_rank_claim<kIdxBigRounds>(bkt, rnk, cnt + w * Bp);
+        warp_rank_claim<kIdxBigRounds>(bkt, rnk, cnt + w * Bp, grp + w * 32);
         __syncthreads();
         const uint32_t n_part = finish_ranks_pair(cnt, Bp, gcur, lstart, misc, grun);
 
@@ -244,13 +247,9 @@ __global__ void __launch_bounds__(kIdxBigThreads, 1) k_scatter_idx_big(const Chu
             const uint32_t off = qq == 0 ? o0 : (qq == 1 ? o1 : (qq == 2 ? o2 : o3));
             uint4 a, b;
             if (KEYED) {
-#ifdef PSL_X_GGATHER
-                ldg_record(aos_in + 2 * ((size_t)(t0 + base + qq) * kTile + ir), a, b);
-#else
                 const uint4* p = reinterpret_cast<const uint4*>(ring + off) + 2 * ir;
                 a = p[0];
                 b = p[1];
-#endif
             } else {
                 const uint32_t* p = ring + off + ir * kRecWords;
                 const uint32_t fi = qq == 0 ? f0 : (qq == 1 ? f1 : (qq == 2 ? f2 : f3));
