@@ -242,7 +242,6 @@ using ScatterCompFn = void (*)(const uint4*, Span, DevBeam, uint32_t, const uint
 using ScatterOtfFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, const uint32_t*, uint32_t, SoAOut, SegStats*,
                               const uint8_t*, FusedScan, StatsTail);
 using ScatterBigFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, const uint32_t*, uint32_t, SoAOut, SegStats*, FusedScan, StatsTail);
-using ScatterIdxAFn = void (*)(const ChunkDesc*, uint32_t, Span, DevGrid, DevBeam, uint32_t, uint32_t, const uint32_t*, uint32_t, uint4*);
 
 template <bool POS, bool EDGES>
 CountFn count_otf_pe(int beam)
@@ -299,12 +298,6 @@ ScatterIdxBigFn scatter_idx_big_a_fn(bool pos, bool edges)
                : (edges ? k_scatter_idx_big<false, false, true> : k_scatter_idx_big<false, false, false>);
 }
 ScatterIdxBigFn scatter_idx_big_b_fn() { return k_scatter_idx_big<true, false, false>; }
-ScatterIdxAFn scatter_idx_a_fn(bool pos, bool edges)
-{
-    return pos ? (edges ? k_scatter_idx_a<true, true> : k_scatter_idx_a<true, false>)
-               : (edges ? k_scatter_idx_a<false, true> : k_scatter_idx_a<false, false>);
-}
-
 }  // namespace
 
 struct psl_ctx {
@@ -335,8 +328,6 @@ struct psl_ctx {
     bool big_tiles = false;  // ONTHEFLY with few keys: the 4096-record-tile scatter
     uint32_t count_stages = kStagesCount, count_split = 1;
     uint32_t sm_count_raw = 0, sm_scatter_otf = 0, sm_idx_a = 0, sm_count_b = 0, sm_idx_b = 0;  // dynamic smem bytes
-    // INDEX passes: 4096-record tiles when the counters of the pass fit shared memory beside the ring, else 1024
-    bool idx_big_a = false, idx_big_b = false;
     uint32_t split_a = 1, split_b = 1;  // histogram CTAs (= table columns) per scatter segment
     struct ChunkLaunch { Span span; uint32_t n_seg; };
     std::vector<ChunkDesc> pending_chunks;  // ONTHEFLY: chunk descriptors not yet on the device
@@ -766,7 +757,7 @@ psl_status finalize_index(psl_ctx* ctx)
         if (s != PSL_OK) return s;
         {
             Prof prof(ctx, PSL_K_INDEX_A);
-            if (ctx->idx_big_a) {
+            {
                 // ONE launch walks every chunk's span with the segments the counts were taken on
                 std::vector<SpanSeg>& hs = ctx->h_spans;  // lives as long as the context: the copy below is asynchronous
                 hs.clear();
@@ -782,12 +773,6 @@ psl_status finalize_index(psl_ctx* ctx)
                     chunks, ctx->n_chunks, d_spans, (uint32_t)hs.size(), unused, nullptr, nullptr, ctx->grid, none, d.B_lo, d.lo_bits, table_a,
                     d.cols_cap, aos);
                 LAUNCHED();
-            } else {
-                for (const psl_ctx::ChunkLaunch& cl : ctx->idx_launches) {  // the same segments the counts were taken on
-                    scatter_idx_a_fn(ctx->grid.has_pos != 0, ctx->grid.ebin_mode != 0)<<<cl.n_seg, kThreads, ctx->sm_idx_a, ctx->stream>>>(
-                        chunks, ctx->n_chunks, cl.span, ctx->grid, none, d.B_lo, d.lo_bits, table_a, d.cols_cap, aos);
-                    LAUNCHED();
-                }
             }
         }
         // pass B runs over the n_idx <= n_records keyed records; the device knows n_idx, the host only the bound
@@ -811,13 +796,9 @@ psl_status finalize_index(psl_ctx* ctx)
         {
             Prof prof(ctx, PSL_K_INDEX_B);
             const Span spb = {0u, 0u, 0u, ctx->split_b};
-            if (ctx->idx_big_b)
-                scatter_idx_big_b_fn()<<<Sb, kIdxBigThreads, ctx->sm_idx_b, ctx->stream>>>(nullptr, 0, nullptr, 0, spb, aos, scalar(ctx, SC_NIDX), ctx->grid, none,
-                                                                                    d.B_hi, d.lo_bits, table_b, kMaxSegments,
-                                                                                    at<uint4>(ctx, L.aos_index));
-            else
-                k_scatter_idx_b<<<Sb, kThreads, ctx->sm_idx_b, ctx->stream>>>(aos, scalar(ctx, SC_NIDX), d.B_hi, d.lo_bits, table_b, kMaxSegments,
-                                                                             at<uint4>(ctx, L.aos_index));
+            scatter_idx_big_b_fn()<<<Sb, kIdxBigThreads, ctx->sm_idx_b, ctx->stream>>>(nullptr, 0, nullptr, 0, spb, aos, scalar(ctx, SC_NIDX), ctx->grid, none,
+                                                                                d.B_hi, d.lo_bits, table_b, kMaxSegments,
+                                                                                at<uint4>(ctx, L.aos_index));
             LAUNCHED();
         }
         k_offsets_by_search_keyed<<<(d.K + 1 + 255) / 256, 256, 0, ctx->stream>>>(at<uint4>(ctx, L.aos_index), scalar(ctx, SC_NIDX), d.K, idx_offsets);
@@ -1120,27 +1101,19 @@ psl_status psl_create(const psl_config* cfg, psl_ctx** out)
     } else {
         ctx->count_stages = d.B_lo * 4 > 8192 ? 2 : kStagesCount;
         ctx->sm_count_raw = count_layout(kTile * kRecBytes, ctx->count_stages, d.B_lo, ne).total;
-        int max_smem = 0;
-        CUC(cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, cfg->device));
-        ctx->idx_big_a = idx_big_layout(false, d.B_lo, ne).total <= (uint32_t)max_smem;  // these kernels have no static shared memory
-        ctx->idx_big_b = idx_big_layout(true, d.B_hi, ne).total <= (uint32_t)max_smem;
-        ctx->split_a = ctx->idx_big_a ? kIdxSplit : 1;
-        ctx->split_b = ctx->idx_big_b ? kIdxSplit : 1;
-        ctx->sm_idx_a = ctx->idx_big_a ? idx_big_layout(false, d.B_lo, ne).total : idx_a_layout(d.B_lo, ne).total;
+        // the two sort passes: 2048-record tiles, two CTAs per SM when the counters leave room (they do up to ~1900 buckets)
+        ctx->split_a = ctx->split_b = kIdxSplit;
+        ctx->sm_idx_a = idx_big_layout(false, d.B_lo, ne).total;
         ctx->sm_count_b = count_layout(0, 0, d.B_hi, 0).total;
-        ctx->sm_idx_b = ctx->idx_big_b ? idx_big_layout(true, d.B_hi, ne).total : idx_b_layout(d.B_hi).total;
+        ctx->sm_idx_b = idx_big_layout(true, d.B_hi, ne).total;
         const bool pos = d.n_pos > 1, edges = cfg->ebin_mode == PSL_EBIN_EDGES;
         CUC(allow_smem(count_idx_fn(pos, edges), ctx->sm_count_raw));
-        if (ctx->idx_big_a) CUC(allow_smem(scatter_idx_big_a_fn(pos, edges), ctx->sm_idx_a));
-        else CUC(allow_smem(scatter_idx_a_fn(pos, edges), ctx->sm_idx_a));
+        CUC(allow_smem(scatter_idx_big_a_fn(pos, edges), ctx->sm_idx_a));
         CUC(allow_smem(k_count_keys, ctx->sm_count_b));
-        if (ctx->idx_big_b) CUC(allow_smem(scatter_idx_big_b_fn(), ctx->sm_idx_b));
-        else CUC(allow_smem(k_scatter_idx_b, ctx->sm_idx_b));
-        if (ctx->idx_big_a) CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, scatter_idx_big_a_fn(pos, edges), kIdxBigThreads, ctx->sm_idx_a));
-        else CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, scatter_idx_a_fn(pos, edges), kThreads, ctx->sm_idx_a));
+        CUC(allow_smem(scatter_idx_big_b_fn(), ctx->sm_idx_b));
+        CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, scatter_idx_big_a_fn(pos, edges), kIdxBigThreads, ctx->sm_idx_a));
         ctx->S_a = width(occ);
-        if (ctx->idx_big_b) CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, scatter_idx_big_b_fn(), kIdxBigThreads, ctx->sm_idx_b));
-        else CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_scatter_idx_b, kThreads, ctx->sm_idx_b));
+        CUC(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, scatter_idx_big_b_fn(), kIdxBigThreads, ctx->sm_idx_b));
         ctx->S_b = width(occ);
     }
     CUC(cudaStreamSynchronize(ctx->stream));

@@ -1,26 +1,31 @@
-// psl_index_big.cuh -- INDEX passes A and B with 4096-record tiles and tile-sorted staging.
+// psl_index_big.cuh -- INDEX passes A and B (paper method 3): two stable LSD passes over the full
+// key, split into two balanced digits key = hi * 2^s + lo (each <= 2048 buckets), with tile-sorted staging.
 //
-// Why: a 32-byte sector that is written by a store request of its own costs the same ~40 G requests/s on
-// B200 whether or not its line is completed later; only a store instruction that covers
-// several consecutive sectors is cheap.  With ~1100 buckets per pass a 4096-record tile holds ~4 records per
-// bucket: ordered by (bucket, input order) inside the tile they form ~128-byte runs, and the lanes of a warp
-// write consecutive 16-byte halves of consecutive slots, so one request covers a whole run.
+//   pass A: raw 28-byte records -> 32-byte keyed records {key, E, x, y, u, v, wt, src}, stably partitioned by lo
+//   pass B: keyed records -> the index: keyed records sorted by the full key (stable partition by hi)
 //
-// One 512-thread CTA per SM: the tile is 4 ring stages of 1024 records that stay where TMA put them, a fifth
-// (pass B) or fifth and sixth (pass A) stage prefetch.  Warp w owns records [256 w, 256 w + 256) of the tile (a quarter of a stage): per-warp private
-// uint16 counters + __match_any_sync give stable ranks, finish_ranks the prefix over the 16 warps.
+// A tile is two ring stages of 1024 records that stay where TMA put them.  Warp w owns records [256 w, 256 w + 256) of
+// the tile (a quarter of a stage): per-warp private uint16 counters + claimed peer masks (warp_rank_claim) give stable
+// ranks, finish_ranks the prefix over the 8 warps; the records are then ordered by (bucket, input order) inside the
+// tile, and every record leaves as ONE 32-byte store request, so that a run of records of one bucket is one request
+// per 128-byte line.
 #pragma once
 
 #include "psl_index.cuh"
 
 namespace psl {
 
-constexpr int kIdxBigQ = 4;                               // ring stages per tile
-constexpr int kIdxBigTile = kIdxBigQ * kTile;             // 4096 records
-constexpr int kIdxBigStagesRaw = 6;    // pass A: 4 being worked on + 2 in flight (28 KB each)
-constexpr int kIdxBigStagesKeyed = 5;  // pass B: 4 + 1 (32 KB each)
-constexpr int kIdxBigThreads = 512;
-constexpr int kIdxBigWarps = kIdxBigThreads / 32;         // 16
+// Two 256-thread CTAs per SM, each on 2048-record tiles (two ring stages, no prefetch stage: while one CTA waits for its
+// next tile the other one ranks or writes).  Measured at config 4 / 5 against one 512-thread CTA per SM on 4096-record
+// tiles with 1-2 stages of prefetch: pass A 3.29 -> 3.07 ms / 16.4 -> 15.3 ms, pass B 3.06 -> 2.77 / 15.2 -> 13.7 ms:
+// the phases of a tile use different units (ranks: counters and the claim words; write-out: the LSU), and a second,
+// independent CTA fills the slots the barriers leave empty.  Runs per bucket halve (2 records), which costs less.
+constexpr int kIdxBigQ = 2;                               // ring stages per tile
+constexpr int kIdxBigTile = kIdxBigQ * kTile;             // 2048 records
+constexpr int kIdxBigStagesRaw = 2;    // pass A (28 KB each)
+constexpr int kIdxBigStagesKeyed = 2;  // pass B (32 KB each)
+constexpr int kIdxBigThreads = 128 * kIdxBigQ;            // 256
+constexpr int kIdxBigWarps = kIdxBigThreads / 32;         // 8
 constexpr int kIdxBigSpan = kIdxBigTile / kIdxBigWarps;   // 256 records per warp
 constexpr int kIdxBigRounds = kIdxBigSpan / 32;           // 8
 
@@ -36,7 +41,7 @@ __host__ __device__ inline IdxBigSmem idx_big_layout(bool keyed, uint32_t B, uin
     const uint32_t stages = keyed ? kIdxBigStagesKeyed : kIdxBigStagesRaw;
     L.ring = p;   p += stages * L.stage_bytes;
     L.cnt = p;    p += round_up(kIdxBigWarps * round_up(B, 8) * 2, 16);
-    L.gcur = p;   p += round_up(B, 8) * 4;                // Bp entries: finish_ranks_pair writes whole 16-byte groups
+    L.gcur = p;   p += round_up(B, 8) * 4;                // Bp entries
     L.lstart = p; p += round_up(B, 8) * 4;
     L.perm = p;   p += kIdxBigTile * 4;                   // tile-sorted slot -> bucket << 12 | record in tile
     L.pbkt = p;
@@ -59,7 +64,7 @@ struct SpanSeg {
 // with the running slots re-read from that span's table columns.  Pass B (KEYED = true) has one span, computed
 // from *n_ptr.
 template <bool KEYED, bool POS, bool EDGES>
-__global__ void __launch_bounds__(kIdxBigThreads, 1) k_scatter_idx_big(const ChunkDesc* __restrict__ chunks, uint32_t n_chunks,
+__global__ void __launch_bounds__(kIdxBigThreads, 2) k_scatter_idx_big(const ChunkDesc* __restrict__ chunks, uint32_t n_chunks,
                                                                 const SpanSeg* __restrict__ spans, uint32_t n_spans, Span sp,
                                                                 const uint4* __restrict__ aos_in,
                                                                 const uint32_t* __restrict__ n_ptr,
@@ -128,10 +133,10 @@ __global__ void __launch_bounds__(kIdxBigThreads, 1) k_scatter_idx_big(const Chu
     }
     if (threadIdx.x == 0)
         for (uint32_t k = 0; k < (uint32_t)kIdxBigStages && k < n; ++k) issue(k);
-    uint32_t grun[8];  // the pair of threads (2g, 2g+1) keeps the running first free slot of buckets 8g..8g+7
+    uint32_t grun[8];  // thread t keeps the running first free slot of buckets 8t..8t+7
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
-        uint32_t b = (threadIdx.x >> 1) * 8 + k;
+        uint32_t b = threadIdx.x * 8 + k;
         grun[k] = b < B ? table[(size_t)b * stride + col] : 0u;
     }
     __syncthreads();
@@ -223,7 +228,7 @@ __global__ void __launch_bounds__(kIdxBigThreads, 1) k_scatter_idx_big(const Chu
         }
         warp_rank_claim<kIdxBigRounds>(bkt, rnk, cnt + w * Bp, grp + w * 32);
         __syncthreads();
-        const uint32_t n_part = finish_ranks_pair(cnt, Bp, gcur, lstart, misc, grun);
+        const uint32_t n_part = finish_ranks<true, kIdxBigWarps>(cnt, B, Bp, gcur, lstart, misc, grun);
 
         // tile-sorted order
 #pragma unroll

@@ -259,67 +259,6 @@ __device__ __forceinline__ uint32_t finish_ranks(uint16_t* cnt, uint32_t B, uint
     return total;
 }
 
-// finish_ranks for the 512-thread kernels (16 warps, STAGED): the PAIR of threads (2g, 2g+1) owns buckets 8g..8g+7, thread 2g
-// sums the counters of warps 0..7 and thread 2g+1 those of warps 8..15, so all 512 threads take part for up to 2048
-// buckets (with one thread per group only 128-150 of them worked while twelve warps waited at the barrier).  Both
-// threads of a pair keep the same running slots grun[8] (initialise them for buckets 8 * (threadIdx.x >> 1) + k).
-// gcur and lstart must hold Bp entries.  Same contract as finish_ranks<true, 16>: call after a __syncthreads, ends
-// with one.
-__device__ __forceinline__ uint32_t finish_ranks_pair(uint16_t* cnt, uint32_t Bp, uint32_t* gcur, uint32_t* lstart,
-                                                      uint32_t* misc, uint32_t (&grun)[8])
-{
-    const uint32_t g = threadIdx.x >> 1, half = threadIdx.x & 1u, b0 = g * 8;
-    const bool act = b0 < Bp;
-    uint4 c[8];
-    uint4 run = make_uint4(0, 0, 0, 0);  // 8 packed uint16 sums (no carry: a tile has <= 4096 records)
-    if (act) {
-#pragma unroll
-        for (int w = 0; w < 8; ++w) {
-            c[w] = *reinterpret_cast<const uint4*>(cnt + (half * 8 + w) * Bp + b0);
-            // the counts proper: warp_rank_claim leaves a stale lane id in the top bits of a word that lost its last claim
-            c[w].x &= kRankCountMask2; c[w].y &= kRankCountMask2; c[w].z &= kRankCountMask2; c[w].w &= kRankCountMask2;
-        }
-#pragma unroll
-        for (int w = 0; w < 8; ++w) { run.x += c[w].x; run.y += c[w].y; run.z += c[w].z; run.w += c[w].w; }
-    }
-    uint4 other;  // the other half's sums
-    other.x = __shfl_xor_sync(0xFFFFFFFFu, run.x, 1); other.y = __shfl_xor_sync(0xFFFFFFFFu, run.y, 1);
-    other.z = __shfl_xor_sync(0xFFFFFFFFu, run.z, 1); other.w = __shfl_xor_sync(0xFFFFFFFFu, run.w, 1);
-    uint32_t t8[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-    uint32_t mine = 0;
-    if (act) {
-        uint4 e = half ? other : make_uint4(0, 0, 0, 0);  // exclusive prefix over the warps, rewritten in place
-#pragma unroll
-        for (int w = 0; w < 8; ++w) {
-            *reinterpret_cast<uint4*>(cnt + (half * 8 + w) * Bp + b0) = e;
-            e.x += c[w].x; e.y += c[w].y; e.z += c[w].z; e.w += c[w].w;
-        }
-        const uint4 tot = make_uint4(run.x + other.x, run.y + other.y, run.z + other.z, run.w + other.w);
-        t8[0] = tot.x & 0xFFFFu; t8[1] = tot.x >> 16; t8[2] = tot.y & 0xFFFFu; t8[3] = tot.y >> 16;
-        t8[4] = tot.z & 0xFFFFu; t8[5] = tot.z >> 16; t8[6] = tot.w & 0xFFFFu; t8[7] = tot.w >> 16;
-#pragma unroll
-        for (int k = 0; k < 8; ++k) mine += t8[k];
-    }
-    uint32_t total;
-    uint32_t ex = block_excl_scan(half == 0 ? mine : 0u, misc, &total);  // thread 2g+1 receives ex(2g) + mine
-    if (act) {
-        if (half) ex -= mine;
-        // thread 2g writes buckets 8g..8g+3, thread 2g+1 buckets 8g+4..8g+7
-        if (half) ex += t8[0] + t8[1] + t8[2] + t8[3];
-        const uint32_t k0 = half ? 4u : 0u;
-        const uint32_t a0 = half ? t8[4] : t8[0], a1 = half ? t8[5] : t8[1], a2 = half ? t8[6] : t8[2];
-        uint4 ls, gc;
-        ls.x = ex; ls.y = ex + a0; ls.z = ls.y + a1; ls.w = ls.z + a2;
-        gc = half ? make_uint4(grun[4], grun[5], grun[6], grun[7]) : make_uint4(grun[0], grun[1], grun[2], grun[3]);
-        *reinterpret_cast<uint4*>(lstart + b0 + k0) = ls;
-        *reinterpret_cast<uint4*>(gcur + b0 + k0) = gc;
-#pragma unroll
-        for (int k = 0; k < 8; ++k) grun[k] += t8[k];
-    }
-    __syncthreads();
-    return total;
-}
-
 // a warp clears its own row of the counter matrix (only that warp ever touches it outside finish_ranks)
 __device__ __forceinline__ void zero_row(uint16_t* row, uint32_t Bp)
 {
