@@ -349,7 +349,7 @@ def run_ours(args):
     chunks = list(w.chunks())
 
     # inputs: generated once into pinned host memory (the e2e source), copied once to the device (the resident source)
-    host = torch.empty(n * RECORD_BYTES, dtype=torch.uint8).pin_memory()
+    host = torch.empty(n * RECORD_BYTES, dtype=torch.uint8, pin_memory=True)  # pinned from the start: no pageable twin
     W.generate_into(w.gen, first_record, n, host.data_ptr(), threads=os.cpu_count() or 1)
     resident = host.to(dev)
     host_chunks = [host[f * RECORD_BYTES:(f + c) * RECORD_BYTES] for f, c in chunks]

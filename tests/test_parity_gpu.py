@@ -485,7 +485,7 @@ def test_config5_streamed_at_1e8_records_nine_beams():
     w = W.config(5, 100_000_000)
     chunk = W.config(5).chunk_records
     n = w.n_records
-    host = torch.empty(n * 28, dtype=torch.uint8).pin_memory()
+    host = torch.empty(n * 28, dtype=torch.uint8, pin_memory=True)
     W.generate_into(w.gen, 0, n, host.data_ptr(), threads=8)
     r = host.numpy().view(W.RECORD_DTYPE)
     ctx = p.PslContext(w.grid, w.geometry, w.mode, max_records=n, max_chunks=n // chunk + 2)
@@ -614,7 +614,7 @@ def test_index_mid_size_chunks_use_two_table_columns_per_tile():
     import torch
 
     n, chunk = w.n_records, 100_000
-    host = torch.empty(n * 28, dtype=torch.uint8).pin_memory()
+    host = torch.empty(n * 28, dtype=torch.uint8, pin_memory=True)
     W.generate_into(w.gen, 0, n, host.data_ptr(), threads=8)
     dev = host.cuda()
     ctx = p.PslContext(w.grid, w.geometry, w.mode, max_records=n)
