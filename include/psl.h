@@ -197,7 +197,8 @@ psl_status psl_roi_bins(const psl_ctx* ctx, const psl_beam* beam, int32_t bins_o
 typedef struct {
     uint32_t struct_size;  /* sizeof(psl_plan), checked */
     uint32_t n_beams;      /* 1..32 */
-    const psl_beam* beams; /* HOST array of n_beams fields (their fluence maps DEVICE); copied by psl_plan_set */
+    const psl_beam* beams; /* HOST array of n_beams fields, copied by psl_plan_set; their fluence maps are DEVICE
+                              memory of the caller and must stay valid for as long as the plan is sampled from */
     uint64_t n_simulate;   /* N_total^simulated: particles to simulate over all fields */
     uint64_t seed;         /* of the random starts and field assignments; give every GPU of a job its own */
     uint32_t rr_group;     /* particles read from a PSL at a time ("a few"); >= 1 */
