@@ -50,12 +50,12 @@ enum { PSL_EBIN_LINEAR = 0,   /* n_ebins uniform bins on [e_min, e_max] (PAPER.m
 enum { PSL_MEM_PAGEABLE = 0, PSL_MEM_PINNED = 1, PSL_MEM_DEVICE = 2 };
 enum { PSL_OUT_PROJ = 1u,           /* also write xp, yp: the position at the fluence-map plane */
        PSL_DROP_ZERO_WEIGHT = 2u,   /* drop survivors whose final weight is exactly 0 (default: keep) */
-       PSL_NO_COMPACT = 4u,
-       PSL_APR = 8u };              /* INDEX mode: azimuthal particle redistribution (PAPER.md:67-71) of every record
-                                       before it is binned: record i of the load order turns about the beam axis by
-                                       2 pi r / 2^32, r from psl_config.apr_seed and i; position and direction together */       /* diagnostic, same results: ONTHEFLY with <= 256 keys and a rejecting beam takes the
+       PSL_NO_COMPACT = 4u,         /* diagnostic, same results: ONTHEFLY with <= 256 keys and a rejecting beam takes the
                                        two-pass path (histogram, then scatter over all records) instead of compacting
                                        the survivors in the histogram pass; used for A/B runs and tests */
+       PSL_APR = 8u };              /* INDEX mode: azimuthal particle redistribution (PAPER.md:67-71) of every record
+                                       before it is binned: record i of the load order turns about the beam axis by
+                                       2 pi r / 2^32, r from psl_config.apr_seed and i; position and direction together */
 
 /* One phase-space particle: 28 bytes, packed, little-endian.  type: 0 photon, 1 electron, 2 positron.
  * (u, v) are direction cosines; the third one is w = sqrt(1 - u^2 - v^2) > 0 (always downstream). */
