@@ -280,6 +280,34 @@ psl_status psl_profile_enable(psl_ctx* ctx, int32_t on);
 /* Synchronises the stream, returns the totals since the last read (or enable) and clears them. */
 psl_status psl_profile_read(psl_ctx* ctx, psl_profile* out);
 
+/* ---- The one call that allocates nothing ------------------------------------------------------------------------------
+ * For callers that may not call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * it): how many particles every (type, energy, position) bin holds (the P_j of the budgets,
+ * PAPER.md:86-90) -- counts[key] over the valid records inside the grid, key as in psl_batch -- the same numbers
+ * psl_build_batches(ctx, NULL) + psl_get_tables give, without a context and without a workspace.  The scratch of the
+ * histogram kernel (one table column per CTA, the per-CTA statistics, the energy-edge table) lives in ONE array of
+ * PSL_STATIC_SCRATCH_BYTES (2.52 MiB) that is part of the library image: every GPU that loads libpsl_b200.so holds it
+ * until the process exits.  The call makes no cudaMalloc / cudaFree / cudaHostAlloc / stream or event creation; it
+ * enqueues at most five kernels on cfg->stream and returns (it does not synchronise).
+ *
+ *   cfg      read: struct_size, n_types, ebin_mode, n_ebins, e_min, e_max, e_edges, n_xbins, n_ybins, x_min, y_min, dx,
+ *            dy, geom (all checked as by psl_create), device, stream.  Ignored: mode, max_*, flags, apr_seed, workspace*.
+ *   records  DEVICE, n packed psl_record, 4-byte aligned (16-byte aligned buffers take the bulk-copy path); read only
+ *   counts   DEVICE, K = n_types * n_ebins * n_xbins * n_ybins uint32, written in full (zeros when n == 0)
+ *   totals   DEVICE or NULL
+ * Limits (PSL_ERR_CAPACITY beyond them, nothing enqueued): K <= PSL_STATIC_MAX_KEYS, n < 2^32.
+ * Shared state: all calls on a GPU use the same array, which keeps the previous call's contents.  Nothing in it has to
+ * start at zero -- every word a call reads, the same call has written before (columns [0, CTAs) of rows [0, K), the
+ * statistics of those CTAs, the edges [0, n_ebins]) -- so calls one after another on ONE stream need no clearing in
+ * between.  Calls that can overlap on the GPU (different streams without an event between them, or two host threads)
+ * RACE on the array and give wrong counts: order them.  The first call on a device looks up the array's address and
+ * opts the kernels into their shared memory (no allocation either, but make it before a graph capture starts). */
+enum { PSL_STATIC_MAX_KEYS = 2048, PSL_STATIC_SCRATCH_BYTES = 2641152 };
+typedef struct {
+    uint64_t n_in, n_invalid, n_outside_grid, n_binned; /* n_in = n; the three classes add up to it (cf. psl_stats) */
+} psl_count_totals;
+psl_status psl_count_static(const psl_config* cfg, const void* records, uint64_t n, uint32_t* counts, psl_count_totals* totals);
+
 #ifdef __cplusplus
 }
 #endif

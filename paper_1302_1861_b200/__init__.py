@@ -8,11 +8,12 @@ built library or without a CUDA device raises.
 from .binding import (  # noqa: F401
     EBIN_EDGES, EBIN_LINEAR, MEM_DEVICE, MEM_PAGEABLE, MEM_PINNED, MODE_INDEX, MODE_ONTHEFLY, OUT_PROJ,
     DROP_ZERO_WEIGHT, NO_COMPACT, APR, PslContext, PslError, exported_symbols, library_path, load_library, psl_roi_from_jaws,
-    workspace_bytes,
+    workspace_bytes, count_static, STATIC_MAX_KEYS, STATIC_SCRATCH_BYTES,
 )
 
 __all__ = [
     "PslContext", "PslError", "load_library", "library_path", "exported_symbols", "workspace_bytes",
     "psl_roi_from_jaws", "MODE_ONTHEFLY", "MODE_INDEX", "EBIN_LINEAR", "EBIN_EDGES", "MEM_PAGEABLE", "MEM_PINNED",
-    "MEM_DEVICE", "OUT_PROJ", "DROP_ZERO_WEIGHT", "NO_COMPACT", "APR",
+    "MEM_DEVICE", "OUT_PROJ", "DROP_ZERO_WEIGHT", "NO_COMPACT", "APR", "count_static", "STATIC_MAX_KEYS",
+    "STATIC_SCRATCH_BYTES",
 ]

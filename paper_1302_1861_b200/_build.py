@@ -8,7 +8,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libpsl_b200.so")
 SOURCES = ["psl_api.cu"]
-HEADERS = ["psl_device.cuh", "psl_partition.cuh", "psl_bigtile.cuh", "psl_index.cuh", "psl_index_big.cuh", "psl_beam.cuh", "psl_compact.cuh", "psl_plan.cuh", os.path.join("..", "..", "include", "psl.h")]
+HEADERS = ["psl_device.cuh", "psl_partition.cuh", "psl_bigtile.cuh", "psl_index.cuh", "psl_index_big.cuh", "psl_beam.cuh", "psl_compact.cuh", "psl_plan.cuh", "psl_static.cuh", os.path.join("..", "..", "include", "psl.h")]
 
 #: -fmad=false: no FMA contraction anywhere in the TU (the arithmetic contract of include/psl.h);
 #: division and square root stay IEEE (nvcc defaults -prec-div=true -prec-sqrt=true, no fast-math).

@@ -94,6 +94,12 @@ class Flush(C.Structure):
     _fields_ = [("n_events", C.c_uint32), ("key", C.c_void_p), ("first", C.c_void_p), ("count", C.c_void_p)]
 
 
+class CountTotals(C.Structure):
+    _fields_ = [(n, C.c_uint64) for n in ("n_in", "n_invalid", "n_outside_grid", "n_binned")]
+
+
+STATIC_MAX_KEYS, STATIC_SCRATCH_BYTES = 2048, 2641152
+
 K_CLASSES = ("count", "scan", "scatter", "index_a", "index_b", "beam", "other", "count_keys", "sample")
 
 
@@ -167,6 +173,8 @@ def load_library(build: bool = True):
     lib.psl_profile_enable.argtypes = [C.c_void_p, C.c_int32]
     lib.psl_profile_read.restype = C.c_int
     lib.psl_profile_read.argtypes = [C.c_void_p, P(Profile)]
+    lib.psl_count_static.restype = C.c_int
+    lib.psl_count_static.argtypes = [P(Config), C.c_void_p, C.c_uint64, C.c_void_p, C.c_void_p]
     _lib = lib
     return lib
 
@@ -220,6 +228,33 @@ def psl_roi_from_jaws(geometry: Dict, jaws, margin: float):
     out = (C.c_float * 4)()
     rc = lib.psl_roi_from_jaws(C.byref(g), C.byref(b), margin, C.byref(out))
     return rc, tuple(float(v) for v in out)
+
+
+def count_static(grid: Dict, geometry: Dict, records, counts, totals=None, stream=None):
+    """psl_count_static: counts[K] of DEVICE-resident records with no allocation in the library.  ``records`` is a
+    contiguous CUDA tensor of packed 28-byte records, ``counts`` a CUDA int32 tensor of K entries and ``totals`` an
+    optional CUDA int64 tensor of 4 entries (n_in, n_invalid, n_outside_grid, n_binned), all on the same device; the
+    work is enqueued on ``stream`` (default: torch's current stream of that device) and not waited for."""
+    import torch
+
+    lib = load_library()
+    if not (isinstance(records, torch.Tensor) and records.is_cuda and records.is_contiguous()):
+        raise TypeError("records must be a contiguous CUDA tensor")
+    nbytes = records.numel() * records.element_size()
+    assert nbytes % RECORD_BYTES == 0
+    n_keys = grid["n_types"] * grid["n_ebins"] * grid["n_xbins"] * grid["n_ybins"]
+    assert counts.is_cuda and counts.is_contiguous() and counts.dtype == torch.int32 and counts.numel() == n_keys
+    assert counts.device == records.device
+    if totals is not None:
+        assert totals.is_cuda and totals.is_contiguous() and totals.dtype == torch.int64 and totals.numel() == 4
+        assert totals.device == records.device
+    cfg, _edges = make_config(grid, geometry, MODE_ONTHEFLY, 1, 0, device=records.device.index)
+    st = stream if stream is not None else torch.cuda.current_stream(records.device)
+    cfg.stream = st.cuda_stream
+    rc = lib.psl_count_static(C.byref(cfg), records.data_ptr(), nbytes // RECORD_BYTES, counts.data_ptr(),
+                              None if totals is None else totals.data_ptr())
+    if rc != 0:
+        raise PslError(rc, lib.psl_last_error(None).decode())
 
 
 class PslContext:

@@ -11,6 +11,7 @@
 #include <stdio.h>
 #include <string.h>
 
+#include <mutex>
 #include <new>
 #include <utility>
 #include <vector>
@@ -23,6 +24,7 @@
 #include "psl_device.cuh"
 #include "psl_partition.cuh"
 #include "psl_plan.cuh"
+#include "psl_static.cuh"
 
 using namespace psl;
 
@@ -1531,3 +1533,126 @@ psl_status psl_roi_from_jaws(const psl_geometry* g, const psl_beam* beam, float 
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------------------
+// psl_count_static: the entry point that allocates nothing (include/psl.h).  Its scratch is this file-scope array, part
+// of the library image on every GPU that loads it.  In HOST code the name below is only a stand-in for the symbol, not a
+// device address: the address is looked up once per device with cudaGetSymbolAddress (that device current) and the
+// kernels get it as an argument.
+// ---------------------------------------------------------------------------------------------------------------------
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticBytes];
+static_assert(kStaticBytes == PSL_STATIC_SCRATCH_BYTES && kStaticMaxKeys == PSL_STATIC_MAX_KEYS, "psl.h states the limits");
+
+namespace {
+
+struct StaticDev {
+    bool ready = false;
+    uint8_t* scratch = nullptr;  // DEVICE address of g_static_scratch on this device
+    int sms = 0;
+};
+constexpr int kStaticMaxDevices = 64;
+StaticDev g_static_dev[kStaticMaxDevices];
+std::mutex g_static_mu;
+
+using CountStaticFn = void (*)(const uint8_t*, uint32_t, DevGrid, uint32_t, uint32_t*, uint32_t, SegStats*);
+CountStaticFn count_static_fn(bool pos, bool edges)
+{
+    return pos ? (edges ? k_count_static<true, true> : k_count_static<true, false>)
+               : (edges ? k_count_static<false, true> : k_count_static<false, false>);
+}
+
+#define CUS(call)                                                                                       \
+    do {                                                                                                \
+        cudaError_t e_ = (call);                                                                        \
+        if (e_ != cudaSuccess) {                                                                        \
+            set_err(g_err, "psl_count_static: %s failed: %s", #call, cudaGetErrorString(e_));           \
+            return PSL_ERR_CUDA;                                                                        \
+        }                                                                                               \
+    } while (0)
+
+// once per device, with that device current
+psl_status static_setup(int device, StaticDev* out)
+{
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    StaticDev& sd = g_static_dev[device];
+    if (!sd.ready) {
+        void* p = nullptr;
+        CUS(cudaGetSymbolAddress(&p, g_static_scratch));
+        if (!p || (reinterpret_cast<uintptr_t>(p) & (kAlign - 1))) { set_err(g_err, "psl_count_static: bad scratch address"); return PSL_ERR_CUDA; }
+        CUS(cudaDeviceGetAttribute(&sd.sms, cudaDevAttrMultiProcessorCount, device));
+        // the most dynamic shared memory any configuration takes: three stages, a 16 KB histogram, 1025 edges
+        const uint32_t smem_max = count_layout(kTile * kRecBytes, kStagesCount, kStaticMaxKeys, kStaticMaxEdges).total;
+        for (int v = 0; v < 4; ++v) CUS(allow_smem(count_static_fn((v & 1) != 0, (v & 2) != 0), smem_max));
+        sd.scratch = static_cast<uint8_t*>(p);
+        sd.ready = true;
+    }
+    *out = sd;
+    return PSL_OK;
+}
+
+}  // namespace
+
+extern "C" psl_status psl_count_static(const psl_config* cfg, const void* records, uint64_t n, uint32_t* counts, psl_count_totals* totals)
+{
+    static_assert(sizeof(psl_count_totals) == sizeof(CountTotals), "psl_count_totals layout");
+    if (!cfg) { set_err(g_err, "psl_count_static: config is NULL"); return PSL_ERR_ARG; }
+    if (cfg->struct_size != sizeof(psl_config)) { set_err(g_err, "config.struct_size %u != %zu", cfg->struct_size, sizeof(psl_config)); return PSL_ERR_ARG; }
+    if (n >= (1ull << 32)) { set_err(g_err, "psl_count_static: %llu records; one call takes fewer than 2^32", (unsigned long long)n); return PSL_ERR_CAPACITY; }
+    if (cfg->n_types >= 1 && cfg->n_ebins >= 1 && cfg->n_xbins >= 1 && cfg->n_ybins >= 1) {
+        const uint64_t K64 = (uint64_t)cfg->n_types * (uint64_t)cfg->n_ebins * (uint64_t)cfg->n_xbins * (uint64_t)cfg->n_ybins;
+        if (K64 > kStaticMaxKeys) {
+            set_err(g_err, "psl_count_static: %llu keys; the static scratch holds at most %u (use a context in PSL_MODE_INDEX)",
+                    (unsigned long long)K64, kStaticMaxKeys);
+            return PSL_ERR_CAPACITY;
+        }
+    }
+    psl_config c = *cfg;  // the grid checks of psl_create, on a configuration that asks for nothing else
+    c.mode = PSL_MODE_ONTHEFLY;
+    c.max_records = n ? n : 1;
+    c.max_host_records = 0;
+    c.max_beam_records = 0;
+    c.max_chunks = 1;
+    c.flags = 0;
+    c.max_launch_records = 0;
+    Derived d;
+    psl_status s = derive(&c, &d, g_err);
+    if (s != PSL_OK) return s;
+    if (!counts) { set_err(g_err, "psl_count_static: counts is NULL"); return PSL_ERR_ARG; }
+    if (n != 0 && (!records || (reinterpret_cast<uintptr_t>(records) & 3u))) { set_err(g_err, "psl_count_static: records must be a 4-byte aligned DEVICE pointer"); return PSL_ERR_ARG; }
+    if (cfg->device < 0 || cfg->device >= kStaticMaxDevices) { set_err(g_err, "psl_count_static: config.device"); return PSL_ERR_ARG; }
+    CUS(cudaSetDevice(cfg->device));
+    StaticDev sd;
+    s = static_setup(cfg->device, &sd);
+    if (s != PSL_OK) return s;
+
+    cudaStream_t stream = static_cast<cudaStream_t>(cfg->stream);
+    float* dev_edges = reinterpret_cast<float*>(sd.scratch + kStaticEdgesOff);
+    SegStats* ss = reinterpret_cast<SegStats*>(sd.scratch + kStaticStatsOff);
+    uint32_t* table = reinterpret_cast<uint32_t*>(sd.scratch + kStaticTableOff);
+    const bool edges = cfg->ebin_mode == PSL_EBIN_EDGES;
+    const uint32_t nt = (uint32_t)((n + kTile - 1) / kTile);
+    uint32_t S = 2u * (uint32_t)sd.sms;  // two resident CTAs per SM: one wave
+    if (S > kStaticMaxCols) S = kStaticMaxCols;
+    if (S > nt) S = nt;
+    if (S != 0) {
+        if (edges) {
+            const uint32_t ne = (uint32_t)cfg->n_ebins + 1u;
+            for (uint32_t f = 0; f < ne; f += 512) {
+                EdgeBatch eb;
+                const uint32_t m = ne - f < 512u ? ne - f : 512u;
+                memcpy(eb.e, cfg->e_edges + f, m * sizeof(float));
+                k_static_edges<<<1, 256, 0, stream>>>(dev_edges, eb, f, m);
+                CUS(cudaGetLastError());
+            }
+        }
+        const DevGrid grid = make_grid(c, d, dev_edges);
+        const uint32_t smem = count_layout(kTile * kRecBytes, kStagesCount, d.K, (uint32_t)cfg->n_ebins + 1u).total;
+        count_static_fn(grid.has_pos != 0, edges)<<<S, kThreads, smem, stream>>>(static_cast<const uint8_t*>(records), (uint32_t)n, grid, d.K,
+                                                                                table, kStaticMaxCols, ss);
+        CUS(cudaGetLastError());
+    }
+    k_static_sum<<<(d.K + 7) / 8 + 1, 256, 0, stream>>>(table, kStaticMaxCols, S, d.K, ss, (unsigned long long)n, counts,
+                                                        reinterpret_cast<CountTotals*>(totals));
+    CUS(cudaGetLastError());
+    return PSL_OK;
+}

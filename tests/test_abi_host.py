@@ -14,7 +14,7 @@ def test_library_loads_and_exports_every_declared_symbol():
     lib = P.load_library()
     names = P.exported_symbols()
     assert {"psl_create", "psl_load_chunk", "psl_build_batches", "psl_get_batch"} <= set(names)  # north_star's four
-    assert len(names) == 20
+    assert len(names) == 21
     for n in names:
         assert hasattr(lib, n), n
 
@@ -25,10 +25,10 @@ def test_struct_layouts_match_the_header():
     import tempfile
 
     root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
-    prog = ('#include <stdio.h>\n#include <stddef.h>\n#include "psl.h"\nint main(){printf("%zu %zu %zu %zu %zu %zu %zu %zu %zu %zu %zu\\n",'
+    prog = ('#include <stdio.h>\n#include <stddef.h>\n#include "psl.h"\nint main(){printf("%zu %zu %zu %zu %zu %zu %zu %zu %zu %zu %zu %zu\\n",'
             'sizeof(psl_config),sizeof(psl_beam),sizeof(psl_stats),sizeof(psl_batch),sizeof(psl_record),'
             'offsetof(psl_config,workspace),offsetof(psl_beam,mu_weight),sizeof(psl_plan),sizeof(psl_launch),sizeof(psl_flush),'
-            'offsetof(psl_plan,phantom_lo));return 0;}')
+            'offsetof(psl_plan,phantom_lo),sizeof(psl_count_totals));return 0;}')
     with tempfile.TemporaryDirectory() as d:
         open(os.path.join(d, "s.c"), "w").write(prog)
         subprocess.run(["gcc", "-I", os.path.join(root, "include"), os.path.join(d, "s.c"), "-o", os.path.join(d, "s")],
@@ -36,7 +36,7 @@ def test_struct_layouts_match_the_header():
         sizes = [int(v) for v in subprocess.run([os.path.join(d, "s")], capture_output=True, text=True).stdout.split()]
     assert sizes == [C.sizeof(B.Config), C.sizeof(B.Beam), C.sizeof(B.Stats), C.sizeof(B.Batch), 28,
                      B.Config.workspace.offset, B.Beam.mu_weight.offset, C.sizeof(B.Plan), C.sizeof(B.Launch), C.sizeof(B.Flush),
-                     B.Plan.phantom_lo.offset]
+                     B.Plan.phantom_lo.offset, C.sizeof(B.CountTotals)]
     w = W.config(2)
     cfg, _ = B.make_config(w.grid, w.geometry, w.mode, 1000)
     cfg.struct_size = 8  # a stale header must be rejected
