@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the phase-space source hot path on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl ours|reference] [--verify]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl ours|reference] [--verify] [--variant 5b]
 
 One "step" is one pass of the whole hot path over one synthetic
 phase-space: psl_reset -> psl_load_chunk x n -> psl_build_batches per beam (INDEX mode: the first build also
@@ -59,6 +59,9 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-next", action="store_true", help="skip the section-8(f) phase lines (sampling layer / shipments)")
+    ap.add_argument("--variant", choices=["5a", "5b"], default="5a",
+                    help="config 5 only: 5a = stream once, index on the device, nine beam builds (the default); 5b = "
+                         "SURVEY 8(d)'s literal per-beam re-stream of the whole phase-space from pinned host memory")
     ap.add_argument("--verify", action="store_true",
                     help="after the timed regions, check the full-size result against the oracle (streaming counts)")
     return ap.parse_args()
@@ -619,6 +622,115 @@ def run_ours(args):
     return 0
 
 
+def run_restream(args):
+    """--variant 5b: no index is kept; for EVERY beam the whole phase-space is streamed
+    again from pinned host memory in the configuration's chunks ("copied in chunks") and that beam's
+    batches are built on the fly from the chunks -- jaws, fluence map, MU weight, stable (type, energy) order; keys have
+    no position part, the jaw test is the cull.  The synthetic stream is not position-sorted, so no chunk can be
+    skipped as a whole: all 105 chunks cross the host link for each of the nine beams (252 GB per step), which is the
+    bound.  One GPU; the value IS the end-to-end value (there is no resident input in this variant)."""
+    import torch
+
+    import paper_1302_1861_b200 as P
+    import workloads as W
+
+    if int(os.environ.get("WORLD_SIZE", "1")) != 1:
+        raise SystemExit("bench.py --variant 5b: one GPU")
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- libpsl_b200 has no CPU path")
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(0)
+    w = W.config(5, args.records or None)
+    if args.records and W.config(5).chunk_records < args.records:
+        w.chunk_records = W.config(5).chunk_records
+    n = w.n_records
+    chunks = list(w.chunks())
+    grid = dict(w.grid, n_xbins=1, n_ybins=1, x_min=-20.0, y_min=-20.0, dx=40.0, dy=40.0)
+    host = torch.empty(n * RECORD_BYTES, dtype=torch.uint8, pin_memory=True)
+    W.generate_into(w.gen, 0, n, host.data_ptr(), threads=os.cpu_count() or 1)
+    host_chunks = [host[f * RECORD_BYTES:(f + c) * RECORD_BYTES] for f, c in chunks]
+    ctx = P.PslContext(grid, w.geometry, P.MODE_ONTHEFLY, max_records=n, max_host_records=n, max_chunks=len(chunks) + 1,
+                       flags=w.flags, device=0)
+    beams = [ctx.beam(dict(b, roi=None)) for b in w.beams]
+    K = grid["n_types"] * grid["n_ebins"]
+    h_counts = torch.empty(K, dtype=torch.int32).pin_memory()
+    h_offsets = torch.empty(K + 1, dtype=torch.int32).pin_memory()
+
+    def step():
+        surv = []
+        for b in beams:
+            ctx.reset()
+            for c in host_chunks:
+                ctx.load_chunk(c)
+            ctx.build_batches(b)
+            counts, offsets = ctx.get_tables()
+            h_counts.copy_(counts, non_blocking=True)
+            h_offsets.copy_(offsets, non_blocking=True)
+            surv.append(ctx.get_stats()["n_survivors"])  # synchronises: the beam's result is on the host
+        return surv
+
+    land = torch.empty(max(c for _, c in chunks) * RECORD_BYTES, dtype=torch.uint8, device=dev)
+    for _ in range(2):  # the host-link ceiling: plain pinned copies of the same chunks, same run
+        torch.cuda.synchronize()
+        c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        c0.record()
+        for hc in host_chunks:
+            land[:hc.numel()].copy_(hc, non_blocking=True)
+        c1.record()
+        torch.cuda.synchronize()
+        h2d_peak = n * RECORD_BYTES / (c0.elapsed_time(c1) * 1e-3) / 1e9
+    del land
+    sampler = ClockSampler(0)
+    sampler.start()
+    surv = step()  # one step of warm-up is nine full streams
+    steps = max(1, min(args.steps, 3))
+    l0 = ctx.kernel_launches()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler.region(True)
+    e0.record()
+    for _ in range(steps):
+        surv = step()
+    e1.record()
+    torch.cuda.synchronize()
+    sampler.region(False)
+    ms = e0.elapsed_time(e1)
+    launches = ctx.kernel_launches() - l0
+    # the device side alone, brackets on: one beam's build over the chunks already in the landing zone
+    ctx.profile_enable(True)
+    ctx.profile_read()
+    ctx.build_batches(beams[-1])
+    prof = {k: v[0] for k, v in ctx.profile_read().items() if v[1]}
+    ctx.profile_enable(False)
+    clocks = sampler.finish()
+    peak, peak_src = measured_peaks()
+    h2d = len(beams) * n * RECORD_BYTES
+    value = n * steps / (ms * 1e-3)
+    cfg = describe(w, 1)
+    cfg.update(variant="5b", keys=K, mode="onthefly", position_bins=[1, 1],
+               l2_policy="every beam re-streams %.0f GB from pinned host memory" % (n * RECORD_BYTES / 1e9))
+    count_gbs = RECORD_BYTES * n / (prof.get("count", 0.0) * 1e-3) / 1e9 if prof.get("count") else None
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": 1, "steps": steps, "warmup": 1, "ms_per_step": ms / steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": cfg, "workload_stats": {"survivors_per_beam": surv, "chunks_skipped": 0}, "clocks": clocks,
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": h2d,
+                "d2h_bytes_per_step": len(beams) * ((2 * K + 1) * 4 + (K + 1) * 4 + 64),
+                "h2d_gbs": h2d * steps / (ms * 1e-3) / 1e9, "h2d_peak_gbs": h2d_peak,
+                "h2d_frac": h2d * steps / (ms * 1e-3) / 1e9 / h2d_peak,
+                "source": "pinned host memory, %d chunk(s) x %d beams per step through psl_load_chunk(PSL_MEM_PINNED)"
+                          % (len(chunks), len(beams))},
+        "gpu_launches": int(launches),
+        "per_phase": {"device_build_ms_one_beam": prof, "note": "kernel classes of one beam's build over the landed chunks"},
+        "roofline": {"bound": "hbm", "kernel": "count", "achieved": count_gbs, "peak": peak, "unit": "GB/s",
+                     "frac": None if count_gbs is None else count_gbs / peak, "peak_source": peak_src, "traffic": None,
+                     "note": "the step itself is bound by the host link (e2e.h2d_frac), not by this kernel"},
+    }
+    print(json.dumps(line))
+    ctx.destroy()
+    return 0
+
+
 def run_verify(ctx, w, host, beams, step, host_chunks):
     """--verify (outside every timed region): the full-size result of the configuration bench.py times, against
     the oracle.  The oracle classifies every record (all host cores, each on its own shard; no sort, no oracle
@@ -682,6 +794,8 @@ def main():
     args = parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.variant == "5b":
+        return run_restream(args)
     return run_ours(args)
 
 

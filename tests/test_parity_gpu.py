@@ -527,6 +527,59 @@ def test_config5_at_its_real_size_through_bench_verify():
     assert v["ok"] and len(v["builds"]) == 10 and all(b["ok"] for b in v["builds"]), v
 
 
+def test_config5_variant_5b_restream_selects_what_the_index_route_selects():
+    """no index; every beam re-streams the chunks from host memory and is built on the fly with
+    (type, energy) keys.  Against the oracle element by element, and against the index route (5a): the index route's
+    survivors are exactly the re-stream's survivors that lie in the position bins the beam's ROI selects (the ROI is a
+    margin, PAPER.md:80: a few scattered particles outside it would still have passed the jaws), with the same weights;
+    only the order inside a (type, energy) batch differs (load order here, PSL order there)."""
+    w = W.config(5, 400_000)
+    r = w.records()
+    g = w.grid
+    grid = dict(g, n_xbins=1, n_ybins=1, x_min=-20.0, y_min=-20.0, dx=40.0, dy=40.0)
+    w_otf = W.Workload("cfg5b", w.n_records, w.gen, 0, grid, geometry=w.geometry)
+    idx = run_library(w, r, None, chunk=w.chunk_records, mem="pinned")
+    otf = None
+    orc = O.Oracle(grid, w.geometry)
+    cut = 0
+    for beam in w.beams[:4]:
+        idx.build_batches(beam)
+        a = library_result(idx)
+        otf = run_library(w_otf, r, dict(beam, roi=None), chunk=w.chunk_records, mem="pinned", ctx=otf)
+        b = library_result(otf)
+        assert_matches_oracle(b, orc.build(r, dict(beam, roi=None)))
+        rx0, rx1, ry0, ry1 = idx.roi_bins(beam)
+        ix = np.floor(b["x"] * np.float32(1.0 / g["dx"])).astype(np.int64) - int(round(g["x_min"] / g["dx"]))
+        iy = np.floor(b["y"] * np.float32(1.0 / g["dy"])).astype(np.int64) - int(round(g["y_min"] / g["dy"]))
+        sel = (rx0 <= ix) & (ix <= rx1) & (ry0 <= iy) & (iy <= ry1)
+        cut += int((~sel).sum())
+        assert 0 < a["n_survivors"] == int(sel.sum()) and (~sel).sum() < 0.002 * len(sel)
+        ia, ib = np.argsort(a["src_index"]), np.argsort(b["src_index"][sel])
+        assert np.array_equal(a["src_index"][ia], b["src_index"][sel][ib])
+        for f in ("E", "x", "y", "u", "v", "w", "wt"):
+            assert np.array_equal(a[f][ia].view(np.uint32), b[f][sel][ib].view(np.uint32)), f
+        otf.reset()
+    assert cut > 0  # the case exists at this size: the two routes are NOT the same set, by the method's design
+    idx.destroy()
+    otf.destroy()
+
+
+def test_bench_variant_5b_runs_at_reduced_size():
+    import json
+    import os
+    import subprocess
+    import sys
+
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    run = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--config", "5", "--variant", "5b", "--records",
+                          "20000000", "--steps", "1"], capture_output=True, text=True, timeout=900)
+    assert run.returncode == 0, run.stderr[-2000:]
+    line = json.loads(run.stdout.strip().splitlines()[-1])
+    assert line["config"]["variant"] == "5b" and line["config"]["beams"] == 9 and line["gpu_launches"] > 0
+    assert line["e2e"]["h2d_bytes_per_step"] == 9 * 20_000_000 * 28 and 0.3 < line["e2e"]["h2d_frac"] <= 1.05
+    assert len(line["workload_stats"]["survivors_per_beam"]) == 9 and min(line["workload_stats"]["survivors_per_beam"]) > 0
+
+
 # ---------------------------------------------------------------------------------------------
 # x/y-asymmetric configurations: n_xbins != n_ybins, dx != dy, x_min != y_min, z_jaw_x != z_jaw_y != z_map,
 # map_nx != map_ny, map_dx != map_dy, map_x0 != map_y0 (every other case in this file is symmetric in x and y, so a
