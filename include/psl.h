@@ -18,6 +18,8 @@
  *   - Errors are return codes; nothing aborts, nothing throws, and a call that fails leaves the
  *     context as it was before the call.  psl_last_error() gives a one-line description.
  *   - A context is not thread-safe.  Total records per context < 2^32.
+ *   - Every call that touches the device makes psl_config.device the calling thread's current CUDA device and leaves
+ *     it current.
  *
  * Arithmetic contract: every expression that decides a bin, a key, the jaw
  * predicate or a map pixel is evaluated in fp32, one IEEE-754 round-to-nearest operation at a
