@@ -106,7 +106,8 @@ typedef struct {
     int32_t has_roi;                      /* INDEX mode only */
     float roi_x1, roi_x2, roi_y1, roi_y2; /* rectangle at z_plane */
     float mu_weight;                      /* MU_i / MU_total */
-    float gantry_deg, coll_deg, couch_deg; /* carried as metadata only */
+    float gantry_deg, coll_deg, couch_deg; /* the field's rotations: used by psl_sample_batch, ignored by
+                                              psl_build_batches (whose batches stay in the beam's-eye-view frame) */
 } psl_beam;
 
 /* Every record loaded is counted in exactly one of the six n_* classes below (tested in this order). */
