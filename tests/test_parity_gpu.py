@@ -707,3 +707,57 @@ def test_roi_far_outside_the_grid_is_empty_and_fast():
         assert_matches_oracle(library_result(ctx), O.Oracle(w.grid, w.geometry).build(w.records(), beam))
     assert time.perf_counter() - t0 < 5.0
     ctx.destroy()
+
+
+# ---------------------------------------------------------------------------------------------
+# skewed key distributions: the ranking inside a tile is built for ~1000 buckets hit at random; these inputs put whole
+# tiles into one bucket, alternate between two, or arrive already sorted / reverse sorted
+# ---------------------------------------------------------------------------------------------
+def _skewed(w, kind, n=300_001, seed=11):
+    r = W.generate(W.GenParams(seed), 0, n)
+    rng = np.random.default_rng(seed)
+    if kind == "one_key":
+        r["type"][:] = 0
+        r["E"][:] = np.float32(1.2345)
+        r["x"][:] = np.float32(0.26)
+        r["y"][:] = np.float32(-0.74)
+    elif kind == "two_keys_alternating":
+        r["type"][:] = np.arange(n) % 2
+        r["E"][:] = np.where(np.arange(n) % 2 == 0, np.float32(0.3), np.float32(5.9))
+        r["x"][:] = np.where(np.arange(n) % 2 == 0, np.float32(-19.9), np.float32(19.9))
+        r["y"][:] = np.where(np.arange(n) % 2 == 0, np.float32(-19.9), np.float32(19.9))
+    elif kind == "hot_bin":
+        hot = rng.random(n) < 0.9
+        r["type"][hot] = 0
+        r["E"][hot] = np.float32(0.51)
+        r["x"][hot] = rng.uniform(1.0, 1.49, int(hot.sum())).astype(np.float32)
+        r["y"][hot] = rng.uniform(2.0, 2.49, int(hot.sum())).astype(np.float32)
+    elif kind in ("sorted", "reverse_sorted"):
+        cls, keys = O.Oracle(w.grid, w.geometry).classify(r, None)
+        order = np.argsort(np.where(cls == O.SURVIVOR, keys, -1), kind="stable")
+        r = r[order[::-1] if kind == "reverse_sorted" else order].copy()
+    return r
+
+
+@pytest.mark.parametrize("kind", ["one_key", "two_keys_alternating", "hot_bin", "sorted", "reverse_sorted"])
+def test_skewed_key_distributions_index(kind):
+    w = W.config(4, 300_001)
+    r = _skewed(w, kind)
+    ctx = run_library(w, r, None, chunk=100_000)
+    orc = O.Oracle(w.grid, w.geometry)
+    assert_matches_oracle(library_result(ctx), orc.build(r, None), index_only=True)
+    ctx.build_batches(w.beams[0])
+    assert_matches_oracle(library_result(ctx), orc.build(r, w.beams[0]))
+    ctx.destroy()
+
+
+@pytest.mark.parametrize("kind", ["one_key", "two_keys_alternating", "hot_bin", "sorted", "reverse_sorted"])
+@pytest.mark.parametrize("cfg", [2, 3])
+def test_skewed_key_distributions_onthefly(kind, cfg):
+    w = W.config(cfg, 300_001)
+    r = _skewed(w, kind)
+    check(w, r, w.beams[0], chunk=100_000)
+    wide = W.Workload("otf_pos", w.n_records, w.gen, w.mode,  # 1536 keys: the 1024-record-tile scatter
+                      W._grid(n_types=3, n_ebins=8, n_xbins=8, n_ybins=8, x_min=-20.0, y_min=-20.0, dx=5.0, dy=5.0),
+                      geometry=w.geometry)
+    check(wide, r, w.beams[0], chunk=100_000)
