@@ -353,7 +353,8 @@ def run_ours(args):
 
     # inputs: generated once into pinned host memory (the e2e source), copied once to the device (the resident source)
     host = torch.empty(n * RECORD_BYTES, dtype=torch.uint8, pin_memory=True)  # pinned from the start: no pageable twin
-    W.generate_into(w.gen, first_record, n, host.data_ptr(), threads=os.cpu_count() or 1)
+    # every rank generates its own shard: share the host cores between the ranks of the node
+    W.generate_into(w.gen, first_record, n, host.data_ptr(), threads=max(1, (os.cpu_count() or 1) // world))
     resident = host.to(dev)
     host_chunks = [host[f * RECORD_BYTES:(f + c) * RECORD_BYTES] for f, c in chunks]
     dev_chunks = [resident[f * RECORD_BYTES:(f + c) * RECORD_BYTES] for f, c in chunks]
