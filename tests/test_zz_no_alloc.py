@@ -133,3 +133,33 @@ def test_limits_are_rejected_with_a_clear_error():
     assert lib.psl_count_static(C.byref(cfg), dev.data_ptr(), 1024, c.data_ptr(), None) == 1  # psl_create's checks
     torch.cuda.synchronize()
     assert int(c.sum()) == 0  # a rejected call enqueues nothing
+
+
+def test_the_call_can_be_captured_into_a_cuda_graph():
+    """what the entry point is for: under stream capture nothing may allocate or synchronise.  Captured once (after a
+    first, uncaptured call has done the per-device set-up), replayed on new contents of the same buffers."""
+    import torch
+
+    import paper_1302_1861_b200 as P
+
+    grid = _grids()["pos_edges_2048"]
+    geom = W.config(2).geometry
+    n = 200_003
+    ra = dirty(W.generate(W.GenParams(4401), 0, n), 1)
+    rb = dirty(W.generate(W.GenParams(4402, half_x=6.0, half_y=6.0), 0, n), 2)
+    dev = _device_records(torch, ra)
+    counts = torch.full((2048,), -1, dtype=torch.int32, device="cuda")
+    totals = torch.full((4,), -1, dtype=torch.int64, device="cuda")
+    P.count_static(grid, geom, dev, counts, totals)  # set-up happens here, outside the capture
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        P.count_static(grid, geom, dev, counts, totals)  # enqueued on the capturing stream (torch's current stream)
+    for r in (ra, rb, ra):
+        dev.copy_(torch.from_numpy(np.ascontiguousarray(r).view(np.uint8).reshape(-1).copy()))
+        counts.fill_(-1)
+        g.replay()
+        torch.cuda.synchronize()
+        ref, st = _existing_path(P, grid, geom, dev, n)
+        assert torch.equal(counts, ref)
+        assert totals.tolist() == [n, st["n_invalid"], st["n_outside_grid"], st["n_survivors"]]
